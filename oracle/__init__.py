@@ -1,0 +1,140 @@
+"""ctypes binding of the CPU oracle (oracle/oracle.c).  TEST INFRASTRUCTURE, not the product.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+may import this package.  It does not import paper_2603_24508_b200 and shares no code with
+the CUDA path.  All arrays are numpy, host memory, modified in place where the C routine
+does so.
+"""
+import ctypes as C
+
+import numpy as np
+
+from . import build as _build
+
+PERIODIC = 0
+ABSORBING = 1
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        dp, ip, u64p = C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_uint64)
+        i64p = C.POINTER(C.c_int64)
+        _lib.oracle_boris_constants.argtypes = [C.c_double, C.c_double, C.c_double, dp, dp]
+        _lib.oracle_boris_constants.restype = None
+        _lib.oracle_push.argtypes = [C.c_int64, dp, dp, dp, dp, ip, C.c_int32, C.c_double, C.c_double,
+                                     C.c_int32, dp, C.c_double, dp, u64p]
+        _lib.oracle_push.restype = C.c_int
+        _lib.oracle_arrange.argtypes = [C.c_int64, dp, dp, dp, dp, ip, dp, dp, dp, dp, ip, C.c_int32, ip, ip]
+        _lib.oracle_arrange.restype = C.c_int64
+        _lib.oracle_run.argtypes = [C.c_int32, C.c_int32, i64p, i64p, dp, dp, dp, dp, ip, dp, dp, dp, dp, ip,
+                                    C.c_int32, C.c_double, C.c_double, C.c_int32, dp, C.c_double, dp, u64p,
+                                    ip, ip]
+        _lib.oracle_run.restype = C.c_int
+    return _lib
+
+
+def _d(a):
+    assert a.dtype == np.float64 and a.flags.c_contiguous
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _i(a):
+    assert a.dtype == np.int32 and a.flags.c_contiguous
+    return a.ctypes.data_as(C.POINTER(C.c_int32))
+
+
+def boris_constants(qm, dt, dx, B):
+    """-> dict h, t(3), s(3), inv_dx  (oracle_boris_constants)."""
+    Bv = np.ascontiguousarray(B, dtype=np.float64)
+    out = np.zeros(8)
+    lib().oracle_boris_constants(qm, dt, dx, _d(Bv), _d(out))
+    return {"h": out[0], "t": out[1:4].copy(), "s": out[4:7].copy(), "inv_dx": out[7]}
+
+
+class State:
+    """Host-side species state driven by the oracle: x, vx, vy, vz (f64), cell (i32), n."""
+
+    def __init__(self, x, vx, vy, vz, cell, *, nc, dx, dt, boundary, E, qm, B, arrange_every=0):
+        self.cap = len(x)
+        self.x = np.array(x, dtype=np.float64)
+        self.vx = np.array(vx, dtype=np.float64)
+        self.vy = np.array(vy, dtype=np.float64)
+        self.vz = np.array(vz, dtype=np.float64)
+        self.cell = np.array(cell, dtype=np.int32)
+        self.n = self.cap
+        self.nc, self.dx, self.dt, self.boundary, self.qm = int(nc), float(dx), float(dt), int(boundary), float(qm)
+        self.E = np.ascontiguousarray(E, dtype=np.float64)
+        assert self.E.shape == (self.nc + 1,)
+        self.B = np.ascontiguousarray(B, dtype=np.float64)
+        self.arrange_every = int(arrange_every)
+        self.steps = 0
+        self.wall = np.zeros(2, dtype=np.uint64)
+        self.count = np.zeros(self.nc, dtype=np.int32)
+        self.offset = np.zeros(self.nc + 1, dtype=np.int32)
+        self._tmp = None
+
+    def _tmpbufs(self):
+        if self._tmp is None:
+            self._tmp = [np.empty(self.cap), np.empty(self.cap), np.empty(self.cap), np.empty(self.cap),
+                         np.empty(self.cap, dtype=np.int32)]
+        return self._tmp
+
+    def push(self, nsteps=1):
+        """nsteps mover steps with the arrange_every rule (oracle_run)."""
+        t = self._tmpbufs()
+        steps = C.c_int64(self.steps)
+        n = C.c_int64(self.n)
+        rc = lib().oracle_run(nsteps, self.arrange_every, C.byref(steps), C.byref(n),
+                              _d(self.x), _d(self.vx), _d(self.vy), _d(self.vz), _i(self.cell),
+                              _d(t[0]), _d(t[1]), _d(t[2]), _d(t[3]), _i(t[4]),
+                              self.nc, self.dx, self.dt, self.boundary, _d(self.E), self.qm, _d(self.B),
+                              self.wall.ctypes.data_as(C.POINTER(C.c_uint64)), _i(self.count), _i(self.offset))
+        if rc:
+            raise RuntimeError(f"oracle_run failed rc={rc}")
+        self.steps, self.n = steps.value, n.value
+
+    def push_only(self):
+        """one bare mover step, no arrange, over slots [0,n) (oracle_push)."""
+        rc = lib().oracle_push(self.n, _d(self.x), _d(self.vx), _d(self.vy), _d(self.vz), _i(self.cell),
+                               self.nc, self.dx, self.dt, self.boundary, _d(self.E), self.qm, _d(self.B),
+                               self.wall.ctypes.data_as(C.POINTER(C.c_uint64)))
+        if rc:
+            raise RuntimeError(f"oracle_push failed rc={rc}")
+        self.steps += 1
+
+    def arrange(self):
+        """explicit arrange (oracle_arrange); does not touch the step counter."""
+        t = self._tmpbufs()
+        nl = lib().oracle_arrange(self.n, _d(self.x), _d(self.vx), _d(self.vy), _d(self.vz), _i(self.cell),
+                                  _d(t[0]), _d(t[1]), _d(t[2]), _d(t[3]), _i(t[4]), self.nc,
+                                  _i(self.count), _i(self.offset))
+        if nl < 0:
+            raise RuntimeError("oracle_arrange failed")
+        for dst, src in zip((self.x, self.vx, self.vy, self.vz, self.cell), t):
+            dst[:nl] = src[:nl]
+        self.n = int(nl)
+
+    def live(self):
+        """the five arrays over [0,n)."""
+        n = self.n
+        return self.x[:n], self.vx[:n], self.vy[:n], self.vz[:n], self.cell[:n]
+
+
+def arrange_arrays(x, vx, vy, vz, cell, nc):
+    """Pure function form of oracle_arrange -> (xo, vxo, vyo, vzo, cello, count, offset, n_live)."""
+    n = len(x)
+    a = [np.ascontiguousarray(v, dtype=np.float64) for v in (x, vx, vy, vz)]
+    c = np.ascontiguousarray(cell, dtype=np.int32)
+    o = [np.zeros(n) for _ in range(4)]
+    co = np.full(n, -7, dtype=np.int32)
+    count = np.zeros(nc, dtype=np.int32)
+    offset = np.zeros(nc + 1, dtype=np.int32)
+    nl = lib().oracle_arrange(n, _d(a[0]), _d(a[1]), _d(a[2]), _d(a[3]), _i(c), _d(o[0]), _d(o[1]), _d(o[2]),
+                              _d(o[3]), _i(co), nc, _i(count), _i(offset))
+    if nl < 0:
+        raise RuntimeError("oracle_arrange failed")
+    return o[0][:nl], o[1][:nl], o[2][:nl], o[3][:nl], co[:nl], count, offset, int(nl)
