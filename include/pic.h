@@ -1,0 +1,194 @@
+/*
+ * pic.h -- C ABI of libpic: the BIT1-style particle mover + arranger on one B200.
+ *
+ * What the calls compute (citations are PAPER.md lines of arxiv/paper_2603_24508; the
+ * paper prints no equations for these routines, so the concrete scheme is the one fixed
+ * in DESIGN.md section 3, "arithmetic contract"):
+ *
+ *   pic_push     the particle mover, phases (i)+(iv) of the PIC cycle (the
+ *                grey box of Fig. 1; `move0`/`moveb`): linear
+ *                (cloud-in-cell) gather of E_x from the 1D node grid, Boris velocity
+ *                update in a uniform B, x advance, periodic wrap or absorbing-wall flag
+ *                ("plasma is absorbed at the walls"), new cell index.
+ *   pic_arrange  the arranger `arrj`, "a sorting function" that restores
+ *                the per-cell grouping ("natural sorting"), together
+ *                with the particle removal `rempar2`: a STABLE counting
+ *                sort of the live particles by cell; absorbed particles are dropped.
+ *   pic_wall_flux per-wall absorbed-particle counters.
+ *
+ * Memory model (allocate once, keep resident, release at the end;
+ * kernels take raw device pointers).  The CALLER owns every large device
+ * array (the two particle buffer sets and the workspace; normally torch tensors) and
+ * keeps them alive and untouched until pic_destroy.  The library owns the handle and
+ * small device objects (E copy, per-cell count/offset, counters).  HOST pointers are
+ * copied during the call and never retained.  Every pointer below says HOST or DEVICE.
+ *
+ * All functions return PIC_OK (0) or a negative pic_status; nothing throws or aborts.
+ * Work is enqueued on the stream given at pic_create; calls documented "syncs" wait for
+ * it.  One host thread per pic_sim.  There is no CPU fallback: without a CUDA device
+ * every compute entry point fails with PIC_ECUDA.
+ */
+#ifndef PIC_H_
+#define PIC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    PIC_OK = 0,
+    PIC_EINVAL = -1,    /* NULL / non-finite / out-of-range argument */
+    PIC_ENOMEM = -2,    /* host or device allocation failed */
+    PIC_ECUDA = -3,     /* CUDA runtime error (text via pic_last_error) */
+    PIC_ECAPACITY = -4, /* n > capacity, or workspace too small */
+    PIC_ESTATE = -5     /* call not valid in the current state (see each call) */
+} pic_status;
+
+typedef enum { PIC_PERIODIC = 0, PIC_ABSORBING = 1 } pic_boundary;
+
+/* The 1D grid: nc cells of width dx, nodes j = 0..nc at x_j = j*dx, domain [0, L),
+ * L = nc*dx.  E_nodes: nc+1 doubles, HOST, copied (for a periodic grid the caller sets
+ * E_nodes[nc] = E_nodes[0]).  B: uniform field; omega_c = |q/m|*|B|; the caller does
+ * the trigonometry.  stream: a cudaStream_t (e.g. torch.cuda.Stream.cuda_stream) or
+ * NULL for the legacy default stream. */
+typedef struct {
+    int32_t nc;
+    int32_t boundary; /* pic_boundary */
+    double dx, dt;
+    const double *E_nodes; /* HOST, nc+1 */
+    double B[3];
+    void *stream;
+} pic_grid_desc;
+
+/* One species.  x, vx, vy, vz (fp64) and cell (int32) are structure-of-arrays DEVICE
+ * buffers of `capacity` elements each, 16-byte aligned, in two sets [0] and [1]
+ * (ping-pong: the arranger writes the other set).  Set [0] holds the initial state in
+ * slots [0, n): every particle live, 0 <= x < L, cell == min(floor(x*(1/dx)), nc-1).
+ * If the initial state is grouped by cell (cell non-decreasing) the fast arranger is
+ * used from the first step; otherwise the first arrange takes the general path.
+ * arrange_every: 0 = arrange only on pic_arrange(); k > 0 = pic_push also arranges
+ * right after every mover step whose cumulative step count is a multiple of k.
+ * workspace: DEVICE scratch of workspace_bytes >= pic_workspace_bytes(nc, capacity),
+ * 256-byte aligned; may be NULL only if workspace_bytes is 0, in which case an arrange
+ * that needs the general path fails with PIC_ECAPACITY. */
+typedef struct {
+    double qm; /* q/m: -1 electrons, +1/3672 D+ */
+    int64_t n, capacity;
+    double *x[2], *vx[2], *vy[2], *vz[2]; /* DEVICE */
+    int32_t *cell[2];                     /* DEVICE */
+    int32_t arrange_every;
+    int32_t reserved;
+    void *workspace; /* DEVICE */
+    size_t workspace_bytes;
+} pic_species_desc;
+
+/* Filled by pic_wall_flux.  left = wall at x = 0 (absorbed iff x' < 0), right = wall at
+ * x = L (absorbed iff x' >= L).  *_recent cover the interval since the previous
+ * pic_wall_flux call on this species; flux = count / (steps * dt), left to the caller. */
+typedef struct {
+    uint64_t left_total, right_total;
+    uint64_t left_recent, right_recent;
+    uint64_t steps_total, steps_recent;
+} pic_wall_flux_t;
+
+typedef struct pic_sim pic_sim;
+typedef struct pic_species pic_species;
+
+/* Create a simulation of `nspecies` species on the current CUDA device.  Copies E to the
+ * device, computes the per-species Boris constants on the host, validates the initial
+ * state on the device and builds per-cell count/offset.  Syncs.  Errors: PIC_EINVAL
+ * (NULL, nc < 1, dx/dt/B/qm not finite or dx,dt <= 0, n < 0, misaligned pointers),
+ * PIC_ECAPACITY (n > capacity or n >= 2^31-64), PIC_ESTATE (a particle violates the
+ * initial-state conditions above), PIC_ECUDA, PIC_ENOMEM.  On error *out is NULL. */
+int pic_create(const pic_grid_desc *grid, const pic_species_desc *species, int nspecies, pic_sim **out);
+
+/* Species handle i (0-based), or NULL.  Owned by the pic_sim. */
+pic_species *pic_species_at(pic_sim *sim, int i);
+
+/* nsteps mover steps (with the arrange_every rule).  Asynchronous on the stream.
+ * Absorbed particles are flagged cell = -1, keep their final x', v' and stay in their
+ * slot until the next arrange.  Errors: PIC_EINVAL (NULL, nsteps < 0), PIC_ECUDA. */
+int pic_push(pic_species *sp, int nsteps);
+
+/* One arrange now: per-cell histogram, device-wide exclusive scan, stable scatter into
+ * the other buffer set, which becomes the active one; afterwards slots [0, n_live) hold
+ * the live particles grouped by cell, in their previous relative order.  Asynchronous.
+ * Does not touch the step counter.  Errors: PIC_EINVAL, PIC_ECUDA; a displacement bound
+ * or workspace problem found on the device is reported by the next syncing call. */
+int pic_arrange(pic_species *sp);
+
+/* Read the wall counters.  Syncs.  Also reports any deferred device-side error
+ * (PIC_ESTATE: a particle left the domain's gather range; PIC_ECAPACITY: the general
+ * arranger was needed but the workspace is too small). */
+int pic_wall_flux(pic_species *sp, pic_wall_flux_t *out);
+
+/* Replace E (HOST, nc+1 doubles, copied; stream-ordered). */
+int pic_set_field(pic_sim *sim, const double *E_nodes_host);
+
+/* Number of slots in use: n_live after an arrange, else n at the last arrange (dead
+ * particles included).  Syncs. */
+int pic_n_slots(pic_species *sp, int64_t *n);
+
+/* Which buffer set (0 or 1) holds the current state.  Does not sync. */
+int pic_active_buffer(pic_species *sp, int *which);
+
+/* Per-cell counts (nc) and exclusive offsets (nc+1, offset[nc] = n_live) of the last
+ * arrange, copied to HOST arrays (either may be NULL).  Syncs.  PIC_ESTATE if the
+ * state has been pushed since the last arrange (the arrays would be stale). */
+int pic_cell_counts(pic_species *sp, int32_t *count_host, int32_t *offset_host);
+
+/* Cumulative mover steps of this species since pic_create.  Does not sync. */
+int pic_step_count(pic_species *sp, int64_t *steps);
+
+/* Largest displacement bound (in cells) accumulated since the last arrange, and whether
+ * the last arrange used the general path (0/1).  Diagnostics for tests.  Syncs. */
+int pic_arrange_info(pic_species *sp, int32_t *w_bound, int32_t *used_general);
+
+/* Bytes of caller-allocated workspace a species of this size needs. */
+size_t pic_workspace_bytes(int32_t nc, int64_t capacity);
+
+/* Mover/arranger variant switches for measurements (profiles/ compares them):
+ * key "e_stage": 0 = E through the read-only global path, 1 = E window staged in
+ * shared memory by TMA bulk copy (default); key "fused": 1 = single-pass push+arrange
+ * when arrange_every == 1 (default), 0 = separate mover / scan / scatter kernels.
+ * PIC_EINVAL for an unknown key or value. */
+int pic_set_option(pic_sim *sim, const char *key, int value);
+
+/* Number of kernel launches the library has enqueued for this sim since pic_create. */
+int pic_launch_count(pic_sim *sim, uint64_t *launches);
+
+/* One species described by HOST arrays, for pic_run_host.  x, vx, vy, vz (n doubles) and
+ * cell (n int32) are HOST pointers, read as the initial state (same conditions as
+ * pic_species_desc) and overwritten with the final state: slots [0, n_out) of the active
+ * buffer (live particles grouped by cell if the last step arranged; otherwise absorbed ones
+ * are still in place with cell = -1).  n_out, wall_left, wall_right are outputs. */
+typedef struct {
+    double qm;
+    int64_t n;
+    double *x, *vx, *vy, *vz; /* HOST, in/out */
+    int32_t *cell;            /* HOST, in/out */
+    int32_t arrange_every;
+    int32_t reserved;
+    int64_t n_out;
+    uint64_t wall_left, wall_right;
+} pic_host_species;
+
+/* End-to-end convenience with HOST buffers: allocates device memory, copies the species up,
+ * runs pic_create + pic_push(nsteps) on every species, copies the final state and the wall
+ * counters back and releases everything.  grid->stream is used as in pic_create.  Pinned
+ * host arrays make the copies faster but are not required.  Syncs.  Errors as pic_create /
+ * pic_push, PIC_ENOMEM when the device allocation fails. */
+int pic_run_host(const pic_grid_desc *grid, pic_host_species *species, int nspecies, int nsteps);
+
+int pic_sync(pic_sim *sim);     /* wait for the stream; reports deferred device errors */
+void pic_destroy(pic_sim *sim); /* frees library-owned memory; caller buffers untouched */
+const char *pic_strerror(int status);
+const char *pic_last_error(void); /* text of the last CUDA error seen by this thread */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PIC_H_ */

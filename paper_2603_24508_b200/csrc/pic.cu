@@ -1,0 +1,597 @@
+// pic.cu -- host side of libpic: the C ABI of include/pic.h (handles, validation, per-species
+// constants, kernel launches on the caller's stream).  No torch types; no CPU compute path.
+#include "../../include/pic.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "pic_device.cuh"
+#include "mover.cuh"
+#include "scan.cuh"
+#include "arranger.cuh"
+#include "general.cuh"
+#include "fused.cuh"
+
+using namespace pic;
+
+static thread_local char g_err[512] = "";
+
+static int cuda_fail(cudaError_t e, const char *what)
+{
+    snprintf(g_err, sizeof g_err, "%s: %s", what, cudaGetErrorString(e));
+    return PIC_ECUDA;
+}
+#define CU(call)                                            \
+    do {                                                    \
+        cudaError_t e_ = (call);                            \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
+    } while (0)
+
+struct pic_species {
+    pic_sim *sim = nullptr;
+    PushConst k{};
+    double qm = 0;
+    long long n_ub = 0, capacity = 0; // host-known upper bound of DevState::n
+    double *x[2]{}, *vx[2]{}, *vy[2]{}, *vz[2]{};
+    int *cell[2]{};
+    int cur = 0; // active buffer set
+    int arrange_every = 0;
+    DevState *d_st = nullptr;
+    int *d_count[2]{}, *d_off[2]{};
+    int cur_off = 0; // d_off[cur_off] / d_count[cur_off] describe the last arrange
+    unsigned long long *d_scan = nullptr;
+    size_t scan_words = 0;
+    FusedScratch fused{};
+    void *ws = nullptr;
+    size_t ws_bytes = 0;
+    long long steps = 0, steps_at_last_flux = 0;
+    unsigned long long wall_last[2]{};
+    bool counts_fresh = false; // count/offset describe the current state
+    bool all_live = true;      // no flagged-dead particle in [0, n)
+    bool reset_w = false;      // an arrange ran since the displacement bound was last folded
+};
+
+struct pic_sim {
+    cudaStream_t stream = nullptr;
+    double *d_E = nullptr;
+    int nc = 0, periodic = 0;
+    double dx = 0, dt = 0;
+    double B[3]{};
+    std::vector<pic_species *> sp;
+    unsigned long long launches = 0;
+    int opt_e_stage = 1, opt_fused = 1;
+    int sm_count = 148;
+};
+
+static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+extern "C" const char *pic_strerror(int s)
+{
+    switch (s) {
+    case PIC_OK: return "ok";
+    case PIC_EINVAL: return "invalid argument";
+    case PIC_ENOMEM: return "out of memory";
+    case PIC_ECUDA: return "CUDA error";
+    case PIC_ECAPACITY: return "capacity or workspace too small";
+    case PIC_ESTATE: return "invalid state";
+    default: return "unknown status";
+    }
+}
+extern "C" const char *pic_last_error(void) { return g_err; }
+
+extern "C" size_t pic_workspace_bytes(int32_t nc, int64_t capacity)
+{
+    (void)nc;
+    if (capacity < 0) return 0;
+    return general_workspace_bytes((long long)capacity);
+}
+
+static void free_species(pic_species *s)
+{
+    if (!s) return;
+    cudaFree(s->d_st);
+    for (int b = 0; b < 2; ++b) { cudaFree(s->d_count[b]); cudaFree(s->d_off[b]); }
+    cudaFree(s->d_scan);
+    cudaFree(s->fused.block_state);
+    cudaFree(s->fused.cell_bound);
+    delete s;
+}
+
+extern "C" void pic_destroy(pic_sim *sim)
+{
+    if (!sim) return;
+    cudaStreamSynchronize(sim->stream);
+    for (pic_species *s : sim->sp) free_species(s);
+    cudaFree(sim->d_E);
+    delete sim;
+}
+
+// Per-species Boris constants, DESIGN.md section 3 (each line one rounded operation; host
+// code is compiled with -ffp-contract=off).
+static void boris_constants(double qm, double dt, double dx, const double *B, PushConst &k)
+{
+    volatile double h = (qm * dt) * 0.5;
+    volatile double tx = h * B[0], ty = h * B[1], tz = h * B[2];
+    volatile double txx = tx * tx, tyy = ty * ty, tzz = tz * tz;
+    volatile double t2a = txx + tyy;
+    volatile double t2 = t2a + tzz;
+    volatile double den = 1.0 + t2;
+    volatile double f = 2.0 / den;
+    k.h = h; k.tx = tx; k.ty = ty; k.tz = tz;
+    volatile double sx = f * tx, sy = f * ty, sz = f * tz;
+    k.sx = sx; k.sy = sy; k.sz = sz;
+    volatile double inv = 1.0 / dx;
+    k.inv_dx = inv;
+    k.dt = dt;
+}
+
+static int launch_check(pic_sim *sim, const char *what)
+{
+    sim->launches++;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, what);
+    return PIC_OK;
+}
+
+static int status_to_rc(int status)
+{
+    if (status & ERR_BAD_INITIAL) return PIC_ESTATE;
+    if (status & ERR_OUT_OF_DOMAIN) return PIC_ESTATE;
+    if (status & ERR_NEED_WORKSPACE) return PIC_ECAPACITY;
+    return PIC_OK;
+}
+
+static int run_scan(pic_species *s, const int *in, int *out, int m, ScanFold fold)
+{
+    pic_sim *sim = s->sim;
+    size_t words = scan_scratch_words(m);
+    CU(cudaMemsetAsync(s->d_scan, 0, words * sizeof(unsigned long long), sim->stream));
+    int ntiles = (m + SCAN_TILE - 1) / SCAN_TILE;
+    scan_exclusive_kernel<<<ntiles, SCAN_THREADS, 0, sim->stream>>>(in, out, m, s->d_scan, fold);
+    return launch_check(sim, "scan_exclusive_kernel");
+}
+
+// ------------------------------------------------------------------------------------------
+// create
+// ------------------------------------------------------------------------------------------
+static int create_species(pic_sim *sim, const pic_species_desc &d, pic_species **out)
+{
+    if (!std::isfinite(d.qm) || d.n < 0 || d.capacity < 0 || d.arrange_every < 0) return PIC_EINVAL;
+    if (d.n > d.capacity) return PIC_ECAPACITY;
+    if (d.capacity >= (1LL << 31) - 64) return PIC_ECAPACITY;
+    for (int b = 0; b < 2; ++b) {
+        if (d.capacity > 0 && (!d.x[b] || !d.vx[b] || !d.vy[b] || !d.vz[b] || !d.cell[b])) return PIC_EINVAL;
+        if (!aligned16(d.x[b]) || !aligned16(d.vx[b]) || !aligned16(d.vy[b]) || !aligned16(d.vz[b]) ||
+            !aligned16(d.cell[b]))
+            return PIC_EINVAL;
+    }
+    if ((d.workspace == nullptr) != (d.workspace_bytes == 0)) return PIC_EINVAL;
+    if (d.workspace && (reinterpret_cast<uintptr_t>(d.workspace) & 255u)) return PIC_EINVAL;
+
+    pic_species *s = new (std::nothrow) pic_species;
+    if (!s) return PIC_ENOMEM;
+    *out = s;
+    s->sim = sim;
+    s->qm = d.qm;
+    s->n_ub = d.n;
+    s->capacity = d.capacity;
+    for (int b = 0; b < 2; ++b) {
+        s->x[b] = d.x[b]; s->vx[b] = d.vx[b]; s->vy[b] = d.vy[b]; s->vz[b] = d.vz[b]; s->cell[b] = d.cell[b];
+    }
+    s->arrange_every = d.arrange_every;
+    s->ws = d.workspace;
+    s->ws_bytes = d.workspace_bytes;
+    boris_constants(d.qm, sim->dt, sim->dx, sim->B, s->k);
+    s->k.nc = sim->nc;
+    s->k.periodic = sim->periodic;
+    s->k.L = (double)sim->nc * sim->dx;
+
+    const int nc = sim->nc;
+    CU(cudaMalloc(&s->d_st, sizeof(DevState)));
+    for (int b = 0; b < 2; ++b) {
+        CU(cudaMalloc(&s->d_count[b], sizeof(int) * ((size_t)nc + 16)));
+        CU(cudaMalloc(&s->d_off[b], sizeof(int) * ((size_t)nc + 16)));
+        CU(cudaMemsetAsync(s->d_count[b], 0, sizeof(int) * ((size_t)nc + 16), sim->stream));
+        CU(cudaMemsetAsync(s->d_off[b], 0, sizeof(int) * ((size_t)nc + 16), sim->stream));
+    }
+    // scan scratch sized for the largest array the library scans (per-cell counts, or the
+    // general path's per-tile digit histograms)
+    long long max_scan = std::max<long long>((long long)nc + 1, general_scan_elems(d.capacity));
+    s->scan_words = scan_scratch_words(max_scan);
+    CU(cudaMalloc(&s->d_scan, s->scan_words * sizeof(unsigned long long)));
+
+    DevState h{};
+    h.n = (int)d.n;
+    CU(cudaMemcpyAsync(s->d_st, &h, sizeof h, cudaMemcpyHostToDevice, sim->stream));
+    CU(cudaStreamSynchronize(sim->stream)); // h is a stack object
+
+    // validate the initial state, build count/offset of the initial grouping
+    if (d.n > 0) {
+        int blocks = (int)((d.n + 255) / 256);
+        validate_kernel<<<blocks, 256, 0, sim->stream>>>(s->x[0], s->cell[0], s->k, s->d_st);
+        if (int rc = launch_check(sim, "validate_kernel")) return rc;
+    }
+    CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, sim->stream));
+    CU(cudaStreamSynchronize(sim->stream));
+    if (h.status & ERR_BAD_INITIAL) {
+        snprintf(g_err, sizeof g_err, "initial state violates 0<=x<L, cell==floor(x/dx), all live");
+        return PIC_ESTATE;
+    }
+    bool grouped = !(h.status & ERR_NOT_GROUPED);
+    if (d.n > 0) {
+        int blocks = (int)((d.n + HIST_THREADS * HIST_ITEMS - 1) / (HIST_THREADS * HIST_ITEMS));
+        hist_kernel<<<blocks, HIST_THREADS, 0, sim->stream>>>(s->cell[0], s->d_count[0], s->d_st);
+        if (int rc = launch_check(sim, "hist_kernel")) return rc;
+    }
+    ScanFold nofold{nullptr, 0, 0, nullptr};
+    if (int rc = run_scan(s, s->d_count[0], s->d_off[0], nc, nofold)) return rc;
+    h.status = 0;
+    h.w_acc = grouped ? 0 : W_UNKNOWN;
+    CU(cudaMemcpyAsync(s->d_st, &h, sizeof h, cudaMemcpyHostToDevice, sim->stream));
+    CU(cudaStreamSynchronize(sim->stream));
+    s->cur = 0;
+    s->cur_off = 0;
+    s->counts_fresh = grouped;
+    s->all_live = true;
+    s->reset_w = false;
+    if (int rc = fused_alloc(s->fused, nc, d.capacity)) return rc == PIC_ENOMEM ? PIC_ENOMEM : cuda_fail(cudaGetLastError(), "fused_alloc");
+    return PIC_OK;
+}
+
+extern "C" int pic_create(const pic_grid_desc *g, const pic_species_desc *species, int nspecies, pic_sim **out)
+{
+    if (out) *out = nullptr;
+    if (!g || !species || !out || nspecies < 1) return PIC_EINVAL;
+    if (g->nc < 1 || g->nc >= (1 << 30) || !g->E_nodes) return PIC_EINVAL;
+    if (!(g->dx > 0) || !(g->dt > 0) || !std::isfinite(g->dx) || !std::isfinite(g->dt)) return PIC_EINVAL;
+    if (g->boundary != PIC_PERIODIC && g->boundary != PIC_ABSORBING) return PIC_EINVAL;
+    for (int a = 0; a < 3; ++a)
+        if (!std::isfinite(g->B[a])) return PIC_EINVAL;
+    for (int j = 0; j <= g->nc; ++j)
+        if (!std::isfinite(g->E_nodes[j])) return PIC_EINVAL;
+
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    pic_sim *sim = new (std::nothrow) pic_sim;
+    if (!sim) return PIC_ENOMEM;
+    sim->stream = static_cast<cudaStream_t>(g->stream);
+    sim->nc = g->nc;
+    sim->periodic = g->boundary == PIC_PERIODIC;
+    sim->dx = g->dx;
+    sim->dt = g->dt;
+    for (int a = 0; a < 3; ++a) sim->B[a] = g->B[a];
+    int rc = PIC_OK;
+    do {
+        cudaError_t e = cudaDeviceGetAttribute(&sim->sm_count, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) { rc = cuda_fail(e, "cudaDeviceGetAttribute"); break; }
+        // E padded to an even number of nodes (+2) so that 16-byte bulk copies of any window stay inside
+        e = cudaMalloc(&sim->d_E, sizeof(double) * ((size_t)g->nc + 8));
+        if (e != cudaSuccess) { rc = e == cudaErrorMemoryAllocation ? PIC_ENOMEM : cuda_fail(e, "cudaMalloc E"); break; }
+        e = cudaMemsetAsync(sim->d_E, 0, sizeof(double) * ((size_t)g->nc + 8), sim->stream);
+        if (e != cudaSuccess) { rc = cuda_fail(e, "cudaMemsetAsync E"); break; }
+        e = cudaMemcpyAsync(sim->d_E, g->E_nodes, sizeof(double) * ((size_t)g->nc + 1), cudaMemcpyHostToDevice, sim->stream);
+        if (e != cudaSuccess) { rc = cuda_fail(e, "cudaMemcpyAsync E"); break; }
+        e = cudaStreamSynchronize(sim->stream);
+        if (e != cudaSuccess) { rc = cuda_fail(e, "cudaStreamSynchronize"); break; }
+        for (int i = 0; i < nspecies && rc == PIC_OK; ++i) {
+            pic_species *s = nullptr;
+            rc = create_species(sim, species[i], &s);
+            if (s) sim->sp.push_back(s);
+        }
+    } while (0);
+    if (rc != PIC_OK) {
+        pic_destroy(sim);
+        return rc;
+    }
+    *out = sim;
+    return PIC_OK;
+}
+
+extern "C" pic_species *pic_species_at(pic_sim *sim, int i)
+{
+    if (!sim || i < 0 || i >= (int)sim->sp.size()) return nullptr;
+    return sim->sp[i];
+}
+
+extern "C" int pic_set_field(pic_sim *sim, const double *E)
+{
+    if (!sim || !E) return PIC_EINVAL;
+    for (int j = 0; j <= sim->nc; ++j)
+        if (!std::isfinite(E[j])) return PIC_EINVAL;
+    CU(cudaMemcpyAsync(sim->d_E, E, sizeof(double) * ((size_t)sim->nc + 1), cudaMemcpyHostToDevice, sim->stream));
+    CU(cudaStreamSynchronize(sim->stream)); // E is a caller buffer that may be pageable
+    return PIC_OK;
+}
+
+extern "C" int pic_set_option(pic_sim *sim, const char *key, int value)
+{
+    if (!sim || !key || (value != 0 && value != 1)) return PIC_EINVAL;
+    if (!strcmp(key, "e_stage")) sim->opt_e_stage = value;
+    else if (!strcmp(key, "fused")) sim->opt_fused = value;
+    else return PIC_EINVAL;
+    return PIC_OK;
+}
+
+extern "C" int pic_launch_count(pic_sim *sim, uint64_t *launches)
+{
+    if (!sim || !launches) return PIC_EINVAL;
+    *launches = sim->launches;
+    return PIC_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// arrange (split path): [histogram] -> scan -> destination-driven scatter [-> general path]
+// ------------------------------------------------------------------------------------------
+static int arrange_split(pic_species *s, bool hist_ready)
+{
+    pic_sim *sim = s->sim;
+    const int nc = sim->nc;
+    const int src = s->cur, dst = s->cur ^ 1;
+    const int oo = s->cur_off, on = s->cur_off ^ 1;
+    if (!hist_ready) {
+        CU(cudaMemsetAsync(s->d_count[on], 0, sizeof(int) * (size_t)nc, sim->stream));
+        if (s->n_ub > 0) {
+            int blocks = (int)((s->n_ub + HIST_THREADS * HIST_ITEMS - 1) / (HIST_THREADS * HIST_ITEMS));
+            hist_kernel<<<blocks, HIST_THREADS, 0, sim->stream>>>(s->cell[src], s->d_count[on], s->d_st);
+            if (int rc = launch_check(sim, "hist_kernel")) return rc;
+        }
+    }
+    ScanFold fold{s->d_st, s->reset_w ? 1 : 0, 1, nullptr};
+    s->reset_w = false;
+    if (int rc = run_scan(s, s->d_count[on], s->d_off[on], nc, fold)) return rc;
+
+    ScatterArgs a{};
+    a.sx = s->x[src]; a.svx = s->vx[src]; a.svy = s->vy[src]; a.svz = s->vz[src]; a.scell = s->cell[src];
+    a.dx = s->x[dst]; a.dvx = s->vx[dst]; a.dvy = s->vy[dst]; a.dvz = s->vz[dst]; a.dcell = s->cell[dst];
+    a.off_old = s->d_off[oo]; a.count_new = s->d_count[on]; a.off_new = s->d_off[on];
+    a.st = s->d_st; a.nc = nc; a.periodic = sim->periodic;
+    a.w_limit = FAST_W_LIMIT;
+    {
+        long long want = ((long long)nc + SCATTER_THREADS / 32 - 1) / (SCATTER_THREADS / 32);
+        int blocks = (int)std::min<long long>(want, (long long)sim->sm_count * 64);
+        scatter_fast_kernel<<<blocks, SCATTER_THREADS, 0, sim->stream>>>(a);
+        if (int rc = launch_check(sim, "scatter_fast_kernel")) return rc;
+    }
+    // general path: every kernel returns at once unless scatter_fast_kernel declined
+    GeneralArgs ga{};
+    ga.sx = a.sx; ga.svx = a.svx; ga.svy = a.svy; ga.svz = a.svz; ga.scell = a.scell;
+    ga.dx = a.dx; ga.dvx = a.dvx; ga.dvy = a.dvy; ga.dvz = a.dvz; ga.dcell = a.dcell;
+    ga.st = s->d_st; ga.nc = nc; ga.n_ub = s->n_ub; ga.ws = s->ws; ga.ws_bytes = s->ws_bytes;
+    ga.off_old = s->d_off[oo];
+    ga.scan_scratch = s->d_scan;
+    if (int rc = general_arrange(ga, sim->stream, sim->sm_count, &sim->launches)) return rc == PIC_ECUDA ? cuda_fail(cudaGetLastError(), "general_arrange") : rc;
+
+    s->cur = dst;
+    s->cur_off = on;
+    s->counts_fresh = true;
+    s->all_live = true;
+    s->reset_w = true;
+    return PIC_OK;
+}
+
+extern "C" int pic_arrange(pic_species *s)
+{
+    if (!s) return PIC_EINVAL;
+    return arrange_split(s, false);
+}
+
+// ------------------------------------------------------------------------------------------
+// push
+// ------------------------------------------------------------------------------------------
+template <bool RC, bool H>
+static void launch_mover(pic_species *s, const MoverArgs &a, int blocks)
+{
+    mover_kernel<RC, H><<<blocks, MOVER_THREADS, 0, s->sim->stream>>>(a);
+}
+
+static int push_split(pic_species *s, bool will_arrange)
+{
+    pic_sim *sim = s->sim;
+    const int nc = sim->nc;
+    const int on = s->cur_off ^ 1;
+    if (will_arrange) CU(cudaMemsetAsync(s->d_count[on], 0, sizeof(int) * (size_t)nc, sim->stream));
+    if (s->n_ub > 0) {
+        MoverArgs a{};
+        a.x = s->x[s->cur]; a.vx = s->vx[s->cur]; a.vy = s->vy[s->cur]; a.vz = s->vz[s->cur];
+        a.cell = s->cell[s->cur];
+        a.E = sim->d_E; a.count = s->d_count[on]; a.st = s->d_st; a.k = s->k;
+        long long pairs = (s->n_ub + 1) / 2;
+        int blocks = (int)((pairs + MOVER_THREADS - 1) / MOVER_THREADS);
+        const bool rc = !s->all_live;
+        if (rc) { if (will_arrange) launch_mover<true, true>(s, a, blocks); else launch_mover<true, false>(s, a, blocks); }
+        else    { if (will_arrange) launch_mover<false, true>(s, a, blocks); else launch_mover<false, false>(s, a, blocks); }
+        if (int r = launch_check(sim, "mover_kernel")) return r;
+    }
+    if (!sim->periodic) s->all_live = false;
+    s->counts_fresh = false;
+    if (!will_arrange) {
+        end_step_kernel<<<1, 1, 0, sim->stream>>>(s->d_st, s->reset_w ? 1 : 0);
+        s->reset_w = false;
+        if (int r = launch_check(sim, "end_step_kernel")) return r;
+    }
+    return PIC_OK;
+}
+
+extern "C" int pic_push(pic_species *s, int nsteps)
+{
+    if (!s || nsteps < 0) return PIC_EINVAL;
+    for (int it = 0; it < nsteps; ++it) {
+        const bool will_arrange = s->arrange_every > 0 && ((s->steps + 1) % s->arrange_every) == 0;
+        if (int rc = push_split(s, will_arrange)) return rc;
+        s->steps++;
+        if (will_arrange)
+            if (int rc = arrange_split(s, true)) return rc;
+    }
+    return PIC_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// read-outs
+// ------------------------------------------------------------------------------------------
+static int read_state(pic_species *s, DevState &h)
+{
+    CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, s->sim->stream));
+    CU(cudaStreamSynchronize(s->sim->stream));
+    if (h.n >= 0 && h.n <= s->n_ub) s->n_ub = h.n;
+    return PIC_OK;
+}
+
+extern "C" int pic_wall_flux(pic_species *s, pic_wall_flux_t *out)
+{
+    if (!s || !out) return PIC_EINVAL;
+    DevState h;
+    if (int rc = read_state(s, h)) return rc;
+    out->left_total = h.wall[0];
+    out->right_total = h.wall[1];
+    out->left_recent = h.wall[0] - s->wall_last[0];
+    out->right_recent = h.wall[1] - s->wall_last[1];
+    out->steps_total = (uint64_t)s->steps;
+    out->steps_recent = (uint64_t)(s->steps - s->steps_at_last_flux);
+    s->wall_last[0] = h.wall[0];
+    s->wall_last[1] = h.wall[1];
+    s->steps_at_last_flux = s->steps;
+    return status_to_rc(h.status);
+}
+
+extern "C" int pic_n_slots(pic_species *s, int64_t *n)
+{
+    if (!s || !n) return PIC_EINVAL;
+    DevState h;
+    if (int rc = read_state(s, h)) return rc;
+    *n = h.n;
+    return status_to_rc(h.status);
+}
+
+extern "C" int pic_active_buffer(pic_species *s, int *which)
+{
+    if (!s || !which) return PIC_EINVAL;
+    *which = s->cur;
+    return PIC_OK;
+}
+
+extern "C" int pic_step_count(pic_species *s, int64_t *steps)
+{
+    if (!s || !steps) return PIC_EINVAL;
+    *steps = s->steps;
+    return PIC_OK;
+}
+
+extern "C" int pic_cell_counts(pic_species *s, int32_t *count_host, int32_t *offset_host)
+{
+    if (!s) return PIC_EINVAL;
+    if (!s->counts_fresh) return PIC_ESTATE;
+    const int nc = s->sim->nc;
+    if (count_host)
+        CU(cudaMemcpyAsync(count_host, s->d_count[s->cur_off], sizeof(int) * (size_t)nc, cudaMemcpyDeviceToHost, s->sim->stream));
+    if (offset_host)
+        CU(cudaMemcpyAsync(offset_host, s->d_off[s->cur_off], sizeof(int) * ((size_t)nc + 1), cudaMemcpyDeviceToHost, s->sim->stream));
+    CU(cudaStreamSynchronize(s->sim->stream));
+    return PIC_OK;
+}
+
+extern "C" int pic_arrange_info(pic_species *s, int32_t *w_bound, int32_t *used_general)
+{
+    if (!s) return PIC_EINVAL;
+    DevState h;
+    if (int rc = read_state(s, h)) return rc;
+    if (w_bound) *w_bound = h.w_acc;
+    if (used_general) *used_general = h.used_general;
+    return PIC_OK;
+}
+
+extern "C" int pic_sync(pic_sim *sim)
+{
+    if (!sim) return PIC_EINVAL;
+    CU(cudaStreamSynchronize(sim->stream));
+    int rc = PIC_OK;
+    for (pic_species *s : sim->sp) {
+        DevState h;
+        if (int r = read_state(s, h)) return r;
+        if (int r = status_to_rc(h.status)) rc = r;
+    }
+    return rc;
+}
+
+// ------------------------------------------------------------------------------------------
+// end-to-end call with host buffers
+// ------------------------------------------------------------------------------------------
+extern "C" int pic_run_host(const pic_grid_desc *g, pic_host_species *hs, int nspecies, int nsteps)
+{
+    if (!g || !hs || nspecies < 1 || nsteps < 0) return PIC_EINVAL;
+    cudaStream_t stream = static_cast<cudaStream_t>(g->stream);
+    std::vector<pic_species_desc> descs(nspecies);
+    std::vector<void *> allocs;
+    int rc = PIC_OK;
+    pic_sim *sim = nullptr;
+    auto dmalloc = [&](size_t bytes) -> void * {
+        void *p = nullptr;
+        if (cudaMalloc(&p, bytes ? bytes : 16) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        allocs.push_back(p);
+        return p;
+    };
+    do {
+        for (int i = 0; i < nspecies && rc == PIC_OK; ++i) {
+            pic_host_species &h = hs[i];
+            if (h.n < 0 || (h.n > 0 && (!h.x || !h.vx || !h.vy || !h.vz || !h.cell))) { rc = PIC_EINVAL; break; }
+            pic_species_desc &d = descs[i];
+            memset(&d, 0, sizeof d);
+            d.qm = h.qm; d.n = h.n; d.capacity = h.n; d.arrange_every = h.arrange_every;
+            const size_t nb = sizeof(double) * (size_t)h.n, ni = sizeof(int32_t) * (size_t)h.n;
+            for (int b = 0; b < 2; ++b) {
+                d.x[b] = (double *)dmalloc(nb); d.vx[b] = (double *)dmalloc(nb);
+                d.vy[b] = (double *)dmalloc(nb); d.vz[b] = (double *)dmalloc(nb);
+                d.cell[b] = (int32_t *)dmalloc(ni);
+                if (!d.x[b] || !d.vx[b] || !d.vy[b] || !d.vz[b] || !d.cell[b]) { rc = PIC_ENOMEM; break; }
+            }
+            if (rc) break;
+            d.workspace_bytes = pic_workspace_bytes(g->nc, h.n);
+            d.workspace = dmalloc(d.workspace_bytes);
+            if (!d.workspace) { rc = PIC_ENOMEM; break; }
+            cudaError_t e = cudaSuccess;
+            if (h.n > 0) {
+                e = cudaMemcpyAsync(d.x[0], h.x, nb, cudaMemcpyHostToDevice, stream);
+                if (e == cudaSuccess) e = cudaMemcpyAsync(d.vx[0], h.vx, nb, cudaMemcpyHostToDevice, stream);
+                if (e == cudaSuccess) e = cudaMemcpyAsync(d.vy[0], h.vy, nb, cudaMemcpyHostToDevice, stream);
+                if (e == cudaSuccess) e = cudaMemcpyAsync(d.vz[0], h.vz, nb, cudaMemcpyHostToDevice, stream);
+                if (e == cudaSuccess) e = cudaMemcpyAsync(d.cell[0], h.cell, ni, cudaMemcpyHostToDevice, stream);
+            }
+            if (e != cudaSuccess) { rc = cuda_fail(e, "cudaMemcpyAsync H2D"); break; }
+        }
+        if (rc) break;
+        rc = pic_create(g, descs.data(), nspecies, &sim);
+        if (rc) break;
+        for (int i = 0; i < nspecies && rc == PIC_OK; ++i) rc = pic_push(sim->sp[i], nsteps);
+        if (rc) break;
+        for (int i = 0; i < nspecies && rc == PIC_OK; ++i) {
+            pic_species *s = sim->sp[i];
+            pic_host_species &h = hs[i];
+            pic_wall_flux_t wf;
+            rc = pic_wall_flux(s, &wf);
+            if (rc) break;
+            int64_t n = 0;
+            rc = pic_n_slots(s, &n);
+            if (rc) break;
+            h.n_out = n; h.wall_left = wf.left_total; h.wall_right = wf.right_total;
+            const size_t nb = sizeof(double) * (size_t)n, ni = sizeof(int32_t) * (size_t)n;
+            const int b = s->cur;
+            cudaError_t e = cudaSuccess;
+            if (n > 0) {
+                e = cudaMemcpyAsync(h.x, s->x[b], nb, cudaMemcpyDeviceToHost, stream);
+                if (e == cudaSuccess) e = cudaMemcpyAsync(h.vx, s->vx[b], nb, cudaMemcpyDeviceToHost, stream);
+                if (e == cudaSuccess) e = cudaMemcpyAsync(h.vy, s->vy[b], nb, cudaMemcpyDeviceToHost, stream);
+                if (e == cudaSuccess) e = cudaMemcpyAsync(h.vz, s->vz[b], nb, cudaMemcpyDeviceToHost, stream);
+                if (e == cudaSuccess) e = cudaMemcpyAsync(h.cell, s->cell[b], ni, cudaMemcpyDeviceToHost, stream);
+            }
+            if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+            if (e != cudaSuccess) { rc = cuda_fail(e, "cudaMemcpyAsync D2H"); break; }
+        }
+    } while (0);
+    if (sim) pic_destroy(sim);
+    else cudaStreamSynchronize(stream);
+    for (void *p : allocs) cudaFree(p);
+    return rc;
+}

@@ -1,0 +1,227 @@
+"""GPU parity: libpic (CUDA, through the C ABI) against the CPU oracle, element by element, on the
+seeded inputs of the five BASELINE.json configs at sizes the oracle finishes in seconds that
+still span many tiles and ragged tails, plus the arranger's edge and degenerate cases.
+Full-size runs live in test_gpu_fullsize.py."""
+import numpy as np
+import pytest
+
+import oracle
+import paper_2603_24508_b200 as pic
+from paper_2603_24508_b200 import workloads
+from parity_util import compare, make_pair, run_bulk, run_stepwise
+
+pytestmark = pytest.mark.gpu
+
+VARIANTS = [
+    pytest.param({"fused": 0, "e_stage": 0}, id="split-ldg"),
+    pytest.param({"fused": 0, "e_stage": 1}, id="split-tma"),
+    pytest.param({"fused": 1, "e_stage": 1}, id="fused"),
+]
+
+
+@pytest.mark.parametrize("options", VARIANTS)
+def test_config1_full_200_steps(options):
+    """configs[0]: 1,024 periodic cells x 64 = 65,536 electrons, 200 steps, arrange every step."""
+    inp = workloads.make(1)
+    run_stepwise(inp, 200, options=options)
+
+
+@pytest.mark.parametrize("options", VARIANTS)
+def test_config1_bulk_equals_stepwise(options):
+    inp = workloads.make(1)
+    run_bulk(inp, 200, options=options)
+
+
+@pytest.mark.parametrize("options", VARIANTS)
+def test_config2_reduced_absorbing(options):
+    """configs[1] shape (absorbing walls, 160 ppc, 85 deg) on 2,048 cells: 327,680 particles, ragged tail."""
+    inp = workloads.make(2, nc=2048)
+    sim, states = run_stepwise(inp, 100, options=options, check_every=5)
+    assert states[0].wall.sum() > 0  # the walls did absorb something, so compaction was exercised
+
+
+@pytest.mark.parametrize("options", VARIANTS)
+def test_config3_reduced_two_species(options):
+    """configs[2] shape: electrons + D+ (q/m = 1/3672), sheath field, absorbing walls, 200 ppc."""
+    inp = workloads.make(3, nc=1000)
+    run_stepwise(inp, 60, options=options, check_every=4)
+
+
+@pytest.mark.parametrize("options", VARIANTS)
+def test_config4_reduced_periodic(options):
+    """configs[3] shape: periodic, 100 ppc, 16 modes; 4,099 cells (odd, prime) -> 409,900 particles."""
+    inp = workloads.make(4, nc=4099)
+    run_stepwise(inp, 50, options=options, check_every=5)
+
+
+@pytest.mark.parametrize("options", VARIANTS)
+def test_config5_reduced_sort_stress(options):
+    """configs[4] shape: 100x density contrast, v_th = 4, arrange every 10 steps, dead particles stay
+    flagged in place between arranges (compared slot by slot)."""
+    inp = workloads.make(5, nc=4096)
+    sim, states = run_stepwise(inp, 40, options=options, check_every=1)
+    w, used_general = pic.pic_arrange_info(sim.species[0])
+    assert used_general == 0
+
+
+def test_explicit_arrange_and_no_auto_arrange():
+    """arrange_every = 0: pushes never arrange; pic_arrange() on demand; arranging twice is the identity."""
+    inp = workloads.make(2, nc=512)
+    sim, (st,) = make_pair(inp, arrange_every=0)
+    sp = sim.species[0]
+    for k in range(7):
+        pic.pic_push(sp, 3)
+        st.push(3)
+        compare(sp, st, where=f"push block {k}")
+        pic.pic_arrange(sp)
+        st.arrange()
+        compare(sp, st, where=f"arrange {k}", counts=True, nc=inp["nc"])
+    pic.pic_arrange(sp)
+    st.arrange()
+    compare(sp, st, where="second arrange", counts=True, nc=inp["nc"])
+    with pytest.raises(pic.PicError):
+        pic.pic_push(sp, 1)
+        pic.pic_cell_counts(sp, inp["nc"])  # stale after a push -> PIC_ESTATE
+
+
+def test_general_path_unsorted_input():
+    """An initial state that is NOT grouped by cell takes the general (radix) path on the first arrange."""
+    inp = workloads.make(1, nc=300, ppc=37)
+    rng = np.random.default_rng(7)
+    s = inp["species"][0]
+    perm = rng.permutation(len(s["x"]))
+    for k in ("x", "vx", "vy", "vz", "cell"):
+        s[k] = np.ascontiguousarray(s[k][perm])
+    sim, (st,) = make_pair(inp)
+    sp = sim.species[0]
+    pic.pic_push(sp, 1)
+    st.push(1)
+    compare(sp, st, where="first arrange (general)", counts=True, nc=inp["nc"])
+    assert pic.pic_arrange_info(sp)[1] == 1
+    pic.pic_push(sp, 5)
+    st.push(5)
+    compare(sp, st, where="later arranges (fast)", counts=True, nc=inp["nc"])
+    assert pic.pic_arrange_info(sp)[1] == 0
+
+
+def test_general_path_large_displacement():
+    """Many pushes without arranging: the displacement bound exceeds the fast path's limit."""
+    inp = workloads.make(5, nc=2048)
+    sim, (st,) = make_pair(inp, arrange_every=0)
+    sp = sim.species[0]
+    pic.pic_push(sp, 150)
+    st.push(150)
+    pic.pic_arrange(sp)
+    st.arrange()
+    compare(sp, st, where="arrange after 150 free steps", counts=True, nc=inp["nc"])
+    assert pic.pic_arrange_info(sp)[1] == 1
+
+
+def test_general_path_without_workspace_reports():
+    inp = workloads.make(1, nc=64, ppc=8)
+    s = inp["species"][0]
+    perm = np.random.default_rng(3).permutation(len(s["x"]))
+    for k in ("x", "vx", "vy", "vz", "cell"):
+        s[k] = np.ascontiguousarray(s[k][perm])
+    sim, _ = make_pair(inp, workspace=None)
+    pic.pic_push(sim.species[0], 1)
+    with pytest.raises(pic.PicError) as e:
+        pic.pic_wall_flux(sim.species[0])
+    assert e.value.status == pic.PIC_ECAPACITY
+
+
+@pytest.mark.parametrize("n", [0, 1, 2, 3, 31, 32, 33, 511, 513])
+@pytest.mark.parametrize("boundary", [workloads.PERIODIC, workloads.ABSORBING])
+def test_tiny_and_ragged(n, boundary):
+    rng = np.random.default_rng(100 + n)
+    nc = 5
+    cell = np.sort(rng.integers(0, nc, n)).astype(np.int32)
+    x = cell + rng.random(n)
+    x = np.where(np.floor(x) != cell, np.nextafter(cell + 1.0, 0), x)
+    v = 6.0 * rng.standard_normal((3, n))
+    inp = dict(nc=nc, dx=1.0, dt=0.1, boundary=boundary, E=rng.uniform(-1, 1, nc + 1), B=np.array([0.3, -1.0, 2.0]),
+               arrange_every=1, species=[dict(qm=-1.0, x=x, vx=v[0], vy=v[1], vz=v[2], cell=cell)])
+    for options in ({"fused": 0}, {"fused": 1}):
+        run_stepwise(inp, 12, options=options)
+
+
+def test_single_cell_and_all_absorbed():
+    rng = np.random.default_rng(5)
+    n = 1000
+    cell = np.zeros(n, dtype=np.int32)
+    x = rng.random(n)
+    inp = dict(nc=1, dx=1.0, dt=0.1, boundary=workloads.ABSORBING, E=np.array([0.1, -0.2]), B=np.array([0.0, 2.0, 0.0]),
+               arrange_every=1,
+               species=[dict(qm=-1.0, x=x, vx=3.0 * rng.standard_normal(n), vy=rng.standard_normal(n),
+                             vz=rng.standard_normal(n), cell=cell)])
+    sim, (st,) = run_stepwise(inp, 40)
+    assert st.n + int(st.wall.sum()) == n
+    # periodic single cell: every particle wraps within the same cell
+    inp["boundary"] = workloads.PERIODIC
+    inp["E"] = np.array([0.1, 0.1])
+    run_stepwise(inp, 20)
+
+
+def test_dx_not_one_and_three_component_B():
+    """dx != 1 exercises the inv_dx products and the clamp reading S8; B with a z component."""
+    rng = np.random.default_rng(11)
+    nc, ppc, dx = 257, 21, 0.37
+    cell = np.repeat(np.arange(nc, dtype=np.int32), ppc)
+    x = (cell + rng.random(nc * ppc)) * dx
+    inv = 1.0 / dx
+    ok = np.minimum(np.floor(x * inv), nc - 1) == cell
+    x = x[ok]; cell = cell[ok]
+    keep = x < nc * dx
+    x = x[keep]; cell = cell[keep]
+    n = len(x)
+    v = rng.standard_normal((3, n))
+    for boundary in (workloads.PERIODIC, workloads.ABSORBING):
+        E = rng.uniform(-0.5, 0.5, nc + 1)
+        if boundary == workloads.PERIODIC:
+            E[nc] = E[0]
+        inp = dict(nc=nc, dx=dx, dt=0.05, boundary=boundary, E=E, B=np.array([1.5, 1.25, 0.5]), arrange_every=1,
+                   species=[dict(qm=-1.0, x=x, vx=v[0], vy=v[1], vz=v[2], cell=cell)])
+        for options in ({"fused": 0}, {"fused": 1}):
+            run_stepwise(inp, 30, options=options)
+
+
+def test_create_rejects_bad_state():
+    inp = workloads.make(1, nc=16, ppc=4)
+    s = inp["species"][0]
+    s["cell"] = s["cell"].copy()
+    s["cell"][5] += 1  # cell != floor(x)
+    with pytest.raises(pic.PicError) as e:
+        make_pair(inp)
+    assert e.value.status == pic.PIC_ESTATE
+
+
+def test_wall_flux_recent_and_step_counters():
+    inp = workloads.make(2, nc=256)
+    sim, (st,) = make_pair(inp)
+    sp = sim.species[0]
+    pic.pic_push(sp, 10)
+    a = pic.pic_wall_flux(sp)
+    pic.pic_push(sp, 15)
+    b = pic.pic_wall_flux(sp)
+    st.push(25)
+    assert b["left_total"] == int(st.wall[0]) and b["right_total"] == int(st.wall[1])
+    assert a["left_recent"] == a["left_total"] and b["left_recent"] == b["left_total"] - a["left_total"]
+    assert b["right_recent"] == b["right_total"] - a["right_total"]
+    assert (a["steps_recent"], b["steps_recent"], b["steps_total"]) == (10, 15, 25)
+    assert pic.pic_step_count(sp) == 25
+
+
+def test_run_host_end_to_end():
+    """pic_run_host: the C-ABI call with HOST buffers (the one bench.py's e2e leg times)."""
+    import ctypes as C
+    inp = workloads.make(2, nc=512)
+    s = inp["species"][0]
+    st = oracle.State(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], nc=inp["nc"], dx=inp["dx"], dt=inp["dt"],
+                      boundary=inp["boundary"], E=inp["E"], qm=s["qm"], B=inp["B"], arrange_every=1)
+    st.push(20)
+    arrs = [np.array(s[k]) for k in ("x", "vx", "vy", "vz", "cell")]
+    n_out, wl, wr = pic.pic_run_host(nc=inp["nc"], dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E_nodes=inp["E"],
+                                     B=inp["B"], species=[dict(qm=s["qm"], arrays=arrs, arrange_every=1)], nsteps=20)[0]
+    assert n_out == st.n and (wl, wr) == (int(st.wall[0]), int(st.wall[1]))
+    for a, o in zip(arrs, st.live()):
+        assert np.array_equal(a[:n_out], o)
