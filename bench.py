@@ -1,0 +1,369 @@
+#!/usr/bin/env python
+"""bench.py -- particle pushes/sec (mover+arranger, fp64) of libpic on B200, with its HBM roofline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 \
+        --master-port P bench.py --gpus N --steps K --warmup W
+
+One "step" is one pass of the whole hot path (gather, Boris update, x
+advance, wall flag, per-cell histogram, scan, stable scatter + compaction, wall counters) over
+every particle of the workload: one pic_push(species, 1) with arrange_every from the config.
+Default workload: BASELINE.json configs[3], the 100 M-particle bandwidth-scale config the
+metric's target is quoted on (3.6 GB of fp64 SoA per buffer set, far above the 126 MB L2, so
+no L2 flush is needed between steps).  Inputs are seeded and synthetic (workloads.py).
+
+N > 1: the path is single-GPU by BASELINE.json; ranks run independent replicas of the workload
+("replicas only"), no data-path collective; value = sum of the ranks'
+pushes / max-over-ranks device time.
+
+Prints ONE JSON line (rank 0).  `value`: inputs resident in HBM, CUDA-event timed on the
+library's stream.  `e2e`: the same metric through the C-ABI call pic_run_host with HOST
+(pinned) buffers, H2D + the config's full step count + D2H inside the timed region.
+`roofline`: the dominant kernel's algorithmic bytes / its mean launch duration measured with
+CUDA events inside the timed region (pic_kernel_time), against MEASURED_PEAKS.json.
+`cpu_baseline`: the CPU oracle (oracle/, as it stands, 1 thread) on a bounded sample.
+
+--impl reference: there is no reference implementation to install (the paper ships no code);
+per the task contract this arm times the CPU oracle on the host cores.
+"""
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "particle pushes/sec (mover+arranger, fp64, 1 B200) and % of HBM peak"
+UNIT = "pushes/s"
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
+
+# Algorithmic bytes per particle per launch: what the step must move.
+#   mover   : read x,vx,vy,vz (32) [+ cell (4) when flagged-dead particles may be present], write all five (36)
+#   scatter : read all five (36), write all five (36)
+#   fused   : read x,vx,vy,vz (32), write all five (36)
+ALG_BYTES = {"mover": (68, 72), "scatter": (72, 72), "fused": (68, 68), "hist": (4, 4)}
+
+
+def env_rank():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def committed_traffic(kernel, workload):
+    """DRAM bytes per launch from the committed ncu --set full capture (profiles/traffic.json), or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            t = json.load(f)
+        return t.get(workload, {}).get(kernel)
+    except Exception:
+        return None
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock / throttle reasons of one GPU through NVML while the timed region runs."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, uuid, period=0.004):
+        super().__init__(daemon=True)
+        self.period, self.samples, self.reasons, self.power = period, [], set(), []
+        self.stop_flag = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            try:
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(uuid.encode() if isinstance(uuid, str) else uuid)
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(uuid)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception as e:  # NVML missing: report that rather than invent clocks
+            self.err = repr(e)
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        while not self.stop_flag.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h) if hasattr(nv, "nvmlDeviceGetCurrentClocksEventReasons") \
+                    else nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in self.REASONS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def result(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "note": "NVML unavailable: " + getattr(self, "err", "no samples")}
+        return {"sm_mhz": statistics.median(self.samples), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples), "power_w_max": max(self.power) if self.power else None}
+
+
+# ----------------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline of the main line; the whole of --impl reference)
+# ----------------------------------------------------------------------------------------------
+def oracle_sample(config, nc_sample, steps):
+    """Time the oracle, as it stands (1 thread), on the first nc_sample cells' worth of the workload.
+    Returns (pushes/s, seconds, pushes, description)."""
+    import oracle
+    from paper_2603_24508_b200 import workloads
+    kw = dict(nc=nc_sample)
+    inp = workloads.make(config, **kw)
+    states = []
+    for s in inp["species"]:
+        states.append(oracle.State(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], nc=inp["nc"], dx=inp["dx"], dt=inp["dt"],
+                                   boundary=inp["boundary"], E=inp["E"], qm=s["qm"], B=inp["B"],
+                                   arrange_every=inp["arrange_every"]))
+    oracle.lib()
+    n0 = sum(st.n for st in states)
+    t0 = time.perf_counter()
+    pushes = 0
+    for _ in range(steps):
+        for st in states:
+            pushes += st.n
+            st.push(1)
+    dt = time.perf_counter() - t0
+    desc = (f"config {config} recipe on {nc_sample} cells ({n0} particles, all species), {steps} steps, "
+            f"arrange every {inp['arrange_every']}, oracle/oracle.c single thread")
+    return pushes / dt, dt, pushes, desc
+
+
+SAMPLE_CELLS = {1: 1024, 2: 25000, 3: 10000, 4: 40000, 5: 20000}  # ~4 M particles each (config 1: all of it)
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return 0
+    steps_total = max(1, args.steps)
+    nc_s = SAMPLE_CELLS[args.config]
+    for _ in range(max(0, min(args.warmup, 1))):
+        oracle_sample(args.config, max(64, nc_s // 16), 1)
+    # each "step" of this arm = one oracle step over the bounded sample; cap the total CPU time
+    steps = min(steps_total, 50)
+    v, dt, pushes, desc = oracle_sample(args.config, nc_s, steps)
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(args.config, None),
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0,
+            "note": "no reference code exists (paper only): this arm is the CPU oracle on the host cores"}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def workload_config(config, inp):
+    from paper_2603_24508_b200 import workloads
+    c = workloads.CONFIGS[config]
+    out = {"workload": f"BASELINE.json configs[{config - 1}]: {c['name']}", "nc": c["nc"],
+           "species": list(c["species"]), "boundary": "periodic" if c["boundary"] == 0 else "absorbing",
+           "arrange_every": c["arrange_every"], "parallelism": "single GPU (replicas only for N>1)",
+           "l2": "inputs (GBs of SoA) far exceed the 126 MB L2; no flush between steps"}
+    if inp is not None:
+        out["particles"] = int(sum(len(s["x"]) for s in inp["species"]))
+    return out
+
+
+# ----------------------------------------------------------------------------------------------
+# main arm
+# ----------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the CPU-oracle baseline leg")
+    ap.add_argument("--option", action="append", default=[], help="pic_set_option key=value (e.g. fused=0)")
+    ap.add_argument("--scale", type=float, default=1.0, help="scale nc (debug only; the line is then not a bench value)")
+    args = ap.parse_args()
+    rank, local_rank, world = env_rank()
+    if args.impl == "reference":
+        return run_reference(args, rank)
+
+    import numpy as np
+    import torch
+    import paper_2603_24508_b200 as pic
+    from paper_2603_24508_b200 import workloads
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    pic.lib()  # fails loudly if libpic.so is missing
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    warmup = max(3, args.warmup)
+
+    kw = {}
+    if args.scale != 1.0:
+        kw["nc"] = max(8, int(workloads.CONFIGS[args.config]["nc"] * args.scale))
+    inp = workloads.make(args.config, replica=rank, **kw)
+    ae = inp["arrange_every"]
+    stream = torch.cuda.Stream(device=dev)
+    with torch.cuda.stream(stream):
+        descs = [pic.make_species(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], qm=s["qm"], arrange_every=ae,
+                                  device=dev) for s in inp["species"]]
+    stream.synchronize()
+    sim = pic.pic_create(nc=inp["nc"], dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E_nodes=inp["E"],
+                         B=inp["B"], species=descs, stream=stream)
+    for kv in args.option:
+        k, v = kv.split("=")
+        pic.pic_set_option(sim, k, int(v))
+    pic.pic_set_option(sim, "kernel_timing", 1)
+
+    def step():
+        for sp in sim.species:
+            pic.pic_push(sp, 1)
+
+    for _ in range(warmup):
+        step()
+    pic.pic_sync(sim)
+    for k in ("mover", "hist", "scan", "scatter", "general", "fused"):
+        pic.pic_kernel_time(sim, k)  # drop warm-up spans
+    n_before = sum(pic.pic_n_slots(sp) for sp in sim.species)
+    launches0 = pic.pic_launch_count(sim)
+
+    uuid = str(torch.cuda.get_device_properties(dev).uuid)
+    sampler = ClockSampler(uuid if uuid.startswith("GPU-") else "GPU-" + uuid)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    sampler.stop_flag.set()
+    sampler.join()
+    ms = e0.elapsed_time(e1)
+    launches = pic.pic_launch_count(sim) - launches0
+    n_after = sum(pic.pic_n_slots(sp) for sp in sim.species)
+    pic.pic_sync(sim)  # raises on a deferred device-side error
+    pushes = 0.5 * (n_before + n_after) * args.steps  # n_live changes only by wall absorption (negligible; exact if periodic)
+    ktimes = {k: pic.pic_kernel_time(sim, k) for k in ("mover", "hist", "scan", "scatter", "general", "fused")}
+    info = [pic.pic_arrange_info(sp) for sp in sim.species]
+
+    if dist is not None:
+        t = torch.tensor([ms, pushes], dtype=torch.float64, device=dev)
+        tmax = t.clone()
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        ms_all, pushes_all = float(tmax[0]), float(t[1])
+    else:
+        ms_all, pushes_all = ms, pushes
+    value = pushes_all / (ms_all * 1e-3)
+
+    # roofline of the dominant kernel (this rank)
+    peak, peak_src = measured_peak()
+    dom = max(ktimes, key=lambda k: ktimes[k][0])
+    dom_ms, dom_n = ktimes[dom]
+    all_live = inp["boundary"] == workloads.PERIODIC
+    per_particle = ALG_BYTES.get(dom, (72, 72))[0 if all_live else 1]
+    n_per_launch = 0.5 * (n_before + n_after) / len(sim.species)
+    roofline = None
+    if dom_n:
+        avg_ms = dom_ms / dom_n
+        achieved = per_particle * n_per_launch / (avg_ms * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                    "frac": achieved / peak, "peak_source": peak_src, "avg_launch_ms": avg_ms,
+                    "algorithmic_bytes_per_particle": per_particle, "particles_per_launch": n_per_launch,
+                    "traffic": committed_traffic(dom, f"config{args.config}"),
+                    "kernel_ms_per_step": {k: v[0] / args.steps for k, v in ktimes.items() if v[1]},
+                    "step_algorithmic_GBps": sum(ALG_BYTES[k][0 if all_live else 1] * n_per_launch * v[1]
+                                                 for k, v in ktimes.items() if k in ALG_BYTES) / (ms * 1e-3) / 1e9}
+        roofline["step_frac"] = roofline["step_algorithmic_GBps"] / peak
+    pic.pic_destroy(sim)
+    del descs, sim
+    torch.cuda.empty_cache()
+
+    # e2e: the C-ABI call with HOST buffers (pic_run_host), copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        cfg_steps = inp["steps"]
+        host_species = []
+        h2d = 0
+        for s in inp["species"]:
+            arrs = []
+            for k in ("x", "vx", "vy", "vz", "cell"):
+                t = torch.from_numpy(s[k]).pin_memory()
+                arrs.append(t)
+                h2d += t.numel() * t.element_size()
+            host_species.append(dict(qm=s["qm"], arrays=arrs, arrange_every=ae))
+        h2d += inp["E"].nbytes
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        t0 = time.perf_counter()
+        res = pic.pic_run_host(nc=inp["nc"], dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E_nodes=inp["E"],
+                               B=inp["B"], species=host_species, nsteps=cfg_steps, stream=stream)
+        torch.cuda.synchronize()
+        t_e2e = time.perf_counter() - t0
+        n_out = sum(r[0] for r in res)
+        d2h = n_out * 36 + 16 * len(res)
+        n0_e = sum(len(s["x"]) for s in inp["species"])
+        e_pushes = 0.5 * (n0_e + n_out) * cfg_steps
+        if dist is not None:
+            t = torch.tensor([t_e2e, e_pushes], dtype=torch.float64, device=dev)
+            tm = t.clone()
+            dist.all_reduce(tm, op=dist.ReduceOp.MAX)
+            dist.all_reduce(t, op=dist.ReduceOp.SUM)
+            t_e2e, e_pushes = float(tm[0]), float(t[1])
+        e2e = {"value": e_pushes / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d / cfg_steps,
+               "d2h_bytes_per_step": d2h / cfg_steps, "steps": cfg_steps, "seconds": t_e2e,
+               "call": "pic_run_host (pinned host SoA in, cudaMalloc + H2D + pic_create + pic_push(nsteps) + D2H + free inside)"}
+        del host_species
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        v, dt_cpu, _, desc = oracle_sample(args.config, min(SAMPLE_CELLS[args.config], inp["nc"]), 50 if args.config != 1 else 200)
+        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc, "seconds": dt_cpu,
+               "host_cores_available": os.cpu_count()}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warmup,
+                "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic", "config": workload_config(args.config, inp),
+                "clocks": sampler.result(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+                "cpu_baseline": cpu,
+                "path": {"arranger": ["general" if g else "fast" for (_, g) in info],
+                         "options": args.option, "numpy": np.__version__}}
+        if args.scale != 1.0:
+            line["config"]["scaled_nc"] = inp["nc"]
+            line["config"]["workload"] += f" SCALED x{args.scale} (debug, not a bench value)"
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -153,9 +153,17 @@ size_t pic_workspace_bytes(int32_t nc, int64_t capacity);
 /* Mover/arranger variant switches for measurements (profiles/ compares them):
  * key "e_stage": 0 = E through the read-only global path, 1 = E window staged in
  * shared memory by TMA bulk copy (default); key "fused": 1 = single-pass push+arrange
- * when arrange_every == 1 (default), 0 = separate mover / scan / scatter kernels.
+ * when arrange_every == 1 (default), 0 = separate mover / scan / scatter kernels; key
+ * "kernel_timing": 1 = record CUDA events around every kernel launch (see pic_kernel_time).
  * PIC_EINVAL for an unknown key or value. */
 int pic_set_option(pic_sim *sim, const char *key, int value);
+
+/* Device time of one kernel class since the previous query of that class, measured with CUDA
+ * event pairs recorded on the sim's stream around each of its launches while option
+ * "kernel_timing" is 1 (default 0: nothing is recorded).  kernel is one of "mover", "hist",
+ * "scan", "scatter", "general", "fused".  *ms_total = summed milliseconds, *spans = number of
+ * timed launches (either may be NULL).  Syncs.  PIC_EINVAL for an unknown name. */
+int pic_kernel_time(pic_sim *sim, const char *kernel, double *ms_total, uint64_t *spans);
 
 /* Number of kernel launches the library has enqueued for this sim since pic_create. */
 int pic_launch_count(pic_sim *sim, uint64_t *launches);

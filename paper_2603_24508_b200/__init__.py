@@ -21,7 +21,7 @@ EXPORTS = [
     "pic_create", "pic_species_at", "pic_push", "pic_arrange", "pic_wall_flux", "pic_set_field", "pic_n_slots",
     "pic_active_buffer", "pic_cell_counts", "pic_step_count", "pic_arrange_info", "pic_workspace_bytes",
     "pic_set_option", "pic_launch_count", "pic_sync", "pic_destroy", "pic_strerror", "pic_last_error",
-    "pic_run_host",
+    "pic_run_host", "pic_kernel_time",
 ]
 
 
@@ -87,6 +87,7 @@ def lib():
         L.pic_workspace_bytes.restype = C.c_size_t
         L.pic_set_option.argtypes = [vp, C.c_char_p, C.c_int]
         L.pic_launch_count.argtypes = [vp, C.POINTER(C.c_uint64)]
+        L.pic_kernel_time.argtypes = [vp, C.c_char_p, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
         L.pic_sync.argtypes = [vp]
         L.pic_destroy.argtypes = [vp]
         L.pic_destroy.restype = None
@@ -270,6 +271,13 @@ def pic_launch_count(sim):
     n = C.c_uint64()
     _check(lib().pic_launch_count(sim.handle, C.byref(n)), "pic_launch_count")
     return n.value
+
+
+def pic_kernel_time(sim, kernel):
+    """-> (milliseconds, timed launches) of one kernel class since the previous query (option kernel_timing)."""
+    ms, n = C.c_double(), C.c_uint64()
+    _check(lib().pic_kernel_time(sim.handle, kernel.encode(), C.byref(ms), C.byref(n)), "pic_kernel_time")
+    return ms.value, n.value
 
 
 def pic_sync(sim):

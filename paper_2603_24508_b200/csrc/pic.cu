@@ -31,6 +31,9 @@ static int cuda_fail(cudaError_t e, const char *what)
         if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
     } while (0)
 
+enum { K_MOVER = 0, K_HIST, K_SCAN, K_SCATTER, K_GENERAL, K_FUSED, K_COUNT };
+static const char *const K_NAMES[K_COUNT] = {"mover", "hist", "scan", "scatter", "general", "fused"};
+
 struct pic_species {
     pic_sim *sim = nullptr;
     PushConst k{};
@@ -63,8 +66,40 @@ struct pic_sim {
     double B[3]{};
     std::vector<pic_species *> sp;
     unsigned long long launches = 0;
-    int opt_e_stage = 1, opt_fused = 1;
+    int opt_e_stage = 1, opt_fused = 1, opt_timing = 0;
     int sm_count = 148;
+    // per-kernel device timing (option "kernel_timing"): event pairs recorded around launches
+    struct Span { int id; cudaEvent_t a, b; };
+    std::vector<Span> spans;
+    std::vector<cudaEvent_t> free_events;
+    double k_ms[K_COUNT] = {};
+    unsigned long long k_launches[K_COUNT] = {};
+};
+
+// Records an event pair around the launches made during its lifetime (only when timing is on).
+struct KernelSpan {
+    pic_sim *sim;
+    cudaEvent_t a = nullptr, b = nullptr;
+    int id;
+    static cudaEvent_t get(pic_sim *sim)
+    {
+        if (!sim->free_events.empty()) { cudaEvent_t e = sim->free_events.back(); sim->free_events.pop_back(); return e; }
+        cudaEvent_t e = nullptr;
+        if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        return e;
+    }
+    KernelSpan(pic_sim *s, int kid) : sim(s), id(kid)
+    {
+        if (!sim->opt_timing) return;
+        a = get(sim); b = get(sim);
+        if (a) cudaEventRecord(a, sim->stream);
+    }
+    ~KernelSpan()
+    {
+        if (!a || !b) return;
+        cudaEventRecord(b, sim->stream);
+        sim->spans.push_back({id, a, b});
+    }
 };
 
 static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -106,6 +141,8 @@ extern "C" void pic_destroy(pic_sim *sim)
     if (!sim) return;
     cudaStreamSynchronize(sim->stream);
     for (pic_species *s : sim->sp) free_species(s);
+    for (auto &sp : sim->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
+    for (cudaEvent_t e : sim->free_events) cudaEventDestroy(e);
     cudaFree(sim->d_E);
     delete sim;
 }
@@ -151,6 +188,7 @@ static int run_scan(pic_species *s, const int *in, int *out, int m, ScanFold fol
     size_t words = scan_scratch_words(m);
     CU(cudaMemsetAsync(s->d_scan, 0, words * sizeof(unsigned long long), sim->stream));
     int ntiles = (m + SCAN_TILE - 1) / SCAN_TILE;
+    KernelSpan span(sim, K_SCAN);
     scan_exclusive_kernel<<<ntiles, SCAN_THREADS, 0, sim->stream>>>(in, out, m, s->d_scan, fold);
     return launch_check(sim, "scan_exclusive_kernel");
 }
@@ -311,8 +349,36 @@ extern "C" int pic_set_option(pic_sim *sim, const char *key, int value)
 {
     if (!sim || !key || (value != 0 && value != 1)) return PIC_EINVAL;
     if (!strcmp(key, "e_stage")) sim->opt_e_stage = value;
+    else if (!strcmp(key, "kernel_timing")) sim->opt_timing = value;
     else if (!strcmp(key, "fused")) sim->opt_fused = value;
     else return PIC_EINVAL;
+    return PIC_OK;
+}
+
+extern "C" int pic_kernel_time(pic_sim *sim, const char *kernel, double *ms_total, uint64_t *spans)
+{
+    if (!sim || !kernel) return PIC_EINVAL;
+    int id = -1;
+    for (int k = 0; k < K_COUNT; ++k)
+        if (!strcmp(kernel, K_NAMES[k])) id = k;
+    if (id < 0) return PIC_EINVAL;
+    CU(cudaStreamSynchronize(sim->stream));
+    for (auto &sp : sim->spans) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, sp.a, sp.b) == cudaSuccess) {
+            sim->k_ms[sp.id] += ms;
+            sim->k_launches[sp.id]++;
+        } else {
+            cudaGetLastError();
+        }
+        sim->free_events.push_back(sp.a);
+        sim->free_events.push_back(sp.b);
+    }
+    sim->spans.clear();
+    if (ms_total) *ms_total = sim->k_ms[id];
+    if (spans) *spans = sim->k_launches[id];
+    sim->k_ms[id] = 0;
+    sim->k_launches[id] = 0;
     return PIC_OK;
 }
 
@@ -336,6 +402,7 @@ static int arrange_split(pic_species *s, bool hist_ready)
         CU(cudaMemsetAsync(s->d_count[on], 0, sizeof(int) * (size_t)nc, sim->stream));
         if (s->n_ub > 0) {
             int blocks = (int)((s->n_ub + HIST_THREADS * HIST_ITEMS - 1) / (HIST_THREADS * HIST_ITEMS));
+            KernelSpan span(sim, K_HIST);
             hist_kernel<<<blocks, HIST_THREADS, 0, sim->stream>>>(s->cell[src], s->d_count[on], s->d_st);
             if (int rc = launch_check(sim, "hist_kernel")) return rc;
         }
@@ -353,6 +420,7 @@ static int arrange_split(pic_species *s, bool hist_ready)
     {
         long long want = ((long long)nc + SCATTER_THREADS / 32 - 1) / (SCATTER_THREADS / 32);
         int blocks = (int)std::min<long long>(want, (long long)sim->sm_count * 64);
+        KernelSpan span(sim, K_SCATTER);
         scatter_fast_kernel<<<blocks, SCATTER_THREADS, 0, sim->stream>>>(a);
         if (int rc = launch_check(sim, "scatter_fast_kernel")) return rc;
     }
@@ -363,6 +431,7 @@ static int arrange_split(pic_species *s, bool hist_ready)
     ga.st = s->d_st; ga.nc = nc; ga.n_ub = s->n_ub; ga.ws = s->ws; ga.ws_bytes = s->ws_bytes;
     ga.off_old = s->d_off[oo];
     ga.scan_scratch = s->d_scan;
+    KernelSpan gspan(sim, K_GENERAL);
     if (int rc = general_arrange(ga, sim->stream, sim->sm_count, &sim->launches)) return rc == PIC_ECUDA ? cuda_fail(cudaGetLastError(), "general_arrange") : rc;
 
     s->cur = dst;
@@ -402,6 +471,7 @@ static int push_split(pic_species *s, bool will_arrange)
         long long pairs = (s->n_ub + 1) / 2;
         int blocks = (int)((pairs + MOVER_THREADS - 1) / MOVER_THREADS);
         const bool rc = !s->all_live;
+        KernelSpan span(sim, K_MOVER);
         if (rc) { if (will_arrange) launch_mover<true, true>(s, a, blocks); else launch_mover<true, false>(s, a, blocks); }
         else    { if (will_arrange) launch_mover<false, true>(s, a, blocks); else launch_mover<false, false>(s, a, blocks); }
         if (int r = launch_check(sim, "mover_kernel")) return r;

@@ -88,15 +88,18 @@ def particles(counts, vth, rng):
     return x, vx, vy, vz, cell
 
 
-def make(config, *, nc=None, ppc=None, n_total=None, steps=None):
+def make(config, *, nc=None, ppc=None, n_total=None, steps=None, replica=0):
     """Inputs of BASELINE.json config `config` (1..5), optionally scaled down (nc / ppc / n_total /
-    steps overrides, used by the parity tests).  Returns a dict of plain numpy arrays and scalars."""
+    steps overrides, used by the parity tests).  replica > 0 draws an independent replica of the same
+    workload (seed + 100000*replica; bench.py gives every rank its own).  Returns a dict of plain
+    numpy arrays and scalars."""
     cfg = CONFIGS[config]
     nc = int(nc if nc is not None else cfg["nc"])
     ppc = ppc if ppc is not None else cfg["ppc"]
     if cfg["density"] == "gaussian":
         n_total = int(n_total if n_total is not None else round(cfg["n_total"] * (nc / cfg["nc"])))
-    rng = np.random.Generator(np.random.PCG64(SEED0 + config))
+    seed = SEED0 + config + 100000 * int(replica)
+    rng = np.random.Generator(np.random.PCG64(seed))
     E = field(cfg, nc, rng)
     B0 = cfg["wcdt"] / (abs(QM["e"]) * DT)
     th = math.radians(cfg["theta"])
@@ -104,7 +107,7 @@ def make(config, *, nc=None, ppc=None, n_total=None, steps=None):
     counts = cell_counts(cfg, nc, ppc, n_total)
     species = []
     for si, name in enumerate(cfg["species"]):
-        srng = rng if si == 0 else np.random.Generator(np.random.PCG64(SEED0 + config + 1000 * si))
+        srng = rng if si == 0 else np.random.Generator(np.random.PCG64(seed + 1000 * si))
         vth = cfg["vth"] if name == "e" else cfg["vth"] * math.sqrt(1.0 / MASS_RATIO)
         x, vx, vy, vz, cell = particles(counts, vth, srng)
         species.append(dict(name=name, qm=QM[name], x=x, vx=vx, vy=vy, vz=vz, cell=cell))
