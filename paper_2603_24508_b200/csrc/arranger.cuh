@@ -28,22 +28,35 @@ __global__ void __launch_bounds__(HIST_THREADS) hist_kernel(const int *__restric
 }
 
 // ---- initial-state validation (pic_create) -------------------------------------------------
-__global__ void validate_kernel(const double *__restrict__ x, const int *__restrict__ cell, PushConst k, DevState *st)
+// Checks 0 <= x < L, cell == min(floor(x*inv_dx), nc-1), all live; notes whether the state is grouped
+// by cell; records the initial speed bound max |v|^2 (float, rounded up) in st->vmax2.
+__global__ void validate_kernel(const double *__restrict__ x, const double *__restrict__ vx, const double *__restrict__ vy,
+                                const double *__restrict__ vz, const int *__restrict__ cell, PushConst k, DevState *st)
 {
     const int n = st->n;
-    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    int c = cell[i];
-    double xv = x[i];
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool valid = i < n;
     int err = 0;
-    if (c < 0 || c >= k.nc || !(xv >= 0.0) || !(xv < k.L)) err = ERR_BAD_INITIAL;
-    else {
-        int cf = (int)floor(__dmul_rn(xv, k.inv_dx));
-        if (cf > k.nc - 1) cf = k.nc - 1;
-        if (cf != c) err = ERR_BAD_INITIAL;
+    unsigned m = 0;
+    if (valid) {
+        const int c = cell[i];
+        const double xv = x[i];
+        if (c < 0 || c >= k.nc || !(xv >= 0.0) || !(xv < k.L)) err = ERR_BAD_INITIAL;
+        else {
+            int cf = (int)floor(__dmul_rn(xv, k.inv_dx));
+            if (cf > k.nc - 1) cf = k.nc - 1;
+            if (cf != c) err = ERR_BAD_INITIAL;
+        }
+        if (i > 0 && cell[i - 1] > c) err |= ERR_NOT_GROUPED;
+        const double a = vx[i], b = vy[i], d = vz[i];
+        m = __float_as_uint(__double2float_ru(a * a + b * b + d * d));
     }
-    if (i > 0 && cell[i - 1] > c) err |= ERR_NOT_GROUPED;
-    if (err) atomicOr(&st->status, err);
+    err = (int)__reduce_or_sync(FULL, (unsigned)err);
+    m = __reduce_max_sync(FULL, m);
+    if ((threadIdx.x & 31) == 0) {
+        if (err) atomicOr(&st->status, err);
+        if (m > *(volatile unsigned *)&st->vmax2) atomicMax(&st->vmax2, m);
+    }
 }
 
 // ---- a-7: destination-driven stable scatter ---------------------------------------------------
@@ -62,6 +75,7 @@ struct ScatterArgs {
     const int *count_new; // nc
     const int *off_new;   // nc+1
     DevState *st;
+    const int *guard; // if not NULL: the kernel returns at once unless *guard != 0
     int nc, periodic, w_limit;
 };
 
@@ -89,6 +103,7 @@ __device__ __forceinline__ int scatter_range(const ScatterArgs &a, int c, int ba
 
 __global__ void __launch_bounds__(SCATTER_THREADS) scatter_fast_kernel(ScatterArgs a)
 {
+    if (a.guard && !*a.guard) return;
     const int W = a.st->w_acc;
     if (W > a.w_limit) {
         if (blockIdx.x == 0 && threadIdx.x == 0) a.st->need_general = 1;

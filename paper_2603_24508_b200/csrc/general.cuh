@@ -177,7 +177,7 @@ static inline int general_arrange(const GeneralArgs &a, cudaStream_t stream, int
         ++*launches;
         const int m = (int)(GEN_RADIX * ntiles);
         if (cudaMemsetAsync(a.scan_scratch, 0, scan_scratch_words(m) * sizeof(unsigned long long), stream) != cudaSuccess) return -3;
-        ScanFold nofold{nullptr, 0, 0, &a.st->need_general};
+        ScanFold nofold{nullptr, 0, 0, 0, &a.st->need_general};
         scan_exclusive_kernel<<<(m + SCAN_TILE - 1) / SCAN_TILE, SCAN_THREADS, 0, stream>>>(hist, hist, m, a.scan_scratch, nofold);
         ++*launches;
         gen_scatter_kernel<<<grid, GEN_THREADS, 0, stream>>>(key[cur], val[cur], key[cur ^ 1], val[cur ^ 1], hist, shift,

@@ -13,6 +13,7 @@ struct MoverArgs {
     const double *E;  // nc+1 nodes
     int *count;       // per-cell histogram of the new cells (HIST only), pre-zeroed
     DevState *st;
+    const int *guard; // if not NULL: the kernel returns at once unless *guard != 0
     PushConst k;
 };
 
@@ -21,8 +22,10 @@ constexpr int MOVER_THREADS = 256;
 template <bool READ_CELL, bool HIST>
 __global__ void __launch_bounds__(MOVER_THREADS) mover_kernel(MoverArgs a)
 {
+    if (a.guard && !*a.guard) return;
     __shared__ int s_max;
-    if (threadIdx.x == 0) s_max = 0;
+    __shared__ unsigned s_vmax;
+    if (threadIdx.x == 0) { s_max = 0; s_vmax = 0; }
     __syncthreads();
 
     const int n = a.st->n;
@@ -50,6 +53,7 @@ __global__ void __launch_bounds__(MOVER_THREADS) mover_kernel(MoverArgs a)
     }
 
     int dmax = 0, nleft = 0, nright = 0, bad = 0;
+    float vm2 = 0.f; // upper bound of max |v'|^2 (feeds the next step's displacement bound)
     int cn[2] = {-1, -1};
 #pragma unroll
     for (int q = 0; q < 2; ++q) {
@@ -61,6 +65,7 @@ __global__ void __launch_bounds__(MOVER_THREADS) mover_kernel(MoverArgs a)
                 PushOut o;
                 push_core(a.k, x[q], vx[q], vy[q], vz[q], xs, jf, j, E0, E1, o);
                 x[q] = o.x; vx[q] = o.vx; vy[q] = o.vy; vz[q] = o.vz;
+                vm2 = fmaxf(vm2, __double2float_ru(o.vx * o.vx + o.vy * o.vy + o.vz * o.vz));
                 cn[q] = o.cell;
                 dmax = max(dmax, o.dcell);
                 nleft += (o.wall == 1); nright += (o.wall == 2);
@@ -98,8 +103,13 @@ __global__ void __launch_bounds__(MOVER_THREADS) mover_kernel(MoverArgs a)
     }
     int wmax = __reduce_max_sync(FULL, dmax);
     if (lane == 0 && wmax > 0) atomicMax(&s_max, wmax);
+    unsigned vmw = __reduce_max_sync(FULL, __float_as_uint(vm2));
+    if (lane == 0 && vmw) atomicMax(&s_vmax, vmw);
     __syncthreads();
-    if (threadIdx.x == 0 && s_max > *(volatile int *)&a.st->step_max) atomicMax(&a.st->step_max, s_max);
+    if (threadIdx.x == 0) {
+        if (s_max > *(volatile int *)&a.st->step_max) atomicMax(&a.st->step_max, s_max);
+        if (s_vmax > *(volatile unsigned *)&a.st->vmax2_next) atomicMax(&a.st->vmax2_next, s_vmax);
+    }
 }
 
 // End of a mover step that is not followed by an arrange: fold the step's displacement
@@ -109,6 +119,8 @@ __global__ void end_step_kernel(DevState *st, int reset)
     int w = (reset ? 0 : st->w_acc) + st->step_max;
     st->w_acc = w > W_UNKNOWN ? W_UNKNOWN : w;
     st->step_max = 0;
+    st->vmax2 = st->vmax2_next;
+    st->vmax2_next = 0;
 }
 
 } // namespace pic

@@ -48,7 +48,20 @@ struct pic_species {
     int cur_off = 0; // d_off[cur_off] / d_count[cur_off] describe the last arrange
     unsigned long long *d_scan = nullptr;
     size_t scan_words = 0;
-    FusedScratch fused{};
+    // fused push+arrange step (fused.cuh)
+    int *d_bound[2]{};                 // block partition of d_off[i]: first cell with offset >= k*T
+    unsigned long long *d_chain = nullptr;
+    int T = FUSED_T_DEFAULT, nb_cap = 0;
+    unsigned epoch = 0;
+    bool bounds_valid = false;         // d_bound[cur_off] describes d_off[cur_off]
+    bool fused_off = false;            // the device reported a declined fused step (sticky)
+    // host-side conservative bound on cell displacement since the last arrange (decides whether the
+    // general-path kernels need to be enqueued at all)
+    double vkick = 0;                  // 2*|h|*max|E|
+    double h_vmax = 0;                 // speed bound at the last sync
+    long long h_steps_since_sync = 0;
+    long long h_wsum = 0;              // sum of per-step displacement bounds since the last arrange
+    bool h_grouped = false;
     void *ws = nullptr;
     size_t ws_bytes = 0;
     long long steps = 0, steps_at_last_flux = 0;
@@ -64,6 +77,7 @@ struct pic_sim {
     int nc = 0, periodic = 0;
     double dx = 0, dt = 0;
     double B[3]{};
+    double Emax = 0; // max |E_node|
     std::vector<pic_species *> sp;
     unsigned long long launches = 0;
     int opt_e_stage = 1, opt_fused = 1, opt_timing = 0;
@@ -131,8 +145,9 @@ static void free_species(pic_species *s)
     cudaFree(s->d_st);
     for (int b = 0; b < 2; ++b) { cudaFree(s->d_count[b]); cudaFree(s->d_off[b]); }
     cudaFree(s->d_scan);
-    cudaFree(s->fused.block_state);
-    cudaFree(s->fused.cell_bound);
+    cudaFree(s->d_bound[0]);
+    cudaFree(s->d_bound[1]);
+    cudaFree(s->d_chain);
     delete s;
 }
 
@@ -193,6 +208,38 @@ static int run_scan(pic_species *s, const int *in, int *out, int m, ScanFold fol
     return launch_check(sim, "scan_exclusive_kernel");
 }
 
+static float bits_to_float(unsigned u)
+{
+    float f;
+    memcpy(&f, &u, sizeof f);
+    return f;
+}
+
+// bound[] (block partition of the fused step) from the offsets in slot `which`
+static int run_bounds(pic_species *s, int which, const int *guard)
+{
+    pic_sim *sim = s->sim;
+    const int nc = sim->nc;
+    bounds_kernel<<<(nc + 255) / 256, 256, 0, sim->stream>>>(s->d_off[which], nc, s->T, s->d_bound[which], s->nb_cap, guard);
+    if (int rc = launch_check(sim, "bounds_kernel")) return rc;
+    if (!guard) s->bounds_valid = true;
+    return PIC_OK;
+}
+
+static bool fused_possible(const pic_species *s)
+{
+    return s->sim->opt_fused && !s->fused_off && s->arrange_every == 1 && s->sim->nc >= FUSED_MIN_NC;
+}
+
+// Host-side bound (cells) on what one more mover step can displace any particle.
+static long long host_step_bound(pic_species *s)
+{
+    const double v = s->h_vmax * (1.0 + 1e-6) + (double)(s->h_steps_since_sync + 1) * s->vkick;
+    const double reach = v * s->k.dt * s->k.inv_dx;
+    if (!(reach < 1e9)) return 1LL << 40;
+    return (long long)std::ceil(reach + 1e-9) + 1;
+}
+
 // ------------------------------------------------------------------------------------------
 // create
 // ------------------------------------------------------------------------------------------
@@ -250,7 +297,7 @@ static int create_species(pic_sim *sim, const pic_species_desc &d, pic_species *
     // validate the initial state, build count/offset of the initial grouping
     if (d.n > 0) {
         int blocks = (int)((d.n + 255) / 256);
-        validate_kernel<<<blocks, 256, 0, sim->stream>>>(s->x[0], s->cell[0], s->k, s->d_st);
+        validate_kernel<<<blocks, 256, 0, sim->stream>>>(s->x[0], s->vx[0], s->vy[0], s->vz[0], s->cell[0], s->k, s->d_st);
         if (int rc = launch_check(sim, "validate_kernel")) return rc;
     }
     CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, sim->stream));
@@ -265,8 +312,23 @@ static int create_species(pic_sim *sim, const pic_species_desc &d, pic_species *
         hist_kernel<<<blocks, HIST_THREADS, 0, sim->stream>>>(s->cell[0], s->d_count[0], s->d_st);
         if (int rc = launch_check(sim, "hist_kernel")) return rc;
     }
-    ScanFold nofold{nullptr, 0, 0, nullptr};
+    ScanFold nofold{nullptr, 0, 0, 0, nullptr};
     if (int rc = run_scan(s, s->d_count[0], s->d_off[0], nc, nofold)) return rc;
+    // fused step: block partition, look-back chain
+    s->T = FUSED_T_DEFAULT;
+    s->nb_cap = (int)(d.capacity / s->T) + 2;
+    for (int b = 0; b < 2; ++b) {
+        CU(cudaMalloc(&s->d_bound[b], sizeof(int) * ((size_t)s->nb_cap + 2)));
+        CU(cudaMemsetAsync(s->d_bound[b], 0, sizeof(int) * ((size_t)s->nb_cap + 2), sim->stream));
+    }
+    CU(cudaMalloc(&s->d_chain, sizeof(unsigned long long) * ((size_t)s->nb_cap + 2)));
+    CU(cudaMemsetAsync(s->d_chain, 0, sizeof(unsigned long long) * ((size_t)s->nb_cap + 2), sim->stream));
+    s->vkick = 2.0 * std::fabs(s->k.h) * sim->Emax;
+    s->h_vmax = std::sqrt((double)bits_to_float(h.vmax2));
+    s->h_grouped = grouped;
+    s->bounds_valid = false;
+    if (grouped)
+        if (int rc = run_bounds(s, 0, nullptr)) return rc;
     h.status = 0;
     h.w_acc = grouped ? 0 : W_UNKNOWN;
     CU(cudaMemcpyAsync(s->d_st, &h, sizeof h, cudaMemcpyHostToDevice, sim->stream));
@@ -276,7 +338,13 @@ static int create_species(pic_sim *sim, const pic_species_desc &d, pic_species *
     s->counts_fresh = grouped;
     s->all_live = true;
     s->reset_w = false;
-    if (int rc = fused_alloc(s->fused, nc, d.capacity)) return rc == PIC_ENOMEM ? PIC_ENOMEM : cuda_fail(cudaGetLastError(), "fused_alloc");
+    {
+        static bool attr_set = false;
+        if (!attr_set) {
+            CU(cudaFuncSetAttribute(fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedShared)));
+            attr_set = true;
+        }
+    }
     return PIC_OK;
 }
 
@@ -289,8 +357,11 @@ extern "C" int pic_create(const pic_grid_desc *g, const pic_species_desc *specie
     if (g->boundary != PIC_PERIODIC && g->boundary != PIC_ABSORBING) return PIC_EINVAL;
     for (int a = 0; a < 3; ++a)
         if (!std::isfinite(g->B[a])) return PIC_EINVAL;
-    for (int j = 0; j <= g->nc; ++j)
+    double emax = 0;
+    for (int j = 0; j <= g->nc; ++j) {
         if (!std::isfinite(g->E_nodes[j])) return PIC_EINVAL;
+        emax = std::max(emax, std::fabs(g->E_nodes[j]));
+    }
 
     int dev = 0;
     CU(cudaGetDevice(&dev));
@@ -302,6 +373,7 @@ extern "C" int pic_create(const pic_grid_desc *g, const pic_species_desc *specie
     sim->dx = g->dx;
     sim->dt = g->dt;
     for (int a = 0; a < 3; ++a) sim->B[a] = g->B[a];
+    sim->Emax = emax;
     int rc = PIC_OK;
     do {
         cudaError_t e = cudaDeviceGetAttribute(&sim->sm_count, cudaDevAttrMultiProcessorCount, dev);
@@ -338,8 +410,13 @@ extern "C" pic_species *pic_species_at(pic_sim *sim, int i)
 extern "C" int pic_set_field(pic_sim *sim, const double *E)
 {
     if (!sim || !E) return PIC_EINVAL;
-    for (int j = 0; j <= sim->nc; ++j)
+    double emax = 0;
+    for (int j = 0; j <= sim->nc; ++j) {
         if (!std::isfinite(E[j])) return PIC_EINVAL;
+        emax = std::max(emax, std::fabs(E[j]));
+    }
+    sim->Emax = emax;
+    for (pic_species *s : sim->sp) s->vkick = 2.0 * std::fabs(s->k.h) * emax;
     CU(cudaMemcpyAsync(sim->d_E, E, sizeof(double) * ((size_t)sim->nc + 1), cudaMemcpyHostToDevice, sim->stream));
     CU(cudaStreamSynchronize(sim->stream)); // E is a caller buffer that may be pageable
     return PIC_OK;
@@ -392,7 +469,10 @@ extern "C" int pic_launch_count(pic_sim *sim, uint64_t *launches)
 // ------------------------------------------------------------------------------------------
 // arrange (split path): [histogram] -> scan -> destination-driven scatter [-> general path]
 // ------------------------------------------------------------------------------------------
-static int arrange_split(pic_species *s, bool hist_ready)
+// guard: NULL = run; else a device flag, every kernel returns at once unless it is non-zero (the
+// fallback chain enqueued behind a fused step).  after_mover: a mover step ran since the last
+// fold, so the scan's fold also commits its speed bound.
+static int arrange_split(pic_species *s, bool hist_ready, const int *guard, bool after_mover)
 {
     pic_sim *sim = s->sim;
     const int nc = sim->nc;
@@ -407,8 +487,7 @@ static int arrange_split(pic_species *s, bool hist_ready)
             if (int rc = launch_check(sim, "hist_kernel")) return rc;
         }
     }
-    ScanFold fold{s->d_st, s->reset_w ? 1 : 0, 1, nullptr};
-    s->reset_w = false;
+    ScanFold fold{s->d_st, (s->reset_w || guard) ? 1 : 0, 1, after_mover ? 1 : 0, guard};
     if (int rc = run_scan(s, s->d_count[on], s->d_off[on], nc, fold)) return rc;
 
     ScatterArgs a{};
@@ -417,6 +496,7 @@ static int arrange_split(pic_species *s, bool hist_ready)
     a.off_old = s->d_off[oo]; a.count_new = s->d_count[on]; a.off_new = s->d_off[on];
     a.st = s->d_st; a.nc = nc; a.periodic = sim->periodic;
     a.w_limit = FAST_W_LIMIT;
+    a.guard = guard;
     {
         long long want = ((long long)nc + SCATTER_THREADS / 32 - 1) / (SCATTER_THREADS / 32);
         int blocks = (int)std::min<long long>(want, (long long)sim->sm_count * 64);
@@ -424,28 +504,39 @@ static int arrange_split(pic_species *s, bool hist_ready)
         scatter_fast_kernel<<<blocks, SCATTER_THREADS, 0, sim->stream>>>(a);
         if (int rc = launch_check(sim, "scatter_fast_kernel")) return rc;
     }
-    // general path: every kernel returns at once unless scatter_fast_kernel declined
-    GeneralArgs ga{};
-    ga.sx = a.sx; ga.svx = a.svx; ga.svy = a.svy; ga.svz = a.svz; ga.scell = a.scell;
-    ga.dx = a.dx; ga.dvx = a.dvx; ga.dvy = a.dvy; ga.dvz = a.dvz; ga.dcell = a.dcell;
-    ga.st = s->d_st; ga.nc = nc; ga.n_ub = s->n_ub; ga.ws = s->ws; ga.ws_bytes = s->ws_bytes;
-    ga.off_old = s->d_off[oo];
-    ga.scan_scratch = s->d_scan;
-    KernelSpan gspan(sim, K_GENERAL);
-    if (int rc = general_arrange(ga, sim->stream, sim->sm_count, &sim->launches)) return rc == PIC_ECUDA ? cuda_fail(cudaGetLastError(), "general_arrange") : rc;
+    // general path: enqueued only if the host-side displacement bound cannot rule it out; every
+    // kernel of it returns at once unless scatter_fast_kernel declined on the device
+    if (!(s->h_grouped && s->h_wsum <= FAST_W_LIMIT)) {
+        GeneralArgs ga{};
+        ga.sx = a.sx; ga.svx = a.svx; ga.svy = a.svy; ga.svz = a.svz; ga.scell = a.scell;
+        ga.dx = a.dx; ga.dvx = a.dvx; ga.dvy = a.dvy; ga.dvz = a.dvz; ga.dcell = a.dcell;
+        ga.st = s->d_st; ga.nc = nc; ga.n_ub = s->n_ub; ga.ws = s->ws; ga.ws_bytes = s->ws_bytes;
+        ga.off_old = s->d_off[oo];
+        ga.scan_scratch = s->d_scan;
+        KernelSpan gspan(sim, K_GENERAL);
+        if (int rc = general_arrange(ga, sim->stream, sim->sm_count, &sim->launches)) return rc == PIC_ECUDA ? cuda_fail(cudaGetLastError(), "general_arrange") : rc;
+    }
+    if (fused_possible(s)) {
+        if (int rc = run_bounds(s, on, guard)) return rc;
+        s->bounds_valid = true;
+    } else {
+        s->bounds_valid = false;
+    }
 
     s->cur = dst;
     s->cur_off = on;
     s->counts_fresh = true;
     s->all_live = true;
     s->reset_w = true;
+    s->h_wsum = 0;
+    s->h_grouped = true;
     return PIC_OK;
 }
 
 extern "C" int pic_arrange(pic_species *s)
 {
     if (!s) return PIC_EINVAL;
-    return arrange_split(s, false);
+    return arrange_split(s, false, nullptr, false);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -457,17 +548,24 @@ static void launch_mover(pic_species *s, const MoverArgs &a, int blocks)
     mover_kernel<RC, H><<<blocks, MOVER_THREADS, 0, s->sim->stream>>>(a);
 }
 
-static int push_split(pic_species *s, bool will_arrange)
+static int push_split(pic_species *s, bool will_arrange, const int *guard)
 {
     pic_sim *sim = s->sim;
     const int nc = sim->nc;
     const int on = s->cur_off ^ 1;
-    if (will_arrange) CU(cudaMemsetAsync(s->d_count[on], 0, sizeof(int) * (size_t)nc, sim->stream));
+    if (will_arrange) {
+        if (guard) {
+            zero_guarded_kernel<<<sim->sm_count, 256, 0, sim->stream>>>(s->d_count[on], nc, guard);
+            if (int r = launch_check(sim, "zero_guarded_kernel")) return r;
+        } else {
+            CU(cudaMemsetAsync(s->d_count[on], 0, sizeof(int) * (size_t)nc, sim->stream));
+        }
+    }
     if (s->n_ub > 0) {
         MoverArgs a{};
         a.x = s->x[s->cur]; a.vx = s->vx[s->cur]; a.vy = s->vy[s->cur]; a.vz = s->vz[s->cur];
         a.cell = s->cell[s->cur];
-        a.E = sim->d_E; a.count = s->d_count[on]; a.st = s->d_st; a.k = s->k;
+        a.E = sim->d_E; a.count = s->d_count[on]; a.st = s->d_st; a.k = s->k; a.guard = guard;
         long long pairs = (s->n_ub + 1) / 2;
         int blocks = (int)((pairs + MOVER_THREADS - 1) / MOVER_THREADS);
         const bool rc = !s->all_live;
@@ -475,6 +573,10 @@ static int push_split(pic_species *s, bool will_arrange)
         if (rc) { if (will_arrange) launch_mover<true, true>(s, a, blocks); else launch_mover<true, false>(s, a, blocks); }
         else    { if (will_arrange) launch_mover<false, true>(s, a, blocks); else launch_mover<false, false>(s, a, blocks); }
         if (int r = launch_check(sim, "mover_kernel")) return r;
+    }
+    if (!guard) {
+        s->h_wsum = std::min<long long>(s->h_wsum + host_step_bound(s), 1LL << 40);
+        s->h_steps_since_sync++;
     }
     if (!sim->periodic) s->all_live = false;
     s->counts_fresh = false;
@@ -486,15 +588,60 @@ static int push_split(pic_species *s, bool will_arrange)
     return PIC_OK;
 }
 
+// One fused push+arrange step, followed by the guarded split chain that redoes the step if the
+// fused kernel declined on the device (DevState::run_split).
+static int push_fused(pic_species *s)
+{
+    pic_sim *sim = s->sim;
+    const int src = s->cur, dst = s->cur ^ 1;
+    const int oo = s->cur_off, on = s->cur_off ^ 1;
+    FusedArgs a{};
+    a.sx = s->x[src]; a.svx = s->vx[src]; a.svy = s->vy[src]; a.svz = s->vz[src];
+    a.dx = s->x[dst]; a.dvx = s->vx[dst]; a.dvy = s->vy[dst]; a.dvz = s->vz[dst]; a.dcell = s->cell[dst];
+    a.E = sim->d_E;
+    a.off_old = s->d_off[oo]; a.bound_old = s->d_bound[oo];
+    a.count_new = s->d_count[on]; a.off_new = s->d_off[on]; a.bound_new = s->d_bound[on];
+    a.chain = s->d_chain;
+    a.st = s->d_st;
+    a.k = s->k;
+    a.vkick = s->vkick;
+    a.capacity = s->capacity;
+    a.T = s->T;
+    a.nblocks = (int)(s->n_ub / s->T) + 1;
+    a.nb_cap = s->nb_cap;
+    a.epoch = ++s->epoch;
+    {
+        KernelSpan span(sim, K_FUSED);
+        fused_kernel<<<a.nblocks, FUSED_THREADS, sizeof(FusedShared), sim->stream>>>(a);
+        if (int rc = launch_check(sim, "fused_kernel")) return rc;
+    }
+    // fallback chain, all guarded by run_split; it leaves the same host-visible state behind
+    const int *guard = &s->d_st->run_split;
+    const long long wsum_before = s->h_wsum;
+    s->h_wsum = std::min<long long>(s->h_wsum + host_step_bound(s), 1LL << 40);
+    s->h_steps_since_sync++;
+    if (int rc = push_split(s, true, guard)) return rc;
+    if (int rc = arrange_split(s, true, guard, true)) return rc; // flips cur / cur_off, marks fresh
+    (void)wsum_before;
+    return PIC_OK;
+}
+
 extern "C" int pic_push(pic_species *s, int nsteps)
 {
     if (!s || nsteps < 0) return PIC_EINVAL;
     for (int it = 0; it < nsteps; ++it) {
         const bool will_arrange = s->arrange_every > 0 && ((s->steps + 1) % s->arrange_every) == 0;
-        if (int rc = push_split(s, will_arrange)) return rc;
+        const bool fused = will_arrange && fused_possible(s) && s->counts_fresh && s->all_live && s->bounds_valid &&
+                           s->n_ub > 0;
+        if (fused) {
+            if (int rc = push_fused(s)) return rc;
+            s->steps++;
+            continue;
+        }
+        if (int rc = push_split(s, will_arrange, nullptr)) return rc;
         s->steps++;
         if (will_arrange)
-            if (int rc = arrange_split(s, true)) return rc;
+            if (int rc = arrange_split(s, true, nullptr, true)) return rc;
     }
     return PIC_OK;
 }
@@ -507,6 +654,9 @@ static int read_state(pic_species *s, DevState &h)
     CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, s->sim->stream));
     CU(cudaStreamSynchronize(s->sim->stream));
     if (h.n >= 0 && h.n <= s->n_ub) s->n_ub = h.n;
+    s->h_vmax = std::sqrt((double)bits_to_float(h.vmax2));
+    s->h_steps_since_sync = 0;
+    if (h.fused_disabled) s->fused_off = true;
     return PIC_OK;
 }
 

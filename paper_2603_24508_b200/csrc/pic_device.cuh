@@ -27,9 +27,15 @@ struct DevState {
     int status;       // ERR_* bits
     int need_general; // fast arranger declined (w_acc too large); the general path must run
     int used_general; // the last arrange ran the general path
-    int fused_ok;     // fused step flag: 1 = result valid, 0 = must redo with the split path
-    int pad;
-    unsigned long long wall[2]; // cumulative absorbed at x<0 / x>=L
+    int run_split;      // set by a fused step: 1 = it declined, the guarded split kernels behind it must run
+    int fused_disabled; // sticky: a fused step has declined; later fused launches exit at once
+    unsigned long long wall[2];      // cumulative absorbed at x<0 / x>=L
+    unsigned long long wall_pend[2]; // fused step in flight: absorbed, not yet committed
+    unsigned vmax2, vmax2_next;      // float bits (rounded up) of max |v|^2: current state / step in flight
+    int n_next;                      // fused step in flight: kept particles so far
+    unsigned ticket, done;           // fused step: block tickets / finished blocks
+    int abort;                       // fused step in flight: some block declined
+    int pad[3];
 };
 
 // Per-species Boris constants (computed once on the host) and grid.

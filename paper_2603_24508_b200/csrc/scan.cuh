@@ -18,6 +18,7 @@ struct ScanFold {      // optional bookkeeping done by tile 0 / the last tile fo
     DevState *st;      // may be NULL
     int reset;         // fold step_max into w_acc starting from 0 (an arrange ran before this step)
     int set_n;         // store the grand total into st->n
+    int set_vmax;      // a mover step ran just before: commit its speed bound (vmax2 = vmax2_next)
     const int *guard;  // if not NULL: return at once unless *guard != 0
 };
 
@@ -43,6 +44,10 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_exclusive_kernel(const int 
         fold.st->step_max = 0;
         fold.st->need_general = 0;
         fold.st->used_general = 0;
+        if (fold.set_vmax) {
+            fold.st->vmax2 = fold.st->vmax2_next;
+            fold.st->vmax2_next = 0;
+        }
     }
 
     const long long base = (long long)tile * SCAN_TILE + (long long)threadIdx.x * SCAN_ITEMS;
