@@ -1,0 +1,124 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (own
+stream, default options: fused single-pass step where arrange_every == 1, TMA-staged E).
+
+Two kinds of check (task contract, parity at full size):
+  * element by element against the oracle for the first steps of every config (the oracle needs
+    about a second per 30-40 M pushes, so a few steps of 100 M particles is still seconds);
+  * after the config's whole step count: on SAMPLED particles the oracle computes one by one
+    (the mover acts on each particle independently, so the oracle follows a sample from its
+    initial state through all steps without arranging; the GPU's final state must contain that
+    exact particle, bit for bit, inside the slot range of its final cell), plus properties that
+    hold at any size (grouped by cell, cell == floor(x*inv_dx), counts/offsets consistent,
+    n_live + absorbed == n_0) and EXACT wall counts from an oracle run over the only particles
+    that can reach a wall (those within `margin` cells of it; checked to be enough).
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2603_24508_b200 as pic
+from paper_2603_24508_b200 import workloads
+from parity_util import compare, make_pair
+
+pytestmark = pytest.mark.gpu
+
+
+def _bench_like_pair(inp):
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        sim, states = make_pair(inp, stream=stream)
+    return sim, states, stream
+
+
+@pytest.mark.parametrize("config,steps,check_every", [(2, 4, 1), (3, 3, 1), (4, 3, 1), (5, 10, 5)])
+def test_fullsize_first_steps_elementwise(config, steps, check_every):
+    inp = workloads.make(config)
+    sim, states, _ = _bench_like_pair(inp)
+    ae = inp["arrange_every"]
+    for step in range(1, steps + 1):
+        for sp, st in zip(sim.species, states):
+            pic.pic_push(sp, 1)
+            st.push(1)
+        if step % check_every == 0 or step == steps:
+            for si, (sp, st) in enumerate(zip(sim.species, states)):
+                compare(sp, st, where=f"config {config} full size, step {step} species {si}",
+                        counts=(step % ae == 0), nc=inp["nc"])
+    pic.pic_sync(sim)
+    for sp in sim.species:
+        assert pic.pic_arrange_info(sp)[1] == 0, "full-size run fell to the general arranger"
+    pic.pic_destroy(sim)
+
+
+def _oracle_subset(inp, s, idx, steps):
+    """Oracle trajectories (no arranging: the mover is per-particle) of the particles idx."""
+    st = oracle.State(s["x"][idx], s["vx"][idx], s["vy"][idx], s["vz"][idx], s["cell"][idx], nc=inp["nc"],
+                      dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E=inp["E"], qm=s["qm"], B=inp["B"],
+                      arrange_every=0)
+    st.push(steps)
+    return st
+
+
+@pytest.mark.parametrize("config,margin", [(2, 2000), (3, 2000), (4, 0), (5, 6000)])
+def test_fullsize_all_steps_sampled_and_properties(config, margin):
+    inp = workloads.make(config)
+    nc, steps, ae = inp["nc"], inp["steps"], inp["arrange_every"]
+    assert steps % ae == 0
+    sim, _states, _ = _bench_like_pair(inp)
+    del _states
+    for sp in sim.species:
+        pic.pic_push(sp, steps)  # one call, as bench.py's e2e leg; the timed leg calls it step by step
+    pic.pic_sync(sim)
+    rng = np.random.default_rng(99 + config)
+    for si, (sp, s) in enumerate(zip(sim.species, inp["species"])):
+        n0 = len(s["x"])
+        wf = pic.pic_wall_flux(sp)
+        n_live = pic.pic_n_slots(sp)
+        x, vx, vy, vz, cell = sp.state()
+        count, offset = pic.pic_cell_counts(sp, nc)
+        assert pic.pic_arrange_info(sp)[1] == 0
+        # ---- properties that hold at any size
+        assert n_live + wf["left_total"] + wf["right_total"] == n0
+        assert int(offset[nc]) == n_live and int(count.sum()) == n_live
+        assert np.array_equal(np.concatenate([[0], np.cumsum(count, dtype=np.int64)]), offset.astype(np.int64))
+        assert bool((cell[1:] >= cell[:-1]).all()), "not grouped by cell"
+        inv_dx = 1.0 / inp["dx"]
+        cf = torch.clamp(torch.floor(x * inv_dx).to(torch.int32), max=nc - 1)
+        assert bool((cf == cell).all()), "cell != floor(x*inv_dx)"
+        assert bool(((x >= 0) & (x < nc * inp["dx"])).all())
+        bc = torch.bincount(cell.to(torch.int64), minlength=nc).to(torch.int32).cpu().numpy()
+        assert np.array_equal(bc, count)
+        # ---- sampled particles, followed one by one by the oracle
+        k = 4096
+        idx = np.sort(rng.choice(n0, size=k, replace=False))
+        if margin:
+            edge = np.concatenate([np.arange(0, 256), np.arange(n0 - 256, n0)])  # some that do hit a wall
+            idx = np.unique(np.concatenate([idx, edge]))
+        st = _oracle_subset(inp, s, idx, steps)
+        live = st.cell >= 0
+        lo = offset[st.cell[live]].astype(np.int64)
+        hi = offset[st.cell[live] + 1].astype(np.int64)
+        xs, vxs, vys, vzs = (torch.from_numpy(a[live]).to(x.device) for a in (st.x, st.vx, st.vy, st.vz))
+        lo_t, hi_t = torch.from_numpy(lo).to(x.device), torch.from_numpy(hi).to(x.device)
+        found = torch.zeros(len(lo), dtype=torch.int64, device=x.device)
+        width = int((hi - lo).max())
+        for j in range(width):
+            p = lo_t + j
+            ok = p < hi_t
+            pc = torch.where(ok, p, lo_t)
+            hit = ok & (x[pc] == xs) & (vx[pc] == vxs) & (vy[pc] == vys) & (vz[pc] == vzs)
+            found += hit.to(torch.int64)
+        assert bool((found == 1).all()), (f"config {config} species {si}: {(found != 1).sum().item()} of {len(lo)} "
+                                          f"sampled particles not found bit-exactly in their final cell")
+        # ---- exact wall counts: only particles that start within `margin` cells of a wall can reach it
+        if inp["boundary"] == workloads.ABSORBING:
+            near = np.flatnonzero((s["cell"] < margin) | (s["cell"] >= nc - margin))
+            sw = _oracle_subset(inp, s, near, steps)
+            dead = sw.cell < 0
+            start = s["cell"][near][dead]
+            reach = np.minimum(start, nc - 1 - start)
+            assert reach.max(initial=0) < margin // 2, "margin too small to certify the wall counts"
+            assert (wf["left_total"], wf["right_total"]) == (int(sw.wall[0]), int(sw.wall[1]))
+        else:
+            assert wf["left_total"] == 0 and wf["right_total"] == 0
+    pic.pic_destroy(sim)
