@@ -147,15 +147,27 @@ int pic_step_count(pic_species *sp, int64_t *steps);
  * the last arrange used the general path (0/1).  Diagnostics for tests.  Syncs. */
 int pic_arrange_info(pic_species *sp, int32_t *w_bound, int32_t *used_general);
 
+/* State of the fused push+arrange step of this species.  *active: 1 if the next pic_push step
+ * with an arrange would take it.  *decline_reasons: OR of the reasons any fused step has been
+ * redone by the split kernels so far (1 = a particle moved more than one cell or broke the
+ * grouping, 2 = a tile did not fit the shared-memory stage, 4 / 8 = a boundary list overflowed);
+ * 0 means every fused step so far completed.  *stage_slots, *ctas_per_sm: the launch geometry
+ * the next fused step would use.  Any pointer may be NULL.  Syncs. */
+int pic_fused_info(pic_species *sp, int32_t *active, int32_t *decline_reasons, int32_t *stage_slots,
+                   int32_t *ctas_per_sm);
+
 /* Bytes of caller-allocated workspace a species of this size needs. */
 size_t pic_workspace_bytes(int32_t nc, int64_t capacity);
 
-/* Mover/arranger variant switches for measurements (profiles/ compares them):
- * key "e_stage": 0 = E through the read-only global path, 1 = E window staged in
- * shared memory by TMA bulk copy (default); key "fused": 1 = single-pass push+arrange
- * when arrange_every == 1 (default), 0 = separate mover / scan / scatter kernels; key
- * "kernel_timing": 1 = record CUDA events around every kernel launch (see pic_kernel_time).
- * PIC_EINVAL for an unknown key or value. */
+/* Variant switches and tuning knobs, for measurements (profiles/ compares them).  Flags (0/1):
+ * "e_stage": 0 = E through the read-only global path, 1 = E window staged in shared memory by
+ * TMA bulk copy (default); "fused": 1 = single-pass push+arrange when arrange_every == 1
+ * (default), 0 = separate mover / scan / scatter kernels; "kernel_timing": 1 = record CUDA
+ * events around every kernel launch (see pic_kernel_time).  Knobs of the fused step:
+ * "fused_tile" (target particles per tile, 64..4096, default 128), "fused_tiles_per_cta"
+ * (1..256, default 64), "fused_stage_slots" (shared-memory slots per tile stage, a multiple of
+ * 32; 0 = automatic from the largest per-cell count).  Results never depend on any of them.
+ * PIC_EINVAL for an unknown key or a value out of range. */
 int pic_set_option(pic_sim *sim, const char *key, int value);
 
 /* Device time of one kernel class since the previous query of that class, measured with CUDA

@@ -21,7 +21,7 @@ EXPORTS = [
     "pic_create", "pic_species_at", "pic_push", "pic_arrange", "pic_wall_flux", "pic_set_field", "pic_n_slots",
     "pic_active_buffer", "pic_cell_counts", "pic_step_count", "pic_arrange_info", "pic_workspace_bytes",
     "pic_set_option", "pic_launch_count", "pic_sync", "pic_destroy", "pic_strerror", "pic_last_error",
-    "pic_run_host", "pic_kernel_time",
+    "pic_run_host", "pic_kernel_time", "pic_fused_info",
 ]
 
 
@@ -88,6 +88,7 @@ def lib():
         L.pic_set_option.argtypes = [vp, C.c_char_p, C.c_int]
         L.pic_launch_count.argtypes = [vp, C.POINTER(C.c_uint64)]
         L.pic_kernel_time.argtypes = [vp, C.c_char_p, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
+        L.pic_fused_info.argtypes = [vp, i32p, i32p, i32p, i32p]
         L.pic_sync.argtypes = [vp]
         L.pic_destroy.argtypes = [vp]
         L.pic_destroy.restype = None
@@ -261,6 +262,13 @@ def pic_arrange_info(sp):
     w, g = C.c_int32(), C.c_int32()
     _check(lib().pic_arrange_info(sp.handle, C.byref(w), C.byref(g)), "pic_arrange_info")
     return w.value, g.value
+
+
+def pic_fused_info(sp):
+    """-> dict(active, decline_reasons, stage_slots, ctas_per_sm) of the fused push+arrange step."""
+    v = [C.c_int32() for _ in range(4)]
+    _check(lib().pic_fused_info(sp.handle, *[C.byref(x) for x in v]), "pic_fused_info")
+    return dict(zip(("active", "decline_reasons", "stage_slots", "ctas_per_sm"), (x.value for x in v)))
 
 
 def pic_set_option(sim, key, value):

@@ -29,9 +29,14 @@ __global__ void __launch_bounds__(MOVER_THREADS) mover_kernel(MoverArgs a)
     __syncthreads();
 
     const int n = a.st->n;
-    const long long p = (long long)blockIdx.x * MOVER_THREADS + threadIdx.x; // pair index
-    const long long i0 = 2 * p;
     const int lane = threadIdx.x & 31;
+    int dmax = 0, nleft = 0, nright = 0, bad = 0;
+    float vm2 = 0.f; // upper bound of max |v'|^2 (feeds the next step's displacement bound)
+    // one pair of neighbouring particles per thread and iteration; the grid normally covers the array in
+    // one iteration (the guarded fallback launch uses a small grid and strides)
+    const long long pairs = ((long long)n + 1) / 2;
+    for (long long pb = (long long)blockIdx.x * MOVER_THREADS; pb < pairs; pb += (long long)gridDim.x * MOVER_THREADS) {
+    const long long i0 = 2 * (pb + threadIdx.x);
 
     double x[2], vx[2], vy[2], vz[2];
     int c[2] = {-1, -1};
@@ -52,8 +57,6 @@ __global__ void __launch_bounds__(MOVER_THREADS) mover_kernel(MoverArgs a)
         x[0] = x[1] = vx[0] = vx[1] = vy[0] = vy[1] = vz[0] = vz[1] = 0.0;
     }
 
-    int dmax = 0, nleft = 0, nright = 0, bad = 0;
-    float vm2 = 0.f; // upper bound of max |v'|^2 (feeds the next step's displacement bound)
     int cn[2] = {-1, -1};
 #pragma unroll
     for (int q = 0; q < 2; ++q) {
@@ -87,6 +90,7 @@ __global__ void __launch_bounds__(MOVER_THREADS) mover_kernel(MoverArgs a)
     } else if (have[0]) {
         a.x[i0] = x[0]; a.vx[i0] = vx[0]; a.vy[i0] = vy[0]; a.vz[i0] = vz[0];
         a.cell[i0] = cn[0];
+    }
     }
 
     // wall counters (ballot/popc: one atomic per warp that absorbed something), error flag,

@@ -49,11 +49,11 @@ struct pic_species {
     unsigned long long *d_scan = nullptr;
     size_t scan_words = 0;
     // fused push+arrange step (fused.cuh)
-    int *d_bound[2]{};                 // block partition of d_off[i]: first cell with offset >= k*T
-    unsigned long long *d_chain = nullptr;
-    int T = FUSED_T_DEFAULT, nb_cap = 0;
-    unsigned epoch = 0;
-    bool bounds_valid = false;         // d_bound[cur_off] describes d_off[cur_off]
+    int2 *d_td[2]{};                   // tile partition of d_off[i] (fused.cuh: bounds_kernel)
+    int T = FUSED_T_DEFAULT, td_cap = 0;
+    int h_maxcount = 0;                // largest per-cell count at the last sync (sizes the fused stage)
+    int h_abort_reason = 0;
+    bool bounds_valid = false;         // d_td[cur_off] describes d_off[cur_off]
     bool fused_off = false;            // the device reported a declined fused step (sticky)
     // host-side conservative bound on cell displacement since the last arrange (decides whether the
     // general-path kernels need to be enqueued at all)
@@ -81,6 +81,7 @@ struct pic_sim {
     std::vector<pic_species *> sp;
     unsigned long long launches = 0;
     int opt_e_stage = 1, opt_fused = 1, opt_timing = 0;
+    int opt_fused_tpc = FUSED_TPC_DEFAULT, opt_fused_cap = 0; // tuning knobs of the fused step (0 = automatic)
     int sm_count = 148;
     // per-kernel device timing (option "kernel_timing"): event pairs recorded around launches
     struct Span { int id; cudaEvent_t a, b; };
@@ -145,9 +146,8 @@ static void free_species(pic_species *s)
     cudaFree(s->d_st);
     for (int b = 0; b < 2; ++b) { cudaFree(s->d_count[b]); cudaFree(s->d_off[b]); }
     cudaFree(s->d_scan);
-    cudaFree(s->d_bound[0]);
-    cudaFree(s->d_bound[1]);
-    cudaFree(s->d_chain);
+    cudaFree(s->d_td[0]);
+    cudaFree(s->d_td[1]);
     delete s;
 }
 
@@ -215,20 +215,23 @@ static float bits_to_float(unsigned u)
     return f;
 }
 
-// bound[] (block partition of the fused step) from the offsets in slot `which`
+// tile partition of the fused step from the offsets in slot `which`
 static int run_bounds(pic_species *s, int which, const int *guard)
 {
     pic_sim *sim = s->sim;
     const int nc = sim->nc;
-    bounds_kernel<<<(nc + 255) / 256, 256, 0, sim->stream>>>(s->d_off[which], nc, s->T, s->d_bound[which], s->nb_cap, guard);
+    bounds_kernel<<<(nc + 255) / 256, 256, 0, sim->stream>>>(s->d_off[which], nc, s->T, s->d_td[which], s->td_cap, s->d_st, guard);
     if (int rc = launch_check(sim, "bounds_kernel")) return rc;
     if (!guard) s->bounds_valid = true;
     return PIC_OK;
 }
 
+static int fused_cap(const pic_species *s, int *ctas_per_sm);
+
 static bool fused_possible(const pic_species *s)
 {
-    return s->sim->opt_fused && !s->fused_off && s->arrange_every == 1 && s->sim->nc >= FUSED_MIN_NC;
+    return s->sim->opt_fused && !s->fused_off && s->arrange_every == 1 && s->sim->nc >= FUSED_MIN_NC &&
+           fused_cap(s, nullptr) > 0;
 }
 
 // Host-side bound (cells) on what one more mover step can displace any particle.
@@ -314,25 +317,28 @@ static int create_species(pic_sim *sim, const pic_species_desc &d, pic_species *
     }
     ScanFold nofold{nullptr, 0, 0, 0, nullptr};
     if (int rc = run_scan(s, s->d_count[0], s->d_off[0], nc, nofold)) return rc;
-    // fused step: block partition, look-back chain
+    // fused step: tile partition (two copies: a fused step reads one and writes the other)
     s->T = FUSED_T_DEFAULT;
-    s->nb_cap = (int)(d.capacity / s->T) + 2;
+    s->td_cap = (int)(d.capacity / FUSED_T_MIN) + 3;
     for (int b = 0; b < 2; ++b) {
-        CU(cudaMalloc(&s->d_bound[b], sizeof(int) * ((size_t)s->nb_cap + 2)));
-        CU(cudaMemsetAsync(s->d_bound[b], 0, sizeof(int) * ((size_t)s->nb_cap + 2), sim->stream));
+        CU(cudaMalloc(&s->d_td[b], sizeof(int2) * (size_t)s->td_cap));
+        CU(cudaMemsetAsync(s->d_td[b], 0, sizeof(int2) * (size_t)s->td_cap, sim->stream));
     }
-    CU(cudaMalloc(&s->d_chain, sizeof(unsigned long long) * ((size_t)s->nb_cap + 2)));
-    CU(cudaMemsetAsync(s->d_chain, 0, sizeof(unsigned long long) * ((size_t)s->nb_cap + 2), sim->stream));
     s->vkick = 2.0 * std::fabs(s->k.h) * sim->Emax;
     s->h_vmax = std::sqrt((double)bits_to_float(h.vmax2));
     s->h_grouped = grouped;
     s->bounds_valid = false;
-    if (grouped)
-        if (int rc = run_bounds(s, 0, nullptr)) return rc;
     h.status = 0;
     h.w_acc = grouped ? 0 : W_UNKNOWN;
+    h.ntiles = 1;
     CU(cudaMemcpyAsync(s->d_st, &h, sizeof h, cudaMemcpyHostToDevice, sim->stream));
     CU(cudaStreamSynchronize(sim->stream));
+    if (grouped) {
+        if (int rc = run_bounds(s, 0, nullptr)) return rc;
+        CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, sim->stream));
+        CU(cudaStreamSynchronize(sim->stream));
+        s->h_maxcount = h.maxcount;
+    }
     s->cur = 0;
     s->cur_off = 0;
     s->counts_fresh = grouped;
@@ -341,7 +347,7 @@ static int create_species(pic_sim *sim, const pic_species_desc &d, pic_species *
     {
         static bool attr_set = false;
         if (!attr_set) {
-            CU(cudaFuncSetAttribute(fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedShared)));
+            CU(cudaFuncSetAttribute(fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, FUSED_SMEM_CTA));
             attr_set = true;
         }
     }
@@ -424,10 +430,15 @@ extern "C" int pic_set_field(pic_sim *sim, const double *E)
 
 extern "C" int pic_set_option(pic_sim *sim, const char *key, int value)
 {
-    if (!sim || !key || (value != 0 && value != 1)) return PIC_EINVAL;
-    if (!strcmp(key, "e_stage")) sim->opt_e_stage = value;
-    else if (!strcmp(key, "kernel_timing")) sim->opt_timing = value;
-    else if (!strcmp(key, "fused")) sim->opt_fused = value;
+    if (!sim || !key) return PIC_EINVAL;
+    const bool flag = value == 0 || value == 1;
+    if (!strcmp(key, "e_stage") && flag) sim->opt_e_stage = value;
+    else if (!strcmp(key, "kernel_timing") && flag) sim->opt_timing = value;
+    else if (!strcmp(key, "fused") && flag) sim->opt_fused = value;
+    else if (!strcmp(key, "fused_tile") && value >= FUSED_T_MIN && value <= 4096) {
+        for (pic_species *s : sim->sp) { s->T = value; s->bounds_valid = false; }
+    } else if (!strcmp(key, "fused_tiles_per_cta") && value >= 1 && value <= FUSED_TPC_MAX) sim->opt_fused_tpc = value;
+    else if (!strcmp(key, "fused_stage_slots") && value >= 0 && value <= 16384 && value % 32 == 0) sim->opt_fused_cap = value;
     else return PIC_EINVAL;
     return PIC_OK;
 }
@@ -568,6 +579,7 @@ static int push_split(pic_species *s, bool will_arrange, const int *guard)
         a.E = sim->d_E; a.count = s->d_count[on]; a.st = s->d_st; a.k = s->k; a.guard = guard;
         long long pairs = (s->n_ub + 1) / 2;
         int blocks = (int)((pairs + MOVER_THREADS - 1) / MOVER_THREADS);
+        if (guard) blocks = std::min(blocks, sim->sm_count * 8); // fallback behind a fused step: strides if it runs
         const bool rc = !s->all_live;
         KernelSpan span(sim, K_MOVER);
         if (rc) { if (will_arrange) launch_mover<true, true>(s, a, blocks); else launch_mover<true, false>(s, a, blocks); }
@@ -588,8 +600,34 @@ static int push_split(pic_species *s, bool will_arrange, const int *guard)
     return PIC_OK;
 }
 
+// Shared-memory stage (slots per tile) of the fused kernel for this species' current state, or 0 when
+// a tile cannot fit.  A tile holds fewer than T + maxcount particles; maxcount is the bound read at
+// the last sync, so leave room for it to grow, then use whatever the chosen occupancy leaves free.
+static int fused_cap(const pic_species *s, int *ctas_per_sm)
+{
+    const pic_sim *sim = s->sim;
+    if (sim->opt_fused_cap > 0) {
+        const int tot = fused_layout(sim->opt_fused_cap, sim->opt_fused_tpc).total;
+        if (tot > FUSED_SMEM_CTA) return 0;
+        if (ctas_per_sm) *ctas_per_sm = std::max(1, std::min(32, FUSED_SMEM_SM / (tot + 1024)));
+        return sim->opt_fused_cap;
+    }
+    const int mc = std::max(s->h_maxcount, 1);
+    int need = s->T + mc + std::max(mc / 2, 64) + 2;
+    need = (need + 31) & ~31;
+    const int tot = fused_layout(need, sim->opt_fused_tpc).total;
+    if (tot > FUSED_SMEM_CTA) return 0;
+    const int ctas = std::max(1, std::min(32, FUSED_SMEM_SM / (tot + 1024)));
+    int cap = need;
+    while (cap + 32 <= 16384 && fused_layout(cap + 32, sim->opt_fused_tpc).total + 1024 <= FUSED_SMEM_SM / ctas &&
+           fused_layout(cap + 32, sim->opt_fused_tpc).total <= FUSED_SMEM_CTA)
+        cap += 32;
+    if (ctas_per_sm) *ctas_per_sm = ctas;
+    return cap;
+}
+
 // One fused push+arrange step, followed by the guarded split chain that redoes the step if the
-// fused kernel declined on the device (DevState::run_split).
+// fused kernels declined on the device (DevState::run_split).
 static int push_fused(pic_species *s)
 {
     pic_sim *sim = s->sim;
@@ -599,30 +637,30 @@ static int push_fused(pic_species *s)
     a.sx = s->x[src]; a.svx = s->vx[src]; a.svy = s->vy[src]; a.svz = s->vz[src];
     a.dx = s->x[dst]; a.dvx = s->vx[dst]; a.dvy = s->vy[dst]; a.dvz = s->vz[dst]; a.dcell = s->cell[dst];
     a.E = sim->d_E;
-    a.off_old = s->d_off[oo]; a.bound_old = s->d_bound[oo];
-    a.count_new = s->d_count[on]; a.off_new = s->d_off[on]; a.bound_new = s->d_bound[on];
-    a.chain = s->d_chain;
+    a.off_old = s->d_off[oo]; a.td_old = s->d_td[oo];
+    a.count_new = s->d_count[on]; a.off_new = s->d_off[on]; a.td_new = s->d_td[on];
     a.st = s->d_st;
     a.k = s->k;
-    a.vkick = s->vkick;
     a.capacity = s->capacity;
     a.T = s->T;
-    a.nblocks = (int)(s->n_ub / s->T) + 1;
-    a.nb_cap = s->nb_cap;
-    a.epoch = ++s->epoch;
+    a.TPC = sim->opt_fused_tpc;
+    a.td_cap = s->td_cap;
+    a.CAP = fused_cap(s, nullptr);
+    const int ntiles_ub = (int)(s->n_ub / s->T) + 1;
+    const int grid = (ntiles_ub + a.TPC - 1) / a.TPC;
     {
         KernelSpan span(sim, K_FUSED);
-        fused_kernel<<<a.nblocks, FUSED_THREADS, sizeof(FusedShared), sim->stream>>>(a);
+        fused_edge_kernel<<<1, 128, 0, sim->stream>>>(a);
+        if (int rc = launch_check(sim, "fused_edge_kernel")) return rc;
+        fused_kernel<<<grid, 32, fused_layout(a.CAP, a.TPC).total, sim->stream>>>(a);
         if (int rc = launch_check(sim, "fused_kernel")) return rc;
     }
     // fallback chain, all guarded by run_split; it leaves the same host-visible state behind
     const int *guard = &s->d_st->run_split;
-    const long long wsum_before = s->h_wsum;
     s->h_wsum = std::min<long long>(s->h_wsum + host_step_bound(s), 1LL << 40);
     s->h_steps_since_sync++;
     if (int rc = push_split(s, true, guard)) return rc;
     if (int rc = arrange_split(s, true, guard, true)) return rc; // flips cur / cur_off, marks fresh
-    (void)wsum_before;
     return PIC_OK;
 }
 
@@ -631,9 +669,10 @@ extern "C" int pic_push(pic_species *s, int nsteps)
     if (!s || nsteps < 0) return PIC_EINVAL;
     for (int it = 0; it < nsteps; ++it) {
         const bool will_arrange = s->arrange_every > 0 && ((s->steps + 1) % s->arrange_every) == 0;
-        const bool fused = will_arrange && fused_possible(s) && s->counts_fresh && s->all_live && s->bounds_valid &&
-                           s->n_ub > 0;
+        const bool fused = will_arrange && fused_possible(s) && s->counts_fresh && s->all_live && s->n_ub > 0;
         if (fused) {
+            if (!s->bounds_valid)
+                if (int rc = run_bounds(s, s->cur_off, nullptr)) return rc;
             if (int rc = push_fused(s)) return rc;
             s->steps++;
             continue;
@@ -657,6 +696,8 @@ static int read_state(pic_species *s, DevState &h)
     s->h_vmax = std::sqrt((double)bits_to_float(h.vmax2));
     s->h_steps_since_sync = 0;
     if (h.fused_disabled) s->fused_off = true;
+    s->h_maxcount = h.maxcount;
+    s->h_abort_reason = h.abort_reason;
     return PIC_OK;
 }
 
@@ -720,6 +761,21 @@ extern "C" int pic_arrange_info(pic_species *s, int32_t *w_bound, int32_t *used_
     if (int rc = read_state(s, h)) return rc;
     if (w_bound) *w_bound = h.w_acc;
     if (used_general) *used_general = h.used_general;
+    return PIC_OK;
+}
+
+extern "C" int pic_fused_info(pic_species *s, int32_t *active, int32_t *decline_reasons, int32_t *stage_slots,
+                              int32_t *ctas_per_sm)
+{
+    if (!s) return PIC_EINVAL;
+    DevState h;
+    if (int rc = read_state(s, h)) return rc;
+    if (active) *active = fused_possible(s) ? 1 : 0;
+    if (decline_reasons) *decline_reasons = h.abort_reason;
+    int ctas = 0;
+    const int cap = fused_cap(s, &ctas);
+    if (stage_slots) *stage_slots = cap;
+    if (ctas_per_sm) *ctas_per_sm = ctas;
     return PIC_OK;
 }
 

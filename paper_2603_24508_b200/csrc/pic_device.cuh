@@ -32,10 +32,14 @@ struct DevState {
     unsigned long long wall[2];      // cumulative absorbed at x<0 / x>=L
     unsigned long long wall_pend[2]; // fused step in flight: absorbed, not yet committed
     unsigned vmax2, vmax2_next;      // float bits (rounded up) of max |v|^2: current state / step in flight
-    int n_next;                      // fused step in flight: kept particles so far
-    unsigned ticket, done;           // fused step: block tickets / finished blocks
-    int abort;                       // fused step in flight: some block declined
-    int pad[3];
+    int n_next;                      // fused step in flight: particle count after it
+    unsigned done;                   // fused step: finished CTAs
+    int abort;                       // fused step in flight: some CTA declined
+    int abort_reason;                // FA_* bits of every decline so far (diagnostics)
+    int f_OL, f_AR;                  // fused step in flight: leavers of cell 0 downwards / wrapped arrivals in cell 0
+    int ntiles, ntiles_next;         // tiles of the current partition (fused.cuh) / of the one being written
+    int maxcount, maxcount_next;     // upper bound of the largest per-cell count: current state / step in flight
+    int pad[2];
 };
 
 // Per-species Boris constants (computed once on the host) and grid.

@@ -225,3 +225,65 @@ def test_run_host_end_to_end():
     assert n_out == st.n and (wl, wr) == (int(st.wall[0]), int(st.wall[1]))
     for a, o in zip(arrs, st.live()):
         assert np.array_equal(a[:n_out], o)
+
+
+@pytest.mark.parametrize("config,kw,steps", [(1, {}, 40), (2, dict(nc=2048), 40), (3, dict(nc=1000), 30),
+                                             (4, dict(nc=4099), 30)])
+def test_fused_step_is_the_one_that_runs(config, kw, steps):
+    """Configs 1-4 (arrange every step, |dcell| <= 1): every step is taken by the fused kernels,
+    none is redone by the guarded split chain."""
+    inp = workloads.make(config, **kw)
+    sim, states = run_stepwise(inp, steps, options={"fused": 1}, check_every=10)
+    for sp in sim.species:
+        info = pic.pic_fused_info(sp)
+        assert info["active"] == 1 and info["decline_reasons"] == 0, info
+        assert pic.pic_arrange_info(sp)[1] == 0
+
+
+@pytest.mark.parametrize("knobs", [
+    {"fused_tile": 64}, {"fused_tile": 256, "fused_tiles_per_cta": 1}, {"fused_tile": 1024, "fused_tiles_per_cta": 3},
+    {"fused_tiles_per_cta": 256}, {"fused_stage_slots": 512}, {"fused_tile": 64, "fused_tiles_per_cta": 2},
+])
+@pytest.mark.parametrize("config,kw", [(4, dict(nc=4099)), (2, dict(nc=1500))])
+def test_fused_knobs_do_not_change_results(knobs, config, kw):
+    """Tile size, tiles per CTA and stage size only move the tile / chunk borders (halo cells,
+    deferred right-movers, carried counts land elsewhere); results stay bit-identical."""
+    inp = workloads.make(config, **kw)
+    sim, _ = run_stepwise(inp, 12, options={"fused": 1, **knobs}, check_every=3)
+    info = pic.pic_fused_info(sim.species[0])
+    assert info["decline_reasons"] == 0, info
+
+
+def test_fused_declines_when_a_tile_does_not_fit_and_split_redoes_the_step():
+    """A stage too small for the tiles (64 slots against 160 particles per cell): the fused step
+    aborts on the device, the guarded split kernels redo it from the untouched source buffers."""
+    inp = workloads.make(2, nc=1024)
+    sim, _ = run_stepwise(inp, 6, options={"fused": 1, "fused_stage_slots": 64}, check_every=1)
+    info = pic.pic_fused_info(sim.species[0])
+    assert info["decline_reasons"] & 2 and info["active"] == 0, info
+
+
+def test_fused_declines_on_a_two_cell_jump():
+    """One particle fast enough to cross two cells in a step: the fused step declines (reason 1),
+    the split path takes over for good, results unchanged."""
+    inp = workloads.make(1, nc=512, ppc=40)
+    s = inp["species"][0]
+    s["vx"] = s["vx"].copy()
+    s["vx"][12345] = 23.0
+    sim, _ = run_stepwise(inp, 8, options={"fused": 1}, check_every=1)
+    info = pic.pic_fused_info(sim.species[0])
+    assert info["decline_reasons"] & 1 and info["active"] == 0, info
+
+
+def test_fused_empty_cells_and_sparse_density():
+    """Many empty cells and cells of very different size (config-5 density, slow particles so the
+    fused step applies): empty tiles, empty halo cells, tiles of many cells."""
+    inp = workloads.make(5, nc=2048, n_total=150000)
+    for s in inp["species"]:
+        for k in ("vx", "vy", "vz"):
+            s[k] = s[k] * 0.25
+    inp["arrange_every"] = 1
+    sim, states = run_stepwise(inp, 25, options={"fused": 1, "fused_tile": 64}, check_every=1)
+    assert (states[0].count == 0).any()
+    info = pic.pic_fused_info(sim.species[0])
+    assert info["decline_reasons"] == 0, info
