@@ -150,7 +150,7 @@ int pic_arrange_info(pic_species *sp, int32_t *w_bound, int32_t *used_general);
 /* State of the fused push+arrange step of this species.  *active: 1 if the next pic_push step
  * with an arrange would take it.  *decline_reasons: OR of the reasons any fused step has been
  * redone by the split kernels so far (1 = a particle moved more than one cell or broke the
- * grouping, 2 = a tile did not fit the shared-memory stage, 4 / 8 = a boundary list overflowed);
+ * grouping, 2 = a cell did not fit a tile, 4 / 8 = a boundary list overflowed);
  * 0 means every fused step so far completed.  *stage_slots, *ctas_per_sm: the launch geometry
  * the next fused step would use.  Any pointer may be NULL.  Syncs. */
 int pic_fused_info(pic_species *sp, int32_t *active, int32_t *decline_reasons, int32_t *stage_slots,
@@ -164,9 +164,9 @@ size_t pic_workspace_bytes(int32_t nc, int64_t capacity);
  * TMA bulk copy (default); "fused": 1 = single-pass push+arrange when arrange_every == 1
  * (default), 0 = separate mover / scan / scatter kernels; "kernel_timing": 1 = record CUDA
  * events around every kernel launch (see pic_kernel_time).  Knobs of the fused step:
- * "fused_tile" (target particles per tile, 64..4096, default 128), "fused_tiles_per_cta"
- * (1..256, default 64), "fused_stage_slots" (shared-memory slots per tile stage, a multiple of
- * 32; 0 = automatic from the largest per-cell count).  Results never depend on any of them.
+ * "fused_cells_per_cta" (cells per chunk, 1..256; 0 = automatic, at most 64), "fused_rows" (rows
+ * of 32 slots per tile: 8, 12 or 16; 0 = automatic from the largest per-cell count).  Results
+ * never depend on any of them.
  * PIC_EINVAL for an unknown key or a value out of range. */
 int pic_set_option(pic_sim *sim, const char *key, int value);
 

@@ -17,33 +17,31 @@
 //
 // fused_edge_kernel (one small block) pushes cells 0, 1, nc-2, nc-1, publishes OL / AR, counts the
 // walls and writes the wrapped particles.  fused_kernel streams everything else: each 32-thread
-// CTA owns a contiguous chunk of cell-aligned tiles (~T particles each), stages tile after tile in
-// a two-stage shared-memory ring with TMA bulk copies (x, vx, vy, vz and the E nodes of the
-// tile's cells; cp.async.bulk + mbarrier), pushes in place, ranks with ballot/popc prefix counts,
-// and stores every particle straight to its final slot.  Across tiles it carries the counts of the
-// previous cell; right-movers of a tile's last cell wait (a few particles, in shared memory) for
-// the next tile's first-cell count.  Chunk ends push one halo cell redundantly instead of talking
-// to the neighbour CTA.  Anything unexpected (a particle moving two cells, a tile larger than the
-// shared-memory stage) aborts the whole step: the source buffers are untouched, and the guarded
-// split kernels launched right behind (mover / scan / scatter) redo it.
+// CTA owns a chunk of CPC consecutive cells, cuts it greedily into tiles of whole cells that fit
+// RMAX rows of 32 slots, stages tile after tile in a two-stage shared-memory ring with TMA bulk
+// copies (cp.async.bulk + mbarrier; the E nodes of the chunk are staged once the same way),
+// pushes each tile into REGISTERS (the stage is refilled at once), ranks with ballot/popc prefix
+// counts per class, and stores every particle straight to its final slot.  Across tiles it
+// carries the counts of the previous cell; right-movers of a tile's last cell wait (a few
+// particles, in shared memory) for the next tile's first-cell count.  Chunk ends push one halo
+// cell redundantly instead of talking to the neighbour CTA.  Anything unexpected (a particle
+// moving two cells, a cell larger than a tile) aborts the whole step: the source buffers are
+// untouched, and the guarded split kernels launched right behind (mover / scan / scatter) redo it.
 #pragma once
 #include "pic_device.cuh"
 
 namespace pic {
 
 constexpr int FUSED_MIN_NC = 16;
-constexpr int FUSED_T_DEFAULT = 128;   // target particles per tile
-constexpr int FUSED_T_MIN = 64;
-constexpr int FUSED_TPC_DEFAULT = 64;  // tiles per chunk (per CTA)
-constexpr int FUSED_TPC_MAX = 256;
-constexpr int FUSED_KMAX = 63;         // cells per tile
+constexpr int FUSED_CPC_DEFAULT = 64;  // cells per chunk (per CTA)
+constexpr int FUSED_CPC_MAX = 256;
+constexpr int FUSED_KMAX = 32;         // cells per tile (one lane per cell)
 constexpr int FUSED_DEF = 32;          // deferred right-movers of a tile's last cell
 constexpr int FUSED_XCAP = 256;        // edge kernel: leavers per edge cell
 constexpr int FUSED_SMEM_SM = 233472;  // shared memory per SM (228 KB), 1 KB reserved per CTA
-constexpr int FUSED_SMEM_CTA = 232448; // 227 KB
 
 constexpr int FA_BAD_PARTICLE = 1; // moved more than one cell / left the gather range / broke the grouping
-constexpr int FA_TILE_OVERFLOW = 2; // a tile does not fit the stage (CAP slots, KMAX cells)
+constexpr int FA_TILE_OVERFLOW = 2; // a cell does not fit a tile (RMAX*32 slots)
 constexpr int FA_DEFER_OVERFLOW = 4;
 constexpr int FA_EDGE_OVERFLOW = 8;
 
@@ -52,38 +50,32 @@ struct FusedArgs {
     double *dx, *dvx, *dvy, *dvz;
     int *dcell;
     const double *E;
-    const int *off_old;  // nc+1
-    const int2 *td_old;  // tile k covers cells [td[k].x, td[k+1].x), slots [td[k].y, td[k+1].y)
+    const int *off_old; // nc+1
     int *count_new, *off_new;
-    int2 *td_new;
     DevState *st;
     PushConst k;
     long long capacity; // slots allocated in every particle array
-    int T, CAP, TPC, td_cap;
+    int CPC;
 };
 
-// Dynamic shared memory of one fused_kernel CTA (one warp).
+// Dynamic shared memory of one fused_kernel CTA (one warp); CAP = RMAX*32 slots per stage.
 struct FusedLayout {
-    int stage_bytes; // x, vx, vy, vz [CAP] + E window
-    int off_code, off_start, off_ps, off_pe, off_cnt, off_base, off_q, off_items, off_kind, off_mbar, total;
+    int stage_bytes; // x, vx, vy, vz [CAP]
+    int off_E, off_offs, off_ps, off_base, off_q, off_mbar, total;
 };
 
-__host__ __device__ inline FusedLayout fused_layout(int CAP, int TPC)
+__host__ __device__ inline FusedLayout fused_layout(int CAP, int CPC)
 {
     FusedLayout L;
-    L.stage_bytes = 32 * CAP + 8 * (FUSED_KMAX + 3);
+    L.stage_bytes = 32 * CAP;
     int o = 2 * L.stage_bytes;
-    L.off_code = o;  o += 4 * CAP;
-    L.off_start = o; o += 4 * (FUSED_KMAX + 1);
-    L.off_ps = o;    o += 2 * 3 * (FUSED_KMAX + 1);
-    L.off_pe = o;    o += 2 * 3 * (FUSED_KMAX + 1);
-    L.off_cnt = o;   o += 4 * 3 * (FUSED_KMAX + 1);
-    L.off_base = o;  o += 4 * 3 * (FUSED_KMAX + 1);
-    L.off_q = o;     o += FUSED_DEF * 40;
-    L.off_items = o; o += 16 * (TPC + 2);
-    L.off_kind = o;  o += 4 * (TPC + 2);
+    L.off_E = o;    o += 8 * (CPC + 6);
+    L.off_offs = o; o += 4 * (CPC + 4);
+    L.off_ps = o;   o += 4 * 3 * (FUSED_KMAX + 2);
+    L.off_base = o; o += 4 * 3 * FUSED_KMAX;
     o = (o + 15) & ~15;
-    L.off_mbar = o;  o += 16;
+    L.off_q = o;    o += FUSED_DEF * 40;
+    L.off_mbar = o; o += 32;
     L.total = o;
     return L;
 }
@@ -217,73 +209,101 @@ __global__ void __launch_bounds__(128) fused_edge_kernel(FusedArgs a)
     }
 }
 
-// ---- main kernel ---------------------------------------------------------------------------------
-enum { FK_REAL = 0, FK_HALO = 1, FK_VIRTUAL = 2 };
 
-struct FusedSmem {
-    unsigned char *base;
-    FusedLayout L;
-    int CAP;
-    __device__ __forceinline__ double *sx(int s) const { return reinterpret_cast<double *>(base + s * L.stage_bytes); }
-    __device__ __forceinline__ double *svx(int s) const { return sx(s) + CAP; }
-    __device__ __forceinline__ double *svy(int s) const { return sx(s) + 2 * CAP; }
-    __device__ __forceinline__ double *svz(int s) const { return sx(s) + 3 * CAP; }
-    __device__ __forceinline__ double *sE(int s) const { return sx(s) + 4 * CAP; }
-    __device__ __forceinline__ unsigned *code() const { return reinterpret_cast<unsigned *>(base + L.off_code); }
-    __device__ __forceinline__ int *start() const { return reinterpret_cast<int *>(base + L.off_start); }
-    __device__ __forceinline__ unsigned short *ps() const { return reinterpret_cast<unsigned short *>(base + L.off_ps); }
-    __device__ __forceinline__ unsigned short *pe() const { return reinterpret_cast<unsigned short *>(base + L.off_pe); }
-    __device__ __forceinline__ int *cnt() const { return reinterpret_cast<int *>(base + L.off_cnt); }
-    __device__ __forceinline__ int *bas() const { return reinterpret_cast<int *>(base + L.off_base); }
-    __device__ __forceinline__ double *q() const { return reinterpret_cast<double *>(base + L.off_q); }
-    __device__ __forceinline__ int4 *items() const { return reinterpret_cast<int4 *>(base + L.off_items); }
-    __device__ __forceinline__ int *kind() const { return reinterpret_cast<int *>(base + L.off_kind); }
-    __device__ __forceinline__ unsigned mbar(int s) const { return smem_u32(base + L.off_mbar + 8 * s); }
+// ---- main kernel ---------------------------------------------------------------------------------
+enum { FK_REAL = 0, FK_HALO = 1, FK_VIRTUAL = 2, FK_NONE = 3 };
+
+struct FusedItem {
+    int cA, cB, kind; // cells [cA, cB)
 };
 
-// lane 0: start the bulk copies of one tile (item) into a stage
-__device__ __forceinline__ void fused_issue(const FusedArgs &a, const FusedSmem &S, int4 it, int stage)
+struct FusedCtx { // uniform per CTA
+    int C0, C1, Cm, nc, CAP;
+    const int *offs; // offs[c - Cm] = off_old[c] for the chunk's cells and one halo cell on each side
+};
+
+__device__ __forceinline__ int fused_slots(const FusedCtx &X, int a, int b)
 {
-    const int cA = it.x, cB = it.y, sA = it.z, n = it.w - it.z;
+    const int sa = X.offs[a - X.Cm];
+    return round_up2((sa & 1) + X.offs[b - X.Cm] - sa);
+}
+
+// The chunk's work items in order: [halo cell C0-1] tiles of whole cells (greedy: as many cells as
+// fit CAP slots, at most 32) ... [halo cell C1 | virtual end of the grid].
+__device__ __forceinline__ FusedItem fused_next_item(const FusedCtx &X, int &phase, int &cur, int lane, int &bad)
+{
+    FusedItem I{0, 0, FK_NONE};
+    if (phase == 0) {
+        phase = 1;
+        cur = X.C0;
+        if (X.C0 > 0) I = FusedItem{X.C0 - 1, X.C0, FK_HALO};
+    }
+    if (I.kind == FK_NONE && phase == 1) {
+        if (cur < X.C1) {
+            const int b = cur + 1 + lane;
+            const bool fits = b <= X.C1 && fused_slots(X, cur, b) <= X.CAP;
+            const int nb = __popc(__ballot_sync(FULL, fits)); // fits holds for a prefix of the lanes
+            if (nb == 0) {
+                bad |= FA_TILE_OVERFLOW;
+                phase = 3;
+            } else {
+                I = FusedItem{cur, cur + nb, FK_REAL};
+                cur += nb;
+            }
+        } else {
+            phase = 3;
+            I = X.C1 < X.nc ? FusedItem{X.C1, X.C1 + 1, FK_HALO} : FusedItem{X.nc, X.nc, FK_VIRTUAL};
+        }
+    }
+    if (I.kind == FK_HALO && fused_slots(X, I.cA, I.cB) > X.CAP) {
+        bad |= FA_TILE_OVERFLOW;
+        phase = 3;
+        I.kind = FK_NONE;
+    }
+    return I;
+}
+
+// lane 0: start the bulk copies of one item's particles into a stage
+__device__ __forceinline__ void fused_issue(const FusedArgs &a, const FusedCtx &X, FusedItem I, double *stage, unsigned mb)
+{
+    if (I.kind == FK_NONE || I.kind == FK_VIRTUAL) return;
+    const int sA = X.offs[I.cA - X.Cm], n = X.offs[I.cB - X.Cm] - sA;
     if (n <= 0) return;
     const int pad = sA & 1;
     const long long g0 = sA - pad;
     int cnt = round_up2(pad + n);
     bool tail = false;
     if (g0 + cnt > a.capacity) { cnt -= 2; tail = true; } // the array's last, odd, element
-    const int ea = cA & ~1;
-    const int ecount = round_up2(cB + 1 - ea);
-    const unsigned mb = S.mbar(stage);
-    const unsigned tx = 32u * (unsigned)cnt + 8u * (unsigned)ecount;
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(mb), "r"(tx) : "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(mb), "r"(32u * (unsigned)cnt) : "memory");
     if (cnt > 0) {
         const unsigned bytes = 8u * (unsigned)cnt;
-        bulk_g2s(S.sx(stage), a.sx + g0, bytes, mb);
-        bulk_g2s(S.svx(stage), a.svx + g0, bytes, mb);
-        bulk_g2s(S.svy(stage), a.svy + g0, bytes, mb);
-        bulk_g2s(S.svz(stage), a.svz + g0, bytes, mb);
+        bulk_g2s(stage, a.sx + g0, bytes, mb);
+        bulk_g2s(stage + X.CAP, a.svx + g0, bytes, mb);
+        bulk_g2s(stage + 2 * X.CAP, a.svy + g0, bytes, mb);
+        bulk_g2s(stage + 3 * X.CAP, a.svz + g0, bytes, mb);
     }
-    bulk_g2s(S.sE(stage), a.E + ea, 8u * (unsigned)ecount, mb);
     if (tail) {
         const int li = pad + n - 1;
         const long long gi = (long long)sA + n - 1;
-        S.sx(stage)[li] = a.sx[gi]; S.svx(stage)[li] = a.svx[gi]; S.svy(stage)[li] = a.svy[gi]; S.svz(stage)[li] = a.svz[gi];
+        stage[li] = a.sx[gi]; stage[X.CAP + li] = a.svx[gi]; stage[2 * X.CAP + li] = a.svy[gi]; stage[3 * X.CAP + li] = a.svz[gi];
     }
 }
 
-__device__ __forceinline__ int fused_table_fetch(const FusedArgs &a, int4 it, int idx)
-{
-    return idx <= it.y - it.x ? a.off_old[it.x + idx] : 0;
-}
-
+template <int RMAX>
 __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
 {
     extern __shared__ __align__(128) unsigned char fused_smem[];
-    FusedSmem S;
-    S.base = fused_smem;
-    S.L = fused_layout(a.CAP, a.TPC);
-    S.CAP = a.CAP;
-    constexpr int K1 = FUSED_KMAX + 1; // row stride of the per-cell tables
+    constexpr int CAP = RMAX * 32;
+    constexpr int KP = FUSED_KMAX + 2; // row stride of the prefix samples
+    const FusedLayout L = fused_layout(CAP, a.CPC);
+    double *sE = reinterpret_cast<double *>(fused_smem + L.off_E);
+    int *offs = reinterpret_cast<int *>(fused_smem + L.off_offs);
+    int *PS = reinterpret_cast<int *>(fused_smem + L.off_ps);   // PS[class][cl] = class prefix count at the start of cell cl
+    int *bas = reinterpret_cast<int *>(fused_smem + L.off_base); // bas[class*32 + cl]: final slot = bas + class prefix count
+    double *qx = reinterpret_cast<double *>(fused_smem + L.off_q), *qvx = qx + FUSED_DEF, *qvy = qx + 2 * FUSED_DEF,
+           *qvz = qx + 3 * FUSED_DEF;
+    int *qpos = reinterpret_cast<int *>(qx + 4 * FUSED_DEF);
+    const unsigned mb0 = smem_u32(fused_smem + L.off_mbar), mb1 = mb0 + 8, mbE = mb0 + 16;
     const int lane = threadIdx.x;
     const unsigned lt = (1u << lane) - 1u;
     DevState *st = a.st;
@@ -291,221 +311,158 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
     int bad = 0; // FA_* bits
     int mc = 0;  // largest new per-cell count seen by this lane
     float vm2 = 0.f;
-    int4 *items = S.items();
-    int *kinds = S.kind();
 
-    // ---- the chunk's work items: [halo cell] real tiles ... [halo cell | virtual end] --------------
-    const int ntiles = st->ntiles;
-    const int kA = blockIdx.x * a.TPC;
-    bool active = kA < ntiles && !*(volatile int *)&st->abort;
-    int nitems = 0;
-    if (active) {
-        const int kB = min(kA + a.TPC, ntiles);
-        const int2 d0 = a.td_old[kA], dm = a.td_old[kB];
-        const int cS = d0.x, cE = dm.x;
-        if (cS >= cE) {
-            active = false;
-        } else {
-            if (cS > 0) {
-                if (lane == 0) {
-                    items[0] = make_int4(cS - 1, cS, a.off_old[cS - 1], d0.y);
-                    kinds[0] = FK_HALO;
-                }
-                nitems = 1;
-            }
-            for (int k0 = kA; k0 < kB; k0 += 32) {
-                const int k = k0 + lane;
-                int2 da = make_int2(0, 0), db = da;
-                bool ne = false;
-                if (k < kB) {
-                    da = a.td_old[k];
-                    db = a.td_old[k + 1];
-                    ne = db.x > da.x;
-                }
-                const unsigned m = __ballot_sync(FULL, ne);
-                if (ne) {
-                    const int idx = nitems + __popc(m & lt);
-                    items[idx] = make_int4(da.x, db.x, da.y, db.y);
-                    kinds[idx] = FK_REAL;
-                }
-                nitems += __popc(m);
-            }
-            if (lane == 0) {
-                if (cE < nc) {
-                    items[nitems] = make_int4(cE, cE + 1, dm.y, a.off_old[cE + 1]);
-                    kinds[nitems] = FK_HALO;
-                } else {
-                    items[nitems] = make_int4(nc, nc, dm.y, dm.y);
-                    kinds[nitems] = FK_VIRTUAL;
-                }
-            }
-            ++nitems;
-            __syncwarp();
-            for (int q = lane; q < nitems; q += 32) {
-                const int4 I = items[q];
-                if (round_up2((I.z & 1) + (I.w - I.z)) > a.CAP || I.y - I.x > FUSED_KMAX || I.w < I.z) bad |= FA_TILE_OVERFLOW;
-            }
-            if (__any_sync(FULL, bad != 0)) active = false;
-        }
-    }
-
-    if (active) {
+    if (!*(volatile int *)&st->abort) {
+        FusedCtx X;
+        X.C0 = blockIdx.x * a.CPC;
+        X.C1 = min(X.C0 + a.CPC, nc);
+        X.Cm = max(X.C0 - 1, 0);
+        X.nc = nc;
+        X.CAP = CAP;
+        X.offs = offs;
+        const int Cm = X.Cm, Cp = min(X.C1 + 1, nc);
+        for (int idx = lane; idx <= Cp - Cm; idx += 32) offs[idx] = a.off_old[Cm + idx];
+        const int ea = Cm & ~1;
         if (lane == 0) {
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(S.mbar(0)) : "memory");
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(S.mbar(1)) : "memory");
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(mb0) : "memory");
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(mb1) : "memory");
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(mbE) : "memory");
             asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+            // E nodes Cm .. Cp of the chunk (16-byte aligned window; E is padded)
+            const unsigned eb = 8u * (unsigned)round_up2(Cp + 1 - ea);
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(mbE), "r"(eb) : "memory");
+            bulk_g2s(sE, a.E + ea, eb, mbE);
         }
         __syncwarp();
         const int OL = st->f_OL, AR = st->f_AR, shift = AR - OL;
+        int phase = 0, cur = 0;
+        FusedItem I0 = fused_next_item(X, phase, cur, lane, bad);
+        FusedItem I1 = fused_next_item(X, phase, cur, lane, bad);
+        double *stage0 = reinterpret_cast<double *>(fused_smem), *stage1 = reinterpret_cast<double *>(fused_smem + L.stage_bytes);
         if (lane == 0) {
-            fused_issue(a, S, items[0], 0);
-            if (nitems > 1) fused_issue(a, S, items[1], 1);
+            fused_issue(a, X, I0, stage0, mb0);
+            fused_issue(a, X, I1, stage1, mb1);
         }
-        int *start = S.start();
-        unsigned short *ps = S.ps(), *pe = S.pe();
-        int *cnt = S.cnt(), *bas = S.bas();
-        unsigned *code = S.code();
-        double *qx = S.q(), *qvx = qx + FUSED_DEF, *qvy = qx + 2 * FUSED_DEF, *qvz = qx + 3 * FUSED_DEF;
-        int *qpos = reinterpret_cast<int *>(qx + 4 * FUSED_DEF);
-        if (lane < 3) cnt[lane * K1] = 0;
-        // carry across tiles: counts of the previous tile's last cell sit at table index 0
+        // carry across tiles: class counts of the previous tile's last cell
+        int pvL = 0, pvS = 0, pvR = 0;
         int pvRR = 0;    // R of the cell before the carried one
         int pv_off = 0;  // off_old of the carried cell
         int pv_real = 0; // the carried cell belongs to this chunk (finalize it)
         int ndef = 0;    // deferred right-movers of the carried cell
         unsigned ph0 = 0, ph1 = 0;
-        int4 itn = items[0];
-        int t0 = fused_table_fetch(a, itn, lane), t1 = fused_table_fetch(a, itn, lane + 32);
+        mbar_wait(mbE, 0);
 
-        for (int it = 0; it < nitems; ++it) {
-            const int stage = it & 1;
-            const int4 I = itn;
-            const int kind = kinds[it];
-            const int cA = I.x, cB = I.y, sA = I.z, n = I.w - I.z, ncell = cB - cA, pad = sA & 1;
-            if (lane <= ncell) start[lane] = t0 - sA + pad;
-            if (lane + 32 <= ncell) start[lane + 32] = t1 - sA + pad;
-            if (it + 1 < nitems) {
-                itn = items[it + 1];
-                t0 = fused_table_fetch(a, itn, lane);
-                t1 = fused_table_fetch(a, itn, lane + 32);
-            }
-            __syncwarp();
+        for (int it = 0; I0.kind != FK_NONE; ++it) {
+            const FusedItem I2 = fused_next_item(X, phase, cur, lane, bad);
+            const int kind = I0.kind, cA = I0.cA, cB = I0.cB, ncell = cB - cA;
+            const int sA = kind == FK_VIRTUAL ? 0 : offs[cA - Cm];
+            const int n = kind == FK_VIRTUAL ? 0 : offs[cB - Cm] - sA;
+            const int pad = sA & 1, gbase = sA - pad;
+            const int nrows = n > 0 ? (pad + n + 31) >> 5 : 0;
+            double *px = (it & 1) ? stage1 : stage0;
             if (n > 0) {
-                if (stage == 0) { mbar_wait(S.mbar(0), ph0); ph0 ^= 1u; }
-                else            { mbar_wait(S.mbar(1), ph1); ph1 ^= 1u; }
+                if (it & 1) { mbar_wait(mb1, ph1); ph1 ^= 1u; }
+                else        { mbar_wait(mb0, ph0); ph0 ^= 1u; }
             }
-            double *px = S.sx(stage), *pvx = S.svx(stage), *pvy = S.svy(stage), *pvz = S.svz(stage);
-            const double *pE = S.sE(stage);
-            const int ea = cA & ~1;
-            const int nrows = (pad + n + 31) >> 5;
 
-            // ---- sweep 1: push in place, classify, prefix counts per class ------------------------
-            int runL = 0, runS = 0, runR = 0;
-            for (int r = 0; r < nrows; ++r) {
-                const int i = (r << 5) + lane;
-                int g = 3, cl = 0;
-                bool first = false, last = false;
-                if (i >= pad && i < pad + n) {
-                    const double x = px[i], vx = pvx[i], vy = pvy[i], vz = pvz[i];
+            // ---- sweep 1: push into registers, classify, prefix counts per class --------------------
+            double X_[RMAX], VX_[RMAX], VY_[RMAX], VZ_[RMAX];
+            int PK_[RMAX]; // -1, or (class prefix count << 8) | class*32 + local cell
+            int runL = 0, runS = 0, runR = 0, lastcl = -1;
+#pragma unroll
+            for (int r = 0; r < RMAX; ++r) {
+                if (r < nrows) {
+                    const int i = (r << 5) + lane;
+                    const bool valid = i >= pad && i < pad + n;
+                    const int ic = min(max(i, pad), pad + n - 1);
+                    const double x = px[ic], vx = px[CAP + ic], vy = px[2 * CAP + ic], vz = px[3 * CAP + ic];
                     double xs, jf;
-                    int j;
-                    bool ok = gather_cell(a.k, x, xs, jf, j);
-                    if (ok) {
-                        const int c = j - cA;
-                        ok = c >= 0 && c < ncell;
-                        if (ok) {
-                            const int s0 = start[c], s1 = start[c + 1];
-                            ok = i >= s0 && i < s1;
-                            if (ok) {
-                                cl = c;
-                                first = i == s0;
-                                last = i == s1 - 1;
-                                const double E0 = pE[j - ea], E1 = pE[j - ea + 1];
-                                PushOut o;
-                                push_core(a.k, x, vx, vy, vz, xs, jf, j, E0, E1, o);
-                                int b = 0;
-                                g = fused_classify(a.k, j, o, b);
-                                if (b) { bad |= FA_BAD_PARTICLE; g = 3; }
-                                px[i] = o.x; pvx[i] = o.vx; pvy[i] = o.vy; pvz[i] = o.vz;
-                                vm2 = fmaxf(vm2, __double2float_ru(o.vx * o.vx + o.vy * o.vy + o.vz * o.vz));
-                            }
+                    int j = cA;
+                    const bool dom = gather_cell(a.k, x, xs, jf, j);
+                    const int cl = j - cA;
+                    const bool inr = dom && cl >= 0 && cl < ncell;
+                    if (!inr) { j = cA; jf = (double)cA; }
+                    const double E0 = sE[j - ea], E1 = sE[j - ea + 1];
+                    PushOut o;
+                    push_core(a.k, x, vx, vy, vz, xs, jf, j, E0, E1, o);
+                    int b = 0;
+                    int g = fused_classify(a.k, j, o, b);
+                    const bool good = valid && inr && !b;
+                    if (valid && !good) bad |= FA_BAD_PARTICLE;
+                    if (!good) g = 3;
+                    if (valid && inr) vm2 = fmaxf(vm2, __double2float_ru(o.vx * o.vx + o.vy * o.vy + o.vz * o.vz));
+                    // cell of this slot for the border test: -1 before the tile, ncell behind it
+                    const int cle = valid ? (good ? cl : -1) : (i < pad ? -1 : ncell);
+                    int prev = __shfl_up_sync(FULL, cle, 1);
+                    if (lane == 0) prev = lastcl;
+                    lastcl = __shfl_sync(FULL, cle, 31);
+                    const unsigned mL = __ballot_sync(FULL, g == 0), mS = __ballot_sync(FULL, g == 1), mR = __ballot_sync(FULL, g == 2);
+                    const int bL = runL + __popc(mL & lt), bS = runS + __popc(mS & lt), bR = runR + __popc(mR & lt);
+                    if (cle > prev) {
+                        // first slot of cell cle (cells prev+1 .. cle-1 are empty): sample the prefix counts and
+                        // check the grouping against off_old
+                        for (int q = prev + 1; q <= cle; ++q) {
+                            PS[q] = bL; PS[KP + q] = bS; PS[2 * KP + q] = bR;
+                            if (offs[cA - Cm + q] - gbase != i) bad |= FA_BAD_PARTICLE;
                         }
+                    } else if (cle < prev) {
+                        bad |= FA_BAD_PARTICLE;
                     }
-                    if (!ok) bad |= FA_BAD_PARTICLE;
+                    PK_[r] = g < 3 ? ((g == 0 ? bL : (g == 1 ? bS : bR)) << 8) | (g * 32 + cl) : -1;
+                    X_[r] = o.x; VX_[r] = o.vx; VY_[r] = o.vy; VZ_[r] = o.vz;
+                    runL += __popc(mL); runS += __popc(mS); runR += __popc(mR);
                 }
-                const unsigned mL = __ballot_sync(FULL, g == 0), mS = __ballot_sync(FULL, g == 1), mR = __ballot_sync(FULL, g == 2);
-                const int bL = runL + __popc(mL & lt), bS = runS + __popc(mS & lt), bR = runR + __popc(mR & lt);
-                if (first) {
-                    ps[cl] = (unsigned short)bL; ps[K1 + cl] = (unsigned short)bS; ps[2 * K1 + cl] = (unsigned short)bR;
+            }
+            if (kind != FK_VIRTUAL) {
+                for (int q = lastcl + 1 + lane; q <= ncell; q += 32) {
+                    PS[q] = runL; PS[KP + q] = runS; PS[2 * KP + q] = runR;
+                    if (offs[cA - Cm + q] - gbase != pad + n) bad |= FA_BAD_PARTICLE;
                 }
-                if (last) {
-                    pe[cl] = (unsigned short)(bL + (g == 0)); pe[K1 + cl] = (unsigned short)(bS + (g == 1));
-                    pe[2 * K1 + cl] = (unsigned short)(bR + (g == 2));
-                }
-                const int mine = g == 0 ? bL : (g == 1 ? bS : bR);
-                code[i] = (unsigned)g | ((unsigned)cl << 2) | ((unsigned)mine << 8);
-                runL += __popc(mL); runS += __popc(mS); runR += __popc(mR);
             }
             __syncwarp();
+            // the stage has been read: refill it with the item after next
+            if (lane == 0) fused_issue(a, X, I2, px, (it & 1) ? mb1 : mb0);
 
-            // ---- per-cell phase: counts -> table index cl+1 -----------------------------------------
-            if (kind == FK_VIRTUAL) {
-                if (lane < 3) cnt[lane * K1 + 1] = 0;
-            } else {
-                for (int cl = lane; cl < ncell; cl += 32) {
-                    const bool ne = start[cl + 1] > start[cl];
-                    cnt[cl + 1] = ne ? (int)pe[cl] - (int)ps[cl] : 0;
-                    cnt[K1 + cl + 1] = ne ? (int)pe[K1 + cl] - (int)ps[K1 + cl] : 0;
-                    cnt[2 * K1 + cl + 1] = ne ? (int)pe[2 * K1 + cl] - (int)ps[2 * K1 + cl] : 0;
-                }
+            // ---- per-cell phase (lane = local cell) -------------------------------------------------
+            int Lc = 0, Sc = 0, Rc = 0, psL = 0, psS = 0, psR = 0;
+            if (kind != FK_VIRTUAL && lane < ncell) {
+                psL = PS[lane]; Lc = PS[lane + 1] - psL;
+                psS = PS[KP + lane]; Sc = PS[KP + lane + 1] - psS;
+                psR = PS[2 * KP + lane]; Rc = PS[2 * KP + lane + 1] - psR;
             }
-            __syncwarp();
-            // destination bases of this tile's cells:  slot = base[class][cl] + prefix count
-            if (kind == FK_REAL) {
-                for (int cl = lane; cl < ncell; cl += 32) {
-                    const int c = cA + cl, t = cl + 1;
-                    const int oo = sA + start[cl] - pad, oo1 = sA + start[cl + 1] - pad;
-                    const int Lc = cnt[t], Rc = cnt[2 * K1 + t], Rm1 = cnt[2 * K1 + t - 1];
-                    const int Lp1 = cl < ncell - 1 ? cnt[t + 1] : 0; // last cell: added when the next tile knows it
-                    const int pre_c = (a.k.periodic && c == nc - 1) ? OL : 0;
-                    const int pre_c1 = (a.k.periodic && c + 1 == nc - 1) ? OL : 0;
-                    bas[cl] = oo + (c == 1 ? -OL : shift) - Rm1 - (int)ps[cl];
-                    bas[K1 + cl] = oo + (c >= 1 ? shift : 0) + Lc + pre_c - (int)ps[K1 + cl];
-                    bas[2 * K1 + cl] = oo1 + shift - Rc + Lp1 + pre_c1 - (int)ps[2 * K1 + cl];
-                }
-            }
-            // finalize cells cA-1 .. cB-2 (table index 0 .. ncell-1): count, offset, next partition
-            {
-                const int nfin = kind == FK_REAL ? ncell : 1;
-                for (int t = lane; t < nfin; t += 32) {
-                    if (t == 0 && !pv_real) continue;
-                    const int c = cA - 1 + t;
-                    const int Rm1 = t == 0 ? pvRR : cnt[2 * K1 + t - 1];
-                    const int Lc = cnt[t], Sc = cnt[K1 + t], Lp1 = cnt[t + 1];
-                    const int oo = t == 0 ? pv_off : sA + start[t - 1] - pad;
-                    const int pre_c = (a.k.periodic && c == nc - 1) ? OL : 0;
-                    const int post_c = c == 0 ? AR : 0;
-                    const int cn = pre_c + Rm1 + Sc + Lp1 + post_c;
-                    const int o0 = c == 0 ? 0 : oo + shift - Rm1 + Lc;
-                    const int o1 = o0 + cn;
+            int Rm1 = __shfl_up_sync(FULL, Rc, 1);
+            if (lane == 0) Rm1 = pvR;
+            int Lp1 = __shfl_down_sync(FULL, Lc, 1);
+            if (lane >= ncell - 1) Lp1 = 0; // last cell: added when the next tile knows it
+            const int Lc0 = __shfl_sync(FULL, Lc, 0);
+            if (kind == FK_REAL && lane < ncell) {
+                const int c = cA + lane;
+                const int oo = offs[c - Cm], oo1 = offs[c + 1 - Cm];
+                const int pre_c = (a.k.periodic && c == nc - 1) ? OL : 0;
+                const int pre_c1 = (a.k.periodic && c + 1 == nc - 1) ? OL : 0;
+                bas[lane] = oo + (c == 1 ? -OL : shift) - Rm1 - psL;
+                bas[32 + lane] = oo + (c >= 1 ? shift : 0) + Lc + pre_c - psS;
+                bas[64 + lane] = oo1 + shift - Rc + Lp1 + pre_c1 - psR;
+                if (lane < ncell - 1) { // count / offset of cell c (the tile's last cell waits for the next tile)
+                    const int cn = pre_c + Rm1 + Sc + Lp1 + (c == 0 ? AR : 0);
                     a.count_new[c] = cn;
-                    a.off_new[c] = o0;
+                    a.off_new[c] = c == 0 ? 0 : oo + shift - Rm1 + Lc;
                     mc = max(mc, cn);
-                    for (int kb = o0 / a.T + 1; kb <= o1 / a.T; ++kb)
-                        if (kb < a.td_cap) a.td_new[kb] = make_int2(c + 1, o1);
-                    if (c == 0) a.td_new[0] = make_int2(0, 0);
-                    if (c == nc - 1) {
-                        a.off_new[nc] = o1;
-                        const int nt = o1 / a.T + 1;
-                        if (nt < a.td_cap) a.td_new[nt] = make_int2(nc, o1);
-                        st->ntiles_next = nt;
-                    }
                 }
             }
-            // right-movers of the previous tile's last cell: their cell is cA, its L count is known now
-            if (ndef) {
+            if (pv_real && lane == 0) { // count / offset of the previous tile's last cell
+                const int c = cA - 1;
+                const int pre_c = (a.k.periodic && c == nc - 1) ? OL : 0;
+                const int cn = pre_c + pvRR + pvS + Lc0 + (c == 0 ? AR : 0);
+                const int o0 = c == 0 ? 0 : pv_off + shift - pvRR + pvL;
+                a.count_new[c] = cn;
+                a.off_new[c] = o0;
+                if (c == nc - 1) a.off_new[nc] = o0 + cn;
+                mc = max(mc, cn);
+            }
+            if (ndef) { // right-movers of the previous tile's last cell: their cell is cA, its L count is known now
                 if (lane < ndef) {
-                    const long long p = (long long)qpos[lane] + cnt[1];
+                    const long long p = (long long)qpos[lane] + Lc0;
                     if (p < 0 || p >= a.capacity) bad |= FA_BAD_PARTICLE;
                     else {
                         a.dx[p] = qx[lane]; a.dvx[p] = qvx[lane]; a.dvy[p] = qvy[lane]; a.dvz[p] = qvz[lane];
@@ -516,58 +473,52 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
             }
             __syncwarp();
 
-            // ---- sweep 2: every particle straight to its final slot ---------------------------------
+            // ---- sweep 2: every particle straight to its final slot ----------------------------------
             if (kind == FK_REAL) {
-                for (int r = 0; r < nrows; ++r) {
-                    const int i = (r << 5) + lane;
-                    bool defer = false, store = false;
-                    long long p = 0;
-                    int cl = 0, g = 3;
-                    if (i >= pad && i < pad + n) {
-                        const unsigned cd = code[i];
-                        g = (int)(cd & 3u);
-                        if (g < 3) {
-                            cl = (int)((cd >> 2) & 63u);
-                            p = (long long)bas[g * K1 + cl] + (int)(cd >> 8);
-                            defer = g == 2 && cl == ncell - 1;
-                            store = !defer;
+                const int kdef = 64 + ncell - 1; // class R of the tile's last cell
+#pragma unroll
+                for (int r = 0; r < RMAX; ++r) {
+                    if (r < nrows) {
+                        const int pk = PK_[r];
+                        const int key = pk & 0xff;
+                        const bool has = pk >= 0;
+                        const bool defer = has && key == kdef;
+                        long long p = 0;
+                        if (has) p = (long long)bas[key] + (pk >> 8);
+                        if (has && !defer) {
+                            if (p < 0 || p >= a.capacity) bad |= FA_BAD_PARTICLE;
+                            else {
+                                a.dx[p] = X_[r]; a.dvx[p] = VX_[r]; a.dvy[p] = VY_[r]; a.dvz[p] = VZ_[r];
+                                a.dcell[p] = cA + (key & 31) + (key >> 5) - 1;
+                            }
                         }
-                    }
-                    const unsigned md = __ballot_sync(FULL, defer);
-                    if (store) {
-                        if (p < 0 || p >= a.capacity) bad |= FA_BAD_PARTICLE;
-                        else {
-                            a.dx[p] = px[i]; a.dvx[p] = pvx[i]; a.dvy[p] = pvy[i]; a.dvz[p] = pvz[i];
-                            a.dcell[p] = cA + cl + g - 1;
+                        const unsigned md = __ballot_sync(FULL, defer);
+                        if (md) {
+                            if (defer) {
+                                const int q = ndef + __popc(md & lt);
+                                if (q < FUSED_DEF) {
+                                    qx[q] = X_[r]; qvx[q] = VX_[r]; qvy[q] = VY_[r]; qvz[q] = VZ_[r];
+                                    qpos[q] = (int)p;
+                                } else bad |= FA_DEFER_OVERFLOW;
+                            }
+                            ndef = min(ndef + __popc(md), FUSED_DEF);
                         }
-                    }
-                    if (md) {
-                        if (defer) {
-                            const int q = ndef + __popc(md & lt);
-                            if (q < FUSED_DEF) {
-                                qx[q] = px[i]; qvx[q] = pvx[i]; qvy[q] = pvy[i]; qvz[q] = pvz[i];
-                                qpos[q] = (int)p;
-                            } else bad |= FA_DEFER_OVERFLOW;
-                        }
-                        ndef = min(ndef + __popc(md), FUSED_DEF);
                     }
                 }
             }
-            // carry: this tile's last cell becomes table index 0
+            // carry: this tile's last cell
             if (kind != FK_VIRTUAL) {
-                const int nRR = cnt[2 * K1 + ncell - 1];
-                const int cL_ = cnt[ncell], cS_ = cnt[K1 + ncell], cR_ = cnt[2 * K1 + ncell];
-                const int po = sA + start[ncell - 1] - pad;
-                __syncwarp();
-                if (lane == 0) { cnt[0] = cL_; cnt[K1] = cS_; cnt[2 * K1] = cR_; }
+                const int nRR = ncell >= 2 ? __shfl_sync(FULL, Rc, ncell - 2) : pvR;
+                pvL = __shfl_sync(FULL, Lc, ncell - 1);
+                pvS = __shfl_sync(FULL, Sc, ncell - 1);
+                pvR = __shfl_sync(FULL, Rc, ncell - 1);
                 pvRR = nRR;
-                pv_off = po;
+                pv_off = offs[cB - 1 - Cm];
                 pv_real = kind == FK_REAL;
             }
-            // refill this stage with the tile after next (generic writes above -> async proxy)
-            asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
             __syncwarp();
-            if (lane == 0 && it + 2 < nitems) fused_issue(a, S, items[it + 2], stage);
+            I0 = I1;
+            I1 = I2;
         }
     }
 
@@ -591,7 +542,6 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
                 st->wall[0] += *(volatile unsigned long long *)&st->wall_pend[0];
                 st->wall[1] += *(volatile unsigned long long *)&st->wall_pend[1];
                 st->vmax2 = *(volatile unsigned *)&st->vmax2_next;
-                st->ntiles = *(volatile int *)&st->ntiles_next;
                 st->maxcount = *(volatile int *)&st->maxcount_next;
                 st->w_acc = 0;
                 st->step_max = 0;
@@ -612,28 +562,12 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
     }
 }
 
-// Tile partition of an offset array: td[k] = (first cell whose offset is >= k*T, that offset), for
-// k = 0 .. ntiles with ntiles = n/T + 1 and td[ntiles] = (nc, n).  One thread per cell c settles
-// cell c+1.  Used at pic_create and after every arrange of the split path; a fused step writes the
-// next partition itself.
-__global__ void bounds_kernel(const int *__restrict__ off, int nc, int T, int2 *__restrict__ td, int td_cap, DevState *st,
-                              const int *guard)
+// Largest per-cell count of an offset array (sizes the fused tiles; only ever raises the bound).
+__global__ void maxcount_kernel(const int *__restrict__ off, int nc, DevState *st, const int *guard)
 {
     if (guard && !*guard) return;
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
-    int cn = 0;
-    if (c < nc) {
-        const int o0 = off[c], o1 = off[c + 1];
-        cn = o1 - o0;
-        for (int kb = o0 / T + 1; kb <= o1 / T; ++kb)
-            if (kb < td_cap) td[kb] = make_int2(c + 1, o1);
-        if (c == 0) td[0] = make_int2(0, 0);
-        if (c + 1 == nc) {
-            const int nt = o1 / T + 1;
-            if (nt < td_cap) td[nt] = make_int2(nc, o1);
-            st->ntiles = nt;
-        }
-    }
+    int cn = c < nc ? off[c + 1] - off[c] : 0;
     cn = __reduce_max_sync(FULL, cn);
     if ((threadIdx.x & 31) == 0 && cn > *(volatile int *)&st->maxcount) atomicMax(&st->maxcount, cn);
 }

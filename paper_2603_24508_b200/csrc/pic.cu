@@ -49,11 +49,8 @@ struct pic_species {
     unsigned long long *d_scan = nullptr;
     size_t scan_words = 0;
     // fused push+arrange step (fused.cuh)
-    int2 *d_td[2]{};                   // tile partition of d_off[i] (fused.cuh: bounds_kernel)
-    int T = FUSED_T_DEFAULT, td_cap = 0;
-    int h_maxcount = 0;                // largest per-cell count at the last sync (sizes the fused stage)
+    int h_maxcount = 0;                // bound of the largest per-cell count at the last sync (sizes the fused tiles)
     int h_abort_reason = 0;
-    bool bounds_valid = false;         // d_td[cur_off] describes d_off[cur_off]
     bool fused_off = false;            // the device reported a declined fused step (sticky)
     // host-side conservative bound on cell displacement since the last arrange (decides whether the
     // general-path kernels need to be enqueued at all)
@@ -81,7 +78,7 @@ struct pic_sim {
     std::vector<pic_species *> sp;
     unsigned long long launches = 0;
     int opt_e_stage = 1, opt_fused = 1, opt_timing = 0;
-    int opt_fused_tpc = FUSED_TPC_DEFAULT, opt_fused_cap = 0; // tuning knobs of the fused step (0 = automatic)
+    int opt_fused_cpc = 0, opt_fused_rows = 0; // tuning knobs of the fused step (0 = automatic)
     int sm_count = 148;
     // per-kernel device timing (option "kernel_timing"): event pairs recorded around launches
     struct Span { int id; cudaEvent_t a, b; };
@@ -146,8 +143,6 @@ static void free_species(pic_species *s)
     cudaFree(s->d_st);
     for (int b = 0; b < 2; ++b) { cudaFree(s->d_count[b]); cudaFree(s->d_off[b]); }
     cudaFree(s->d_scan);
-    cudaFree(s->d_td[0]);
-    cudaFree(s->d_td[1]);
     delete s;
 }
 
@@ -215,23 +210,21 @@ static float bits_to_float(unsigned u)
     return f;
 }
 
-// tile partition of the fused step from the offsets in slot `which`
-static int run_bounds(pic_species *s, int which, const int *guard)
+// raise DevState::maxcount to the largest per-cell count of the offsets in slot `which`
+static int run_maxcount(pic_species *s, int which, const int *guard)
 {
     pic_sim *sim = s->sim;
     const int nc = sim->nc;
-    bounds_kernel<<<(nc + 255) / 256, 256, 0, sim->stream>>>(s->d_off[which], nc, s->T, s->d_td[which], s->td_cap, s->d_st, guard);
-    if (int rc = launch_check(sim, "bounds_kernel")) return rc;
-    if (!guard) s->bounds_valid = true;
-    return PIC_OK;
+    maxcount_kernel<<<(nc + 255) / 256, 256, 0, sim->stream>>>(s->d_off[which], nc, s->d_st, guard);
+    return launch_check(sim, "maxcount_kernel");
 }
 
-static int fused_cap(const pic_species *s, int *ctas_per_sm);
+static int fused_rows(const pic_species *s, int *ctas_per_sm);
 
 static bool fused_possible(const pic_species *s)
 {
     return s->sim->opt_fused && !s->fused_off && s->arrange_every == 1 && s->sim->nc >= FUSED_MIN_NC &&
-           fused_cap(s, nullptr) > 0;
+           fused_rows(s, nullptr) > 0;
 }
 
 // Host-side bound (cells) on what one more mover step can displace any particle.
@@ -317,24 +310,15 @@ static int create_species(pic_sim *sim, const pic_species_desc &d, pic_species *
     }
     ScanFold nofold{nullptr, 0, 0, 0, nullptr};
     if (int rc = run_scan(s, s->d_count[0], s->d_off[0], nc, nofold)) return rc;
-    // fused step: tile partition (two copies: a fused step reads one and writes the other)
-    s->T = FUSED_T_DEFAULT;
-    s->td_cap = (int)(d.capacity / FUSED_T_MIN) + 3;
-    for (int b = 0; b < 2; ++b) {
-        CU(cudaMalloc(&s->d_td[b], sizeof(int2) * (size_t)s->td_cap));
-        CU(cudaMemsetAsync(s->d_td[b], 0, sizeof(int2) * (size_t)s->td_cap, sim->stream));
-    }
     s->vkick = 2.0 * std::fabs(s->k.h) * sim->Emax;
     s->h_vmax = std::sqrt((double)bits_to_float(h.vmax2));
     s->h_grouped = grouped;
-    s->bounds_valid = false;
     h.status = 0;
     h.w_acc = grouped ? 0 : W_UNKNOWN;
-    h.ntiles = 1;
     CU(cudaMemcpyAsync(s->d_st, &h, sizeof h, cudaMemcpyHostToDevice, sim->stream));
     CU(cudaStreamSynchronize(sim->stream));
-    if (grouped) {
-        if (int rc = run_bounds(s, 0, nullptr)) return rc;
+    if (grouped) { // largest per-cell count: sizes the tiles of the fused step
+        if (int rc = run_maxcount(s, 0, nullptr)) return rc;
         CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, sim->stream));
         CU(cudaStreamSynchronize(sim->stream));
         s->h_maxcount = h.maxcount;
@@ -347,7 +331,9 @@ static int create_species(pic_sim *sim, const pic_species_desc &d, pic_species *
     {
         static bool attr_set = false;
         if (!attr_set) {
-            CU(cudaFuncSetAttribute(fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, FUSED_SMEM_CTA));
+            CU(cudaFuncSetAttribute(fused_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+            CU(cudaFuncSetAttribute(fused_kernel<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+            CU(cudaFuncSetAttribute(fused_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
             attr_set = true;
         }
     }
@@ -435,10 +421,8 @@ extern "C" int pic_set_option(pic_sim *sim, const char *key, int value)
     if (!strcmp(key, "e_stage") && flag) sim->opt_e_stage = value;
     else if (!strcmp(key, "kernel_timing") && flag) sim->opt_timing = value;
     else if (!strcmp(key, "fused") && flag) sim->opt_fused = value;
-    else if (!strcmp(key, "fused_tile") && value >= FUSED_T_MIN && value <= 4096) {
-        for (pic_species *s : sim->sp) { s->T = value; s->bounds_valid = false; }
-    } else if (!strcmp(key, "fused_tiles_per_cta") && value >= 1 && value <= FUSED_TPC_MAX) sim->opt_fused_tpc = value;
-    else if (!strcmp(key, "fused_stage_slots") && value >= 0 && value <= 16384 && value % 32 == 0) sim->opt_fused_cap = value;
+    else if (!strcmp(key, "fused_cells_per_cta") && value >= 0 && value <= FUSED_CPC_MAX) sim->opt_fused_cpc = value;
+    else if (!strcmp(key, "fused_rows") && (value == 0 || value == 8 || value == 12 || value == 16)) sim->opt_fused_rows = value;
     else return PIC_EINVAL;
     return PIC_OK;
 }
@@ -527,12 +511,8 @@ static int arrange_split(pic_species *s, bool hist_ready, const int *guard, bool
         KernelSpan gspan(sim, K_GENERAL);
         if (int rc = general_arrange(ga, sim->stream, sim->sm_count, &sim->launches)) return rc == PIC_ECUDA ? cuda_fail(cudaGetLastError(), "general_arrange") : rc;
     }
-    if (fused_possible(s)) {
-        if (int rc = run_bounds(s, on, guard)) return rc;
-        s->bounds_valid = true;
-    } else {
-        s->bounds_valid = false;
-    }
+    if (s->sim->opt_fused && s->arrange_every == 1)
+        if (int rc = run_maxcount(s, on, guard)) return rc;
 
     s->cur = dst;
     s->cur_off = on;
@@ -600,30 +580,29 @@ static int push_split(pic_species *s, bool will_arrange, const int *guard)
     return PIC_OK;
 }
 
-// Shared-memory stage (slots per tile) of the fused kernel for this species' current state, or 0 when
-// a tile cannot fit.  A tile holds fewer than T + maxcount particles; maxcount is the bound read at
-// the last sync, so leave room for it to grow, then use whatever the chosen occupancy leaves free.
-static int fused_cap(const pic_species *s, int *ctas_per_sm)
+// Rows of 32 slots per tile (the fused_kernel<RMAX> instance) for this species' current state, or 0
+// when a cell may not fit a tile.  A tile must hold at least one cell; maxcount is the bound read
+// at the last sync, so leave room for it to grow.
+static int fused_cells_per_cta(const pic_species *s)
 {
     const pic_sim *sim = s->sim;
-    if (sim->opt_fused_cap > 0) {
-        const int tot = fused_layout(sim->opt_fused_cap, sim->opt_fused_tpc).total;
-        if (tot > FUSED_SMEM_CTA) return 0;
-        if (ctas_per_sm) *ctas_per_sm = std::max(1, std::min(32, FUSED_SMEM_SM / (tot + 1024)));
-        return sim->opt_fused_cap;
+    if (sim->opt_fused_cpc > 0) return sim->opt_fused_cpc;
+    const long long want = sim->nc / ((long long)sim->sm_count * 16);
+    return (int)std::max<long long>(8, std::min<long long>(FUSED_CPC_DEFAULT, want));
+}
+
+static int fused_rows(const pic_species *s, int *ctas_per_sm)
+{
+    const pic_sim *sim = s->sim;
+    int rows = sim->opt_fused_rows;
+    if (rows == 0) {
+        const int mc = std::max(s->h_maxcount, 1);
+        const int need = mc + std::max(mc / 4, 32) + 2;
+        rows = need <= 8 * 32 ? 8 : need <= 12 * 32 ? 12 : need <= 16 * 32 ? 16 : 0;
     }
-    const int mc = std::max(s->h_maxcount, 1);
-    int need = s->T + mc + std::max(mc / 2, 64) + 2;
-    need = (need + 31) & ~31;
-    const int tot = fused_layout(need, sim->opt_fused_tpc).total;
-    if (tot > FUSED_SMEM_CTA) return 0;
-    const int ctas = std::max(1, std::min(32, FUSED_SMEM_SM / (tot + 1024)));
-    int cap = need;
-    while (cap + 32 <= 16384 && fused_layout(cap + 32, sim->opt_fused_tpc).total + 1024 <= FUSED_SMEM_SM / ctas &&
-           fused_layout(cap + 32, sim->opt_fused_tpc).total <= FUSED_SMEM_CTA)
-        cap += 32;
-    if (ctas_per_sm) *ctas_per_sm = ctas;
-    return cap;
+    if (rows && ctas_per_sm)
+        *ctas_per_sm = std::max(1, std::min(32, FUSED_SMEM_SM / (fused_layout(rows * 32, fused_cells_per_cta(s)).total + 1024)));
+    return rows;
 }
 
 // One fused push+arrange step, followed by the guarded split chain that redoes the step if the
@@ -637,22 +616,22 @@ static int push_fused(pic_species *s)
     a.sx = s->x[src]; a.svx = s->vx[src]; a.svy = s->vy[src]; a.svz = s->vz[src];
     a.dx = s->x[dst]; a.dvx = s->vx[dst]; a.dvy = s->vy[dst]; a.dvz = s->vz[dst]; a.dcell = s->cell[dst];
     a.E = sim->d_E;
-    a.off_old = s->d_off[oo]; a.td_old = s->d_td[oo];
-    a.count_new = s->d_count[on]; a.off_new = s->d_off[on]; a.td_new = s->d_td[on];
+    a.off_old = s->d_off[oo];
+    a.count_new = s->d_count[on]; a.off_new = s->d_off[on];
     a.st = s->d_st;
     a.k = s->k;
     a.capacity = s->capacity;
-    a.T = s->T;
-    a.TPC = sim->opt_fused_tpc;
-    a.td_cap = s->td_cap;
-    a.CAP = fused_cap(s, nullptr);
-    const int ntiles_ub = (int)(s->n_ub / s->T) + 1;
-    const int grid = (ntiles_ub + a.TPC - 1) / a.TPC;
+    a.CPC = fused_cells_per_cta(s);
+    const int rows = fused_rows(s, nullptr);
+    const int grid = (sim->nc + a.CPC - 1) / a.CPC;
+    const size_t smem = (size_t)fused_layout(rows * 32, a.CPC).total;
     {
         KernelSpan span(sim, K_FUSED);
         fused_edge_kernel<<<1, 128, 0, sim->stream>>>(a);
         if (int rc = launch_check(sim, "fused_edge_kernel")) return rc;
-        fused_kernel<<<grid, 32, fused_layout(a.CAP, a.TPC).total, sim->stream>>>(a);
+        if (rows == 8) fused_kernel<8><<<grid, 32, smem, sim->stream>>>(a);
+        else if (rows == 12) fused_kernel<12><<<grid, 32, smem, sim->stream>>>(a);
+        else fused_kernel<16><<<grid, 32, smem, sim->stream>>>(a);
         if (int rc = launch_check(sim, "fused_kernel")) return rc;
     }
     // fallback chain, all guarded by run_split; it leaves the same host-visible state behind
@@ -671,8 +650,6 @@ extern "C" int pic_push(pic_species *s, int nsteps)
         const bool will_arrange = s->arrange_every > 0 && ((s->steps + 1) % s->arrange_every) == 0;
         const bool fused = will_arrange && fused_possible(s) && s->counts_fresh && s->all_live && s->n_ub > 0;
         if (fused) {
-            if (!s->bounds_valid)
-                if (int rc = run_bounds(s, s->cur_off, nullptr)) return rc;
             if (int rc = push_fused(s)) return rc;
             s->steps++;
             continue;
@@ -773,7 +750,7 @@ extern "C" int pic_fused_info(pic_species *s, int32_t *active, int32_t *decline_
     if (active) *active = fused_possible(s) ? 1 : 0;
     if (decline_reasons) *decline_reasons = h.abort_reason;
     int ctas = 0;
-    const int cap = fused_cap(s, &ctas);
+    const int cap = 32 * fused_rows(s, &ctas);
     if (stage_slots) *stage_slots = cap;
     if (ctas_per_sm) *ctas_per_sm = ctas;
     return PIC_OK;

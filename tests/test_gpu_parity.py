@@ -241,26 +241,34 @@ def test_fused_step_is_the_one_that_runs(config, kw, steps):
 
 
 @pytest.mark.parametrize("knobs", [
-    {"fused_tile": 64}, {"fused_tile": 256, "fused_tiles_per_cta": 1}, {"fused_tile": 1024, "fused_tiles_per_cta": 3},
-    {"fused_tiles_per_cta": 256}, {"fused_stage_slots": 512}, {"fused_tile": 64, "fused_tiles_per_cta": 2},
+    {"fused_cells_per_cta": 1}, {"fused_cells_per_cta": 3, "fused_rows": 12}, {"fused_cells_per_cta": 256},
+    {"fused_rows": 16}, {"fused_cells_per_cta": 33, "fused_rows": 8}, {"fused_cells_per_cta": 7},
 ])
 @pytest.mark.parametrize("config,kw", [(4, dict(nc=4099)), (2, dict(nc=1500))])
 def test_fused_knobs_do_not_change_results(knobs, config, kw):
-    """Tile size, tiles per CTA and stage size only move the tile / chunk borders (halo cells,
-    deferred right-movers, carried counts land elsewhere); results stay bit-identical."""
+    """Cells per CTA and rows per tile only move the tile / chunk borders (halo cells, deferred
+    right-movers, carried counts land elsewhere); results stay bit-identical."""
     inp = workloads.make(config, **kw)
     sim, _ = run_stepwise(inp, 12, options={"fused": 1, **knobs}, check_every=3)
     info = pic.pic_fused_info(sim.species[0])
     assert info["decline_reasons"] == 0, info
 
 
-def test_fused_declines_when_a_tile_does_not_fit_and_split_redoes_the_step():
-    """A stage too small for the tiles (64 slots against 160 particles per cell): the fused step
-    aborts on the device, the guarded split kernels redo it from the untouched source buffers."""
-    inp = workloads.make(2, nc=1024)
-    sim, _ = run_stepwise(inp, 6, options={"fused": 1, "fused_stage_slots": 64}, check_every=1)
+def test_fused_declines_when_a_cell_does_not_fit_and_split_redoes_the_step():
+    """Tiles of 8 rows (256 slots) against 300 particles per cell: the fused step aborts on the
+    device, the guarded split kernels redo it from the untouched source buffers."""
+    inp = workloads.make(2, nc=512, ppc=300)
+    sim, _ = run_stepwise(inp, 6, options={"fused": 1, "fused_rows": 8}, check_every=1)
     info = pic.pic_fused_info(sim.species[0])
-    assert info["decline_reasons"] & 2 and info["active"] == 0, info
+    assert info["decline_reasons"] & 2, info
+
+
+def test_fused_large_cells_take_the_wide_tiles():
+    """300 particles per cell: 16-row tiles chosen automatically."""
+    inp = workloads.make(2, nc=512, ppc=300)
+    sim, _ = run_stepwise(inp, 6, options={"fused": 1}, check_every=1)
+    info = pic.pic_fused_info(sim.species[0])
+    assert info["decline_reasons"] == 0 and info["active"] == 1 and info["stage_slots"] == 512, info
 
 
 def test_fused_declines_on_a_two_cell_jump():
@@ -283,7 +291,7 @@ def test_fused_empty_cells_and_sparse_density():
         for k in ("vx", "vy", "vz"):
             s[k] = s[k] * 0.25
     inp["arrange_every"] = 1
-    sim, states = run_stepwise(inp, 25, options={"fused": 1, "fused_tile": 64}, check_every=1)
+    sim, states = run_stepwise(inp, 25, options={"fused": 1}, check_every=1)
     assert (states[0].count == 0).any()
     info = pic.pic_fused_info(sim.species[0])
     assert info["decline_reasons"] == 0, info
