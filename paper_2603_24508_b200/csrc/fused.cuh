@@ -289,9 +289,42 @@ __device__ __forceinline__ void fused_issue(const FusedArgs &a, const FusedCtx &
     }
 }
 
-template <int RMAX>
+// One mover step of one particle given the weight w = xs - floor(xs) and the two node values of its
+// gather cell: the same sequence of rounded operations as push_core, written
+// without branches (the wrapped / unwrapped positions are both formed, one is selected).
+template <bool PERIODIC>
+__device__ __forceinline__ void push_flat(const PushConst &k, double x, double vx, double vy, double vz, double w, double E0,
+                                          double E1, double &xo, double &vxo, double &vyo, double &vzo, int &cn, int &wall)
+{
+    const double dE = __dsub_rn(E1, E0);
+    const double Ep = __dadd_rn(E0, __dmul_rn(w, dE));
+    const double hE = __dmul_rn(k.h, Ep);
+    const double ux = __dadd_rn(vx, hE), uy = vy, uz = vz;
+    const double px = __dadd_rn(ux, __dsub_rn(__dmul_rn(uy, k.tz), __dmul_rn(uz, k.ty)));
+    const double py = __dadd_rn(uy, __dsub_rn(__dmul_rn(uz, k.tx), __dmul_rn(ux, k.tz)));
+    const double pz = __dadd_rn(uz, __dsub_rn(__dmul_rn(ux, k.ty), __dmul_rn(uy, k.tx)));
+    const double wx = __dadd_rn(ux, __dsub_rn(__dmul_rn(py, k.sz), __dmul_rn(pz, k.sy)));
+    const double wy = __dadd_rn(uy, __dsub_rn(__dmul_rn(pz, k.sx), __dmul_rn(px, k.sz)));
+    const double wz = __dadd_rn(uz, __dsub_rn(__dmul_rn(px, k.sy), __dmul_rn(py, k.sx)));
+    const double nvx = __dadd_rn(wx, hE);
+    const double xn = __dadd_rn(x, __dmul_rn(nvx, k.dt));
+    double xw = xn;
+    wall = 0;
+    if (PERIODIC) {
+        const double xm = __dsub_rn(xn, k.L), xp = __dadd_rn(xn, k.L);
+        xw = xn >= k.L ? xm : (xn < 0.0 ? (xp >= k.L ? 0.0 : xp) : xn);
+    } else {
+        wall = xn < 0.0 ? 1 : (xn >= k.L ? 2 : 0);
+    }
+    cn = min(__double2int_rd(__dmul_rn(xw, k.inv_dx)), k.nc - 1);
+    xo = xw; vxo = nvx; vyo = wy; vzo = wz;
+}
+
+template <int RMAX, bool PERIODIC>
 __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
 {
+    constexpr int GS = 4; // rows pushed together in sweep 1a
+    static_assert(RMAX % GS == 0, "RMAX must be a multiple of the row group");
     extern __shared__ __align__(128) unsigned char fused_smem[];
     constexpr int CAP = RMAX * 32;
     constexpr int KP = FUSED_KMAX + 2; // row stride of the prefix samples
@@ -323,6 +356,9 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
         const int Cm = X.Cm, Cp = min(X.C1 + 1, nc);
         for (int idx = lane; idx <= Cp - Cm; idx += 32) offs[idx] = a.off_old[Cm + idx];
         const int ea = Cm & ~1;
+        const double *sEs = sE - ea; // E node j of the chunk's window sits at sEs[j]
+        const double dncm1 = (double)(nc - 1);
+        const unsigned cap32 = (unsigned)a.capacity;
         if (lane == 0) {
             asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(mb0) : "memory");
             asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(mb1) : "memory");
@@ -365,34 +401,61 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
                 else        { mbar_wait(mb0, ph0); ph0 ^= 1u; }
             }
 
-            // ---- sweep 1: push into registers, classify, prefix counts per class --------------------
+            // ---- sweep 1a: push into registers and classify.  Straight-line code, GS rows at a time, no warp
+            // collectives and no branches inside a group, so the rows' dependency chains interleave.
+            // Slots outside the tile (the alignment pad, the tail of the last row, rows behind it inside a
+            // group) recompute a clamped slot and are masked out.
             double X_[RMAX], VX_[RMAX], VY_[RMAX], VZ_[RMAX];
-            int PK_[RMAX]; // -1, or (class prefix count << 8) | class*32 + local cell
+            int W_[RMAX]; // 1a: class | (border cell + 1) << 2 | bad << 8;  1b: -1, or prefix count << 8 | class*32 + cell
+#pragma unroll
+            for (int r0 = 0; r0 < RMAX; r0 += GS) {
+                if (r0 < nrows) {
+#pragma unroll
+                    for (int r = r0; r < r0 + GS; ++r) {
+                        const int i = (r << 5) + lane;
+                        const bool valid = (unsigned)(i - pad) < (unsigned)n;
+                        const int ic = min(max(i, pad), pad + n - 1);
+                        const double x = px[ic], vx = px[CAP + ic], vy = px[2 * CAP + ic], vz = px[3 * CAP + ic];
+                        const double xs = __dmul_rn(x, a.k.inv_dx);
+                        double jf = floor(xs);
+                        const int j0 = __double2int_rd(xs);
+                        const bool dom = xs >= 0.0 && j0 <= nc;
+                        if (j0 > nc - 1) jf = dncm1;
+                        const int jc = min(j0, nc - 1);
+                        const int cl = jc - cA;
+                        const bool inr = dom && (unsigned)cl < (unsigned)ncell;
+                        const int j = inr ? jc : cA;
+                        const double E0 = sEs[j], E1 = sEs[j + 1];
+                        int cn, wall;
+                        push_flat<PERIODIC>(a.k, x, vx, vy, vz, __dsub_rn(xs, jf), E0, E1, X_[r], VX_[r], VY_[r], VZ_[r], cn, wall);
+                        const int d = cn - j;
+                        int g = (unsigned)(d + 1) <= 2u ? d + 1 : 3;
+                        bool legit; // class X: out of cell 0 downwards / out of cell nc-1 upwards only
+                        if (PERIODIC) {
+                            legit = (j == nc - 1 && cn == 0) || (j == 0 && cn == nc - 1);
+                        } else {
+                            if (wall) g = 3;
+                            legit = (wall == 1 && j == 0) || (wall == 2 && j == nc - 1);
+                        }
+                        const bool good = valid && inr && (g < 3 || legit);
+                        if (!good) g = 3;
+                        const float v2 = __double2float_ru(VX_[r] * VX_[r] + VY_[r] * VY_[r] + VZ_[r] * VZ_[r]);
+                        vm2 = fmaxf(vm2, (valid && inr) ? v2 : 0.f);
+                        // cell of this slot for the border test: -1 before the tile, ncell behind it
+                        const int cle = valid ? (good ? cl : -1) : (i < pad ? -1 : ncell);
+                        W_[r] = g | ((cle + 1) << 2) | ((valid && !good) ? 256 : 0);
+                    }
+                }
+            }
+            // ---- sweep 1b: prefix counts per class (ballot/popc), samples at the cell borders -------------
             int runL = 0, runS = 0, runR = 0, lastcl = -1;
 #pragma unroll
             for (int r = 0; r < RMAX; ++r) {
                 if (r < nrows) {
                     const int i = (r << 5) + lane;
-                    const bool valid = i >= pad && i < pad + n;
-                    const int ic = min(max(i, pad), pad + n - 1);
-                    const double x = px[ic], vx = px[CAP + ic], vy = px[2 * CAP + ic], vz = px[3 * CAP + ic];
-                    double xs, jf;
-                    int j = cA;
-                    const bool dom = gather_cell(a.k, x, xs, jf, j);
-                    const int cl = j - cA;
-                    const bool inr = dom && cl >= 0 && cl < ncell;
-                    if (!inr) { j = cA; jf = (double)cA; }
-                    const double E0 = sE[j - ea], E1 = sE[j - ea + 1];
-                    PushOut o;
-                    push_core(a.k, x, vx, vy, vz, xs, jf, j, E0, E1, o);
-                    int b = 0;
-                    int g = fused_classify(a.k, j, o, b);
-                    const bool good = valid && inr && !b;
-                    if (valid && !good) bad |= FA_BAD_PARTICLE;
-                    if (!good) g = 3;
-                    if (valid && inr) vm2 = fmaxf(vm2, __double2float_ru(o.vx * o.vx + o.vy * o.vy + o.vz * o.vz));
-                    // cell of this slot for the border test: -1 before the tile, ncell behind it
-                    const int cle = valid ? (good ? cl : -1) : (i < pad ? -1 : ncell);
+                    const int w = W_[r];
+                    const int g = w & 3, cle = ((w >> 2) & 63) - 1;
+                    if (w & 256) bad |= FA_BAD_PARTICLE;
                     int prev = __shfl_up_sync(FULL, cle, 1);
                     if (lane == 0) prev = lastcl;
                     lastcl = __shfl_sync(FULL, cle, 31);
@@ -401,6 +464,7 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
                     if (cle > prev) {
                         // first slot of cell cle (cells prev+1 .. cle-1 are empty): sample the prefix counts and
                         // check the grouping against off_old
+#pragma unroll 1
                         for (int q = prev + 1; q <= cle; ++q) {
                             PS[q] = bL; PS[KP + q] = bS; PS[2 * KP + q] = bR;
                             if (offs[cA - Cm + q] - gbase != i) bad |= FA_BAD_PARTICLE;
@@ -408,8 +472,7 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
                     } else if (cle < prev) {
                         bad |= FA_BAD_PARTICLE;
                     }
-                    PK_[r] = g < 3 ? ((g == 0 ? bL : (g == 1 ? bS : bR)) << 8) | (g * 32 + cl) : -1;
-                    X_[r] = o.x; VX_[r] = o.vx; VY_[r] = o.vy; VZ_[r] = o.vz;
+                    W_[r] = g < 3 ? ((g == 0 ? bL : (g == 1 ? bS : bR)) << 8) | (g * 32 + cle) : -1;
                     runL += __popc(mL); runS += __popc(mS); runR += __popc(mR);
                 }
             }
@@ -479,18 +542,16 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
 #pragma unroll
                 for (int r = 0; r < RMAX; ++r) {
                     if (r < nrows) {
-                        const int pk = PK_[r];
+                        const int pk = W_[r];
                         const int key = pk & 0xff;
                         const bool has = pk >= 0;
                         const bool defer = has && key == kdef;
-                        long long p = 0;
-                        if (has) p = (long long)bas[key] + (pk >> 8);
-                        if (has && !defer) {
-                            if (p < 0 || p >= a.capacity) bad |= FA_BAD_PARTICLE;
-                            else {
-                                a.dx[p] = X_[r]; a.dvx[p] = VX_[r]; a.dvy[p] = VY_[r]; a.dvz[p] = VZ_[r];
-                                a.dcell[p] = cA + (key & 31) + (key >> 5) - 1;
-                            }
+                        const int p = has ? bas[key] + (pk >> 8) : 0;
+                        const bool inb = (unsigned)p < cap32;
+                        if (has && !inb) bad |= FA_BAD_PARTICLE;
+                        if (has && !defer && inb) {
+                            a.dx[p] = X_[r]; a.dvx[p] = VX_[r]; a.dvy[p] = VY_[r]; a.dvz[p] = VZ_[r];
+                            a.dcell[p] = cA - 1 + (key & 31) + (key >> 5);
                         }
                         const unsigned md = __ballot_sync(FULL, defer);
                         if (md) {
@@ -498,7 +559,7 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
                                 const int q = ndef + __popc(md & lt);
                                 if (q < FUSED_DEF) {
                                     qx[q] = X_[r]; qvx[q] = VX_[r]; qvy[q] = VY_[r]; qvz[q] = VZ_[r];
-                                    qpos[q] = (int)p;
+                                    qpos[q] = p;
                                 } else bad |= FA_DEFER_OVERFLOW;
                             }
                             ndef = min(ndef + __popc(md), FUSED_DEF);

@@ -331,9 +331,12 @@ static int create_species(pic_sim *sim, const pic_species_desc &d, pic_species *
     {
         static bool attr_set = false;
         if (!attr_set) {
-            CU(cudaFuncSetAttribute(fused_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-            CU(cudaFuncSetAttribute(fused_kernel<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-            CU(cudaFuncSetAttribute(fused_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+            CU(cudaFuncSetAttribute(fused_kernel<8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+            CU(cudaFuncSetAttribute(fused_kernel<12, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+            CU(cudaFuncSetAttribute(fused_kernel<16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+            CU(cudaFuncSetAttribute(fused_kernel<8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+            CU(cudaFuncSetAttribute(fused_kernel<12, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+            CU(cudaFuncSetAttribute(fused_kernel<16, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
             attr_set = true;
         }
     }
@@ -629,9 +632,10 @@ static int push_fused(pic_species *s)
         KernelSpan span(sim, K_FUSED);
         fused_edge_kernel<<<1, 128, 0, sim->stream>>>(a);
         if (int rc = launch_check(sim, "fused_edge_kernel")) return rc;
-        if (rows == 8) fused_kernel<8><<<grid, 32, smem, sim->stream>>>(a);
-        else if (rows == 12) fused_kernel<12><<<grid, 32, smem, sim->stream>>>(a);
-        else fused_kernel<16><<<grid, 32, smem, sim->stream>>>(a);
+        void (*kern)(FusedArgs) =
+            sim->periodic ? (rows == 8 ? fused_kernel<8, true> : rows == 12 ? fused_kernel<12, true> : fused_kernel<16, true>)
+                          : (rows == 8 ? fused_kernel<8, false> : rows == 12 ? fused_kernel<12, false> : fused_kernel<16, false>);
+        kern<<<grid, 32, smem, sim->stream>>>(a);
         if (int rc = launch_check(sim, "fused_kernel")) return rc;
     }
     // fallback chain, all guarded by run_split; it leaves the same host-visible state behind
