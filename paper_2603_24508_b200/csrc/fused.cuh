@@ -289,42 +289,115 @@ __device__ __forceinline__ void fused_issue(const FusedArgs &a, const FusedCtx &
     }
 }
 
-// One mover step of one particle given the weight w = xs - floor(xs) and the two node values of its
-// gather cell: the same sequence of rounded operations as push_core, written
-// without branches (the wrapped / unwrapped positions are both formed, one is selected).
-template <bool PERIODIC>
-__device__ __forceinline__ void push_flat(const PushConst &k, double x, double vx, double vy, double vz, double w, double E0,
-                                          double E1, double &xo, double &vxo, double &vyo, double &vzo, int &cn, int &wall)
+// Sweep 1a of fused_kernel for rows R0 .. R0+CNT-1 of a tile: push into registers and classify.  The
+// same sequence of rounded operations as push_core, written as straight-line
+// code without branches or warp collectives so that the rows' dependency chains interleave.  Slots
+// outside the tile (the alignment pad, the tail of the last row, rows behind it inside the group)
+// recompute a clamped slot and are masked out.
+// EDGE = the tile holds cell 0 or cell nc-1: only there can a particle wrap / be absorbed (class X), can
+// floor(x/dx) need the clamp of reading S8, or can x leave the gather range legitimately.  Elsewhere any
+// of that marks the particle bad (it moved more than one cell, or the grouping is broken).
+// W_[r] = class | (border cell + 1) << 2 | bad << 8, where the border cell is the local cell, 0 - 1 before
+// the tile / for a bad particle, ncell behind the tile.
+template <bool PERIODIC, bool EDGE, int RMAX, int R0, int CNT>
+__device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *px, const double *sEs, int lane, int pad, int n,
+                                              int cA, int ncell, double (&X_)[RMAX], double (&VX_)[RMAX], double (&VY_)[RMAX],
+                                              double (&VZ_)[RMAX], int (&W_)[RMAX], int &hmax)
 {
-    const double dE = __dsub_rn(E1, E0);
-    const double Ep = __dadd_rn(E0, __dmul_rn(w, dE));
-    const double hE = __dmul_rn(k.h, Ep);
-    const double ux = __dadd_rn(vx, hE), uy = vy, uz = vz;
-    const double px = __dadd_rn(ux, __dsub_rn(__dmul_rn(uy, k.tz), __dmul_rn(uz, k.ty)));
-    const double py = __dadd_rn(uy, __dsub_rn(__dmul_rn(uz, k.tx), __dmul_rn(ux, k.tz)));
-    const double pz = __dadd_rn(uz, __dsub_rn(__dmul_rn(ux, k.ty), __dmul_rn(uy, k.tx)));
-    const double wx = __dadd_rn(ux, __dsub_rn(__dmul_rn(py, k.sz), __dmul_rn(pz, k.sy)));
-    const double wy = __dadd_rn(uy, __dsub_rn(__dmul_rn(pz, k.sx), __dmul_rn(px, k.sz)));
-    const double wz = __dadd_rn(uz, __dsub_rn(__dmul_rn(px, k.sy), __dmul_rn(py, k.sx)));
-    const double nvx = __dadd_rn(wx, hE);
-    const double xn = __dadd_rn(x, __dmul_rn(nvx, k.dt));
-    double xw = xn;
-    wall = 0;
-    if (PERIODIC) {
-        const double xm = __dsub_rn(xn, k.L), xp = __dadd_rn(xn, k.L);
-        xw = xn >= k.L ? xm : (xn < 0.0 ? (xp >= k.L ? 0.0 : xp) : xn);
-    } else {
-        wall = xn < 0.0 ? 1 : (xn >= k.L ? 2 : 0);
+    constexpr int CAP = RMAX * 32;
+    const int nc = k.nc;
+#pragma unroll
+    for (int r = R0; r < R0 + CNT; ++r) {
+        const int i = (r << 5) + lane;
+        const bool valid = (unsigned)(i - pad) < (unsigned)n;
+        const int ic = min(max(i, pad), pad + n - 1);
+        const double x = px[ic], vx = px[CAP + ic], vy = px[2 * CAP + ic], vz = px[3 * CAP + ic];
+        const double xs = __dmul_rn(x, k.inv_dx);
+        double jf = floor(xs);
+        int jc = __double2int_rd(xs);
+        bool inr = true;
+        if (EDGE) {
+            inr = xs >= 0.0 && jc <= nc;
+            if (jc > nc - 1) { jc = nc - 1; jf = (double)(nc - 1); }
+        }
+        const int cl = jc - cA;
+        inr = inr && (unsigned)cl < (unsigned)ncell;
+        const int j = inr ? jc : cA;
+        const double E0 = sEs[j], E1 = sEs[j + 1];
+        const double w = __dsub_rn(xs, jf);
+        const double dE = __dsub_rn(E1, E0);
+        const double Ep = __dadd_rn(E0, __dmul_rn(w, dE));
+        const double hE = __dmul_rn(k.h, Ep);
+        const double ux = __dadd_rn(vx, hE), uy = vy, uz = vz;
+        const double qx = __dadd_rn(ux, __dsub_rn(__dmul_rn(uy, k.tz), __dmul_rn(uz, k.ty)));
+        const double qy = __dadd_rn(uy, __dsub_rn(__dmul_rn(uz, k.tx), __dmul_rn(ux, k.tz)));
+        const double qz = __dadd_rn(uz, __dsub_rn(__dmul_rn(ux, k.ty), __dmul_rn(uy, k.tx)));
+        const double wx = __dadd_rn(ux, __dsub_rn(__dmul_rn(qy, k.sz), __dmul_rn(qz, k.sy)));
+        const double wy = __dadd_rn(uy, __dsub_rn(__dmul_rn(qz, k.sx), __dmul_rn(qx, k.sz)));
+        const double wz = __dadd_rn(uz, __dsub_rn(__dmul_rn(qx, k.sy), __dmul_rn(qy, k.sx)));
+        const double nvx = __dadd_rn(wx, hE);
+        const double xn = __dadd_rn(x, __dmul_rn(nvx, k.dt));
+        double xw = xn;
+        bool out = false, legit = false;
+        int wall = 0;
+        if (EDGE) {
+            if (PERIODIC) {
+                const double xm = __dsub_rn(xn, k.L), xp = __dadd_rn(xn, k.L);
+                xw = xn >= k.L ? xm : (xn < 0.0 ? (xp >= k.L ? 0.0 : xp) : xn);
+            } else {
+                wall = xn < 0.0 ? 1 : (xn >= k.L ? 2 : 0);
+            }
+        } else {
+            out = xn < 0.0 || xn >= k.L;
+        }
+        const int cn = min(__double2int_rd(__dmul_rn(xw, k.inv_dx)), nc - 1);
+        const int d = cn - j;
+        int g = (unsigned)(d + 1) <= 2u ? d + 1 : 3;
+        if (EDGE) { // class X: out of cell 0 downwards / out of cell nc-1 upwards only
+            if (PERIODIC) {
+                legit = (j == nc - 1 && cn == 0) || (j == 0 && cn == nc - 1);
+            } else {
+                if (wall) g = 3;
+                legit = (wall == 1 && j == 0) || (wall == 2 && j == nc - 1);
+            }
+        } else if (out) {
+            g = 3;
+        }
+        const bool good = valid && inr && (g < 3 || legit);
+        if (!good) g = 3;
+        // speed bound for the split path's displacement estimate: largest high word of |v| components
+        const int hv = max(max(__double2hiint(nvx) & 0x7fffffff, __double2hiint(wy) & 0x7fffffff), __double2hiint(wz) & 0x7fffffff);
+        hmax = max(hmax, (valid && inr) ? hv : 0);
+        const int cle1 = i >= pad + n ? ncell + 1 : (good ? cl + 1 : 0);
+        W_[r] = g | (cle1 << 2) | ((valid && !good) ? 256 : 0);
+        X_[r] = xw; VX_[r] = nvx; VY_[r] = wy; VZ_[r] = wz;
     }
-    cn = min(__double2int_rd(__dmul_rn(xw, k.inv_dx)), k.nc - 1);
-    xo = xw; vxo = nvx; vyo = wy; vzo = wz;
+}
+
+// Row groups of sweep 1a: four rows at a time while at least four remain likely, then two, then single rows,
+// so that a tile of nrows rows pushes at most one surplus row.
+template <bool PERIODIC, bool EDGE, int RMAX>
+__device__ __forceinline__ void fused_sweep1a_all(const PushConst &k, const double *px, const double *sEs, int lane, int pad, int n,
+                                                  int nrows, int cA, int ncell, double (&X_)[RMAX], double (&VX_)[RMAX],
+                                                  double (&VY_)[RMAX], double (&VZ_)[RMAX], int (&W_)[RMAX], int &hmax)
+{
+#define FUSED_ROWS(R0, CNT) \
+    if (R0 < nrows) fused_sweep1a<PERIODIC, EDGE, RMAX, R0, CNT>(k, px, sEs, lane, pad, n, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
+    FUSED_ROWS(0, 4)
+    if (RMAX == 8) {
+        FUSED_ROWS(4, 2) FUSED_ROWS(6, 1) FUSED_ROWS(7, 1)
+    } else if (RMAX == 12) {
+        FUSED_ROWS(4, 4) FUSED_ROWS(8, 2) FUSED_ROWS(10, 1) FUSED_ROWS(11, 1)
+    } else {
+        FUSED_ROWS(4, 4) FUSED_ROWS(8, 4) FUSED_ROWS(12, 2) FUSED_ROWS(14, 1) FUSED_ROWS(15, 1)
+    }
+#undef FUSED_ROWS
 }
 
 template <int RMAX, bool PERIODIC>
 __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
 {
-    constexpr int GS = 4; // rows pushed together in sweep 1a
-    static_assert(RMAX % GS == 0, "RMAX must be a multiple of the row group");
+    static_assert(RMAX == 8 || RMAX == 12 || RMAX == 16, "row groups of sweep 1a are written for these sizes");
     extern __shared__ __align__(128) unsigned char fused_smem[];
     constexpr int CAP = RMAX * 32;
     constexpr int KP = FUSED_KMAX + 2; // row stride of the prefix samples
@@ -343,7 +416,7 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
     const int nc = a.k.nc;
     int bad = 0; // FA_* bits
     int mc = 0;  // largest new per-cell count seen by this lane
-    float vm2 = 0.f;
+    int hmax = 0; // largest high word of the |v'| components seen by this lane
 
     if (!*(volatile int *)&st->abort) {
         FusedCtx X;
@@ -357,7 +430,6 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
         for (int idx = lane; idx <= Cp - Cm; idx += 32) offs[idx] = a.off_old[Cm + idx];
         const int ea = Cm & ~1;
         const double *sEs = sE - ea; // E node j of the chunk's window sits at sEs[j]
-        const double dncm1 = (double)(nc - 1);
         const unsigned cap32 = (unsigned)a.capacity;
         if (lane == 0) {
             asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(mb0) : "memory");
@@ -401,58 +473,18 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
                 else        { mbar_wait(mb0, ph0); ph0 ^= 1u; }
             }
 
-            // ---- sweep 1a: push into registers and classify.  Straight-line code, GS rows at a time, no warp
-            // collectives and no branches inside a group, so the rows' dependency chains interleave.
-            // Slots outside the tile (the alignment pad, the tail of the last row, rows behind it inside a
-            // group) recompute a clamped slot and are masked out.
+            // ---- sweep 1a: push into registers and classify (fused_sweep1a) ----------------------------------
             double X_[RMAX], VX_[RMAX], VY_[RMAX], VZ_[RMAX];
             int W_[RMAX]; // 1a: class | (border cell + 1) << 2 | bad << 8;  1b: -1, or prefix count << 8 | class*32 + cell
-#pragma unroll
-            for (int r0 = 0; r0 < RMAX; r0 += GS) {
-                if (r0 < nrows) {
-#pragma unroll
-                    for (int r = r0; r < r0 + GS; ++r) {
-                        const int i = (r << 5) + lane;
-                        const bool valid = (unsigned)(i - pad) < (unsigned)n;
-                        const int ic = min(max(i, pad), pad + n - 1);
-                        const double x = px[ic], vx = px[CAP + ic], vy = px[2 * CAP + ic], vz = px[3 * CAP + ic];
-                        const double xs = __dmul_rn(x, a.k.inv_dx);
-                        double jf = floor(xs);
-                        const int j0 = __double2int_rd(xs);
-                        const bool dom = xs >= 0.0 && j0 <= nc;
-                        if (j0 > nc - 1) jf = dncm1;
-                        const int jc = min(j0, nc - 1);
-                        const int cl = jc - cA;
-                        const bool inr = dom && (unsigned)cl < (unsigned)ncell;
-                        const int j = inr ? jc : cA;
-                        const double E0 = sEs[j], E1 = sEs[j + 1];
-                        int cn, wall;
-                        push_flat<PERIODIC>(a.k, x, vx, vy, vz, __dsub_rn(xs, jf), E0, E1, X_[r], VX_[r], VY_[r], VZ_[r], cn, wall);
-                        const int d = cn - j;
-                        int g = (unsigned)(d + 1) <= 2u ? d + 1 : 3;
-                        bool legit; // class X: out of cell 0 downwards / out of cell nc-1 upwards only
-                        if (PERIODIC) {
-                            legit = (j == nc - 1 && cn == 0) || (j == 0 && cn == nc - 1);
-                        } else {
-                            if (wall) g = 3;
-                            legit = (wall == 1 && j == 0) || (wall == 2 && j == nc - 1);
-                        }
-                        const bool good = valid && inr && (g < 3 || legit);
-                        if (!good) g = 3;
-                        const float v2 = __double2float_ru(VX_[r] * VX_[r] + VY_[r] * VY_[r] + VZ_[r] * VZ_[r]);
-                        vm2 = fmaxf(vm2, (valid && inr) ? v2 : 0.f);
-                        // cell of this slot for the border test: -1 before the tile, ncell behind it
-                        const int cle = valid ? (good ? cl : -1) : (i < pad ? -1 : ncell);
-                        W_[r] = g | ((cle + 1) << 2) | ((valid && !good) ? 256 : 0);
-                    }
-                }
-            }
+            if (cA == 0 || cB == nc) fused_sweep1a_all<PERIODIC, true, RMAX>(a.k, px, sEs, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
+            else fused_sweep1a_all<PERIODIC, false, RMAX>(a.k, px, sEs, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
+
             // ---- sweep 1b: prefix counts per class (ballot/popc), samples at the cell borders -------------
-            int runL = 0, runS = 0, runR = 0, lastcl = -1;
+            unsigned run = 0; // running class counts of the tile: L | S << 10 | R << 20
+            int lastcl = -1;
 #pragma unroll
             for (int r = 0; r < RMAX; ++r) {
                 if (r < nrows) {
-                    const int i = (r << 5) + lane;
                     const int w = W_[r];
                     const int g = w & 3, cle = ((w >> 2) & 63) - 1;
                     if (w & 256) bad |= FA_BAD_PARTICLE;
@@ -460,22 +492,29 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
                     if (lane == 0) prev = lastcl;
                     lastcl = __shfl_sync(FULL, cle, 31);
                     const unsigned mL = __ballot_sync(FULL, g == 0), mS = __ballot_sync(FULL, g == 1), mR = __ballot_sync(FULL, g == 2);
-                    const int bL = runL + __popc(mL & lt), bS = runS + __popc(mS & lt), bR = runR + __popc(mR & lt);
-                    if (cle > prev) {
-                        // first slot of cell cle (cells prev+1 .. cle-1 are empty): sample the prefix counts and
-                        // check the grouping against off_old
+                    if (cle != prev) {
+                        if (cle > prev) {
+                            // first slot of cell cle (cells prev+1 .. cle-1 are empty): sample the prefix counts and
+                            // check the grouping against off_old
+                            const int i = (r << 5) + lane;
+                            const int bL = (int)(run & 1023u) + __popc(mL & lt), bS = (int)((run >> 10) & 1023u) + __popc(mS & lt),
+                                      bR = (int)(run >> 20) + __popc(mR & lt);
 #pragma unroll 1
-                        for (int q = prev + 1; q <= cle; ++q) {
-                            PS[q] = bL; PS[KP + q] = bS; PS[2 * KP + q] = bR;
-                            if (offs[cA - Cm + q] - gbase != i) bad |= FA_BAD_PARTICLE;
+                            for (int q = prev + 1; q <= cle; ++q) {
+                                PS[q] = bL; PS[KP + q] = bS; PS[2 * KP + q] = bR;
+                                if (offs[cA - Cm + q] - gbase != i) bad |= FA_BAD_PARTICLE;
+                            }
+                        } else {
+                            bad |= FA_BAD_PARTICLE;
                         }
-                    } else if (cle < prev) {
-                        bad |= FA_BAD_PARTICLE;
                     }
-                    W_[r] = g < 3 ? ((g == 0 ? bL : (g == 1 ? bS : bR)) << 8) | (g * 32 + cle) : -1;
-                    runL += __popc(mL); runS += __popc(mS); runR += __popc(mR);
+                    const unsigned mo = g == 0 ? mL : (g == 1 ? mS : mR);
+                    const int mine = (int)((run >> (10 * g)) & 1023u) + __popc(mo & lt);
+                    W_[r] = g < 3 ? (mine << 8) | (g * 32 + cle) : -1;
+                    run += (unsigned)__popc(mL) | ((unsigned)__popc(mS) << 10) | ((unsigned)__popc(mR) << 20);
                 }
             }
+            const int runL = (int)(run & 1023u), runS = (int)((run >> 10) & 1023u), runR = (int)(run >> 20);
             if (kind != FK_VIRTUAL) {
                 for (int q = lastcl + 1 + lane; q <= ncell; q += 32) {
                     PS[q] = runL; PS[KP + q] = runS; PS[2 * KP + q] = runR;
@@ -586,7 +625,10 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
     // ---- CTA epilogue; the last CTA commits or rolls back the step ----------------------------------
     bad = (int)__reduce_or_sync(FULL, (unsigned)bad);
     mc = __reduce_max_sync(FULL, mc);
-    const unsigned vmw = __reduce_max_sync(FULL, __float_as_uint(vm2));
+    // |v'|^2 <= 3 b^2 with b the smallest double whose high word exceeds every component's
+    hmax = __reduce_max_sync(FULL, hmax);
+    const double vb = __hiloint2double(hmax + 1, 0);
+    const unsigned vmw = hmax ? __float_as_uint(__double2float_ru(3.0 * vb * vb)) : 0u;
     if (lane == 0) {
         if (bad) {
             atomicExch(&st->abort, 1);
