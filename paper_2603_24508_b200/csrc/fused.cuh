@@ -35,6 +35,7 @@ namespace pic {
 constexpr int FUSED_MIN_NC = 16;
 constexpr int FUSED_CPC_DEFAULT = 64;  // cells per chunk (per CTA)
 constexpr int FUSED_CPC_MAX = 256;
+constexpr int FUSED_STAGES_DEFAULT = 1;    // stages of the shared-memory ring (1: more CTAs per SM; measured faster than 2)
 constexpr int FUSED_KMAX = 32;         // cells per tile (one lane per cell)
 constexpr int FUSED_DEF = 32;          // deferred right-movers of a tile's last cell
 constexpr int FUSED_XCAP = 256;        // edge kernel: leavers per edge cell
@@ -56,19 +57,21 @@ struct FusedArgs {
     PushConst k;
     long long capacity; // slots allocated in every particle array
     int CPC;
+    int SCAP; // slots per shared-memory stage (<= RMAX*32, even)
+    int NST;  // stages of the ring: 1 or 2
 };
 
-// Dynamic shared memory of one fused_kernel CTA (one warp); CAP = RMAX*32 slots per stage.
+// Dynamic shared memory of one fused_kernel CTA (one warp): NST stages of SCAP slots.
 struct FusedLayout {
     int stage_bytes; // x, vx, vy, vz [CAP]
     int off_E, off_offs, off_ps, off_base, off_q, off_mbar, total;
 };
 
-__host__ __device__ inline FusedLayout fused_layout(int CAP, int CPC)
+__host__ __device__ inline FusedLayout fused_layout(int SCAP, int CPC, int NST)
 {
     FusedLayout L;
-    L.stage_bytes = 32 * CAP;
-    int o = 2 * L.stage_bytes;
+    L.stage_bytes = 32 * SCAP;
+    int o = NST * L.stage_bytes;
     L.off_E = o;    o += 8 * (CPC + 6);
     L.off_offs = o; o += 4 * (CPC + 4);
     L.off_ps = o;   o += 4 * 3 * (FUSED_KMAX + 2);
@@ -300,18 +303,17 @@ __device__ __forceinline__ void fused_issue(const FusedArgs &a, const FusedCtx &
 // W_[r] = class | (border cell + 1) << 2 | bad << 8, where the border cell is the local cell, 0 - 1 before
 // the tile / for a bad particle, ncell behind the tile.
 template <bool PERIODIC, bool EDGE, int RMAX, int R0, int CNT>
-__device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *px, const double *sEs, int lane, int pad, int n,
+__device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *px, int scap, const double *sEs, int lane, int pad, int n,
                                               int cA, int ncell, double (&X_)[RMAX], double (&VX_)[RMAX], double (&VY_)[RMAX],
                                               double (&VZ_)[RMAX], int (&W_)[RMAX], int &hmax)
 {
-    constexpr int CAP = RMAX * 32;
     const int nc = k.nc;
 #pragma unroll
     for (int r = R0; r < R0 + CNT; ++r) {
         const int i = (r << 5) + lane;
         const bool valid = (unsigned)(i - pad) < (unsigned)n;
         const int ic = min(max(i, pad), pad + n - 1);
-        const double x = px[ic], vx = px[CAP + ic], vy = px[2 * CAP + ic], vz = px[3 * CAP + ic];
+        const double x = px[ic], vx = px[scap + ic], vy = px[2 * scap + ic], vz = px[3 * scap + ic];
         const double xs = __dmul_rn(x, k.inv_dx);
         double jf = floor(xs);
         int jc = __double2int_rd(xs);
@@ -377,12 +379,12 @@ __device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *
 // Row groups of sweep 1a: four rows at a time while at least four remain likely, then two, then single rows,
 // so that a tile of nrows rows pushes at most one surplus row.
 template <bool PERIODIC, bool EDGE, int RMAX>
-__device__ __forceinline__ void fused_sweep1a_all(const PushConst &k, const double *px, const double *sEs, int lane, int pad, int n,
+__device__ __forceinline__ void fused_sweep1a_all(const PushConst &k, const double *px, int scap, const double *sEs, int lane, int pad, int n,
                                                   int nrows, int cA, int ncell, double (&X_)[RMAX], double (&VX_)[RMAX],
                                                   double (&VY_)[RMAX], double (&VZ_)[RMAX], int (&W_)[RMAX], int &hmax)
 {
 #define FUSED_ROWS(R0, CNT) \
-    if (R0 < nrows) fused_sweep1a<PERIODIC, EDGE, RMAX, R0, CNT>(k, px, sEs, lane, pad, n, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
+    if (R0 < nrows) fused_sweep1a<PERIODIC, EDGE, RMAX, R0, CNT>(k, px, scap, sEs, lane, pad, n, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
     FUSED_ROWS(0, 4)
     if (RMAX == 8) {
         FUSED_ROWS(4, 2) FUSED_ROWS(6, 1) FUSED_ROWS(7, 1)
@@ -399,9 +401,8 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
 {
     static_assert(RMAX == 8 || RMAX == 12 || RMAX == 16, "row groups of sweep 1a are written for these sizes");
     extern __shared__ __align__(128) unsigned char fused_smem[];
-    constexpr int CAP = RMAX * 32;
     constexpr int KP = FUSED_KMAX + 2; // row stride of the prefix samples
-    const FusedLayout L = fused_layout(CAP, a.CPC);
+    const FusedLayout L = fused_layout(a.SCAP, a.CPC, a.NST);
     double *sE = reinterpret_cast<double *>(fused_smem + L.off_E);
     int *offs = reinterpret_cast<int *>(fused_smem + L.off_offs);
     int *PS = reinterpret_cast<int *>(fused_smem + L.off_ps);   // PS[class][cl] = class prefix count at the start of cell cl
@@ -424,7 +425,7 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
         X.C1 = min(X.C0 + a.CPC, nc);
         X.Cm = max(X.C0 - 1, 0);
         X.nc = nc;
-        X.CAP = CAP;
+        X.CAP = a.SCAP;
         X.offs = offs;
         const int Cm = X.Cm, Cp = min(X.C1 + 1, nc);
         for (int idx = lane; idx <= Cp - Cm; idx += 32) offs[idx] = a.off_old[Cm + idx];
@@ -446,10 +447,11 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
         int phase = 0, cur = 0;
         FusedItem I0 = fused_next_item(X, phase, cur, lane, bad);
         FusedItem I1 = fused_next_item(X, phase, cur, lane, bad);
+        const bool two = a.NST == 2;
         double *stage0 = reinterpret_cast<double *>(fused_smem), *stage1 = reinterpret_cast<double *>(fused_smem + L.stage_bytes);
         if (lane == 0) {
             fused_issue(a, X, I0, stage0, mb0);
-            fused_issue(a, X, I1, stage1, mb1);
+            if (two) fused_issue(a, X, I1, stage1, mb1);
         }
         // carry across tiles: class counts of the previous tile's last cell
         int pvL = 0, pvS = 0, pvR = 0;
@@ -467,17 +469,18 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
             const int n = kind == FK_VIRTUAL ? 0 : offs[cB - Cm] - sA;
             const int pad = sA & 1, gbase = sA - pad;
             const int nrows = n > 0 ? (pad + n + 31) >> 5 : 0;
-            double *px = (it & 1) ? stage1 : stage0;
+            const bool odd = two && (it & 1);
+            double *px = odd ? stage1 : stage0;
             if (n > 0) {
-                if (it & 1) { mbar_wait(mb1, ph1); ph1 ^= 1u; }
+                if (odd) { mbar_wait(mb1, ph1); ph1 ^= 1u; }
                 else        { mbar_wait(mb0, ph0); ph0 ^= 1u; }
             }
 
             // ---- sweep 1a: push into registers and classify (fused_sweep1a) ----------------------------------
             double X_[RMAX], VX_[RMAX], VY_[RMAX], VZ_[RMAX];
             int W_[RMAX]; // 1a: class | (border cell + 1) << 2 | bad << 8;  1b: -1, or prefix count << 8 | class*32 + cell
-            if (cA == 0 || cB == nc) fused_sweep1a_all<PERIODIC, true, RMAX>(a.k, px, sEs, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
-            else fused_sweep1a_all<PERIODIC, false, RMAX>(a.k, px, sEs, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
+            if (cA == 0 || cB == nc) fused_sweep1a_all<PERIODIC, true, RMAX>(a.k, px, a.SCAP, sEs, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
+            else fused_sweep1a_all<PERIODIC, false, RMAX>(a.k, px, a.SCAP, sEs, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
 
             // ---- sweep 1b: prefix counts per class (ballot/popc), samples at the cell borders -------------
             unsigned run = 0; // running class counts of the tile: L | S << 10 | R << 20
@@ -523,7 +526,7 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
             }
             __syncwarp();
             // the stage has been read: refill it with the item after next
-            if (lane == 0) fused_issue(a, X, I2, px, (it & 1) ? mb1 : mb0);
+            if (lane == 0) fused_issue(a, X, two ? I2 : I1, px, odd ? mb1 : mb0);
 
             // ---- per-cell phase (lane = local cell) -------------------------------------------------
             int Lc = 0, Sc = 0, Rc = 0, psL = 0, psS = 0, psR = 0;

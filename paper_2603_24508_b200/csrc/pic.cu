@@ -78,7 +78,7 @@ struct pic_sim {
     std::vector<pic_species *> sp;
     unsigned long long launches = 0;
     int opt_e_stage = 1, opt_fused = 1, opt_timing = 0;
-    int opt_fused_cpc = 0, opt_fused_rows = 0; // tuning knobs of the fused step (0 = automatic)
+    int opt_fused_cpc = 0, opt_fused_rows = 0, opt_fused_slots = 0, opt_fused_stages = 0; // tuning knobs of the fused step (0 = automatic)
     int sm_count = 148;
     // per-kernel device timing (option "kernel_timing"): event pairs recorded around launches
     struct Span { int id; cudaEvent_t a, b; };
@@ -425,6 +425,8 @@ extern "C" int pic_set_option(pic_sim *sim, const char *key, int value)
     else if (!strcmp(key, "kernel_timing") && flag) sim->opt_timing = value;
     else if (!strcmp(key, "fused") && flag) sim->opt_fused = value;
     else if (!strcmp(key, "fused_cells_per_cta") && value >= 0 && value <= FUSED_CPC_MAX) sim->opt_fused_cpc = value;
+    else if (!strcmp(key, "fused_stage_slots") && value >= 0 && value <= 512 && value % 2 == 0) sim->opt_fused_slots = value;
+    else if (!strcmp(key, "fused_stages") && value >= 0 && value <= 2) sim->opt_fused_stages = value;
     else if (!strcmp(key, "fused_rows") && (value == 0 || value == 8 || value == 12 || value == 16)) sim->opt_fused_rows = value;
     else return PIC_EINVAL;
     return PIC_OK;
@@ -594,18 +596,33 @@ static int fused_cells_per_cta(const pic_species *s)
     return (int)std::max<long long>(8, std::min<long long>(FUSED_CPC_DEFAULT, want));
 }
 
-static int fused_rows(const pic_species *s, int *ctas_per_sm)
+struct FusedGeom { int rows, slots, stages, cpc, ctas_per_sm; size_t smem; };
+
+// Launch geometry of the fused step for this species' current state; rows == 0 when a cell may not fit
+// a tile.  A tile must hold at least one cell; maxcount is the bound read at the last sync, so leave room
+// for it to grow.
+static FusedGeom fused_geom(const pic_species *s)
 {
     const pic_sim *sim = s->sim;
-    int rows = sim->opt_fused_rows;
-    if (rows == 0) {
-        const int mc = std::max(s->h_maxcount, 1);
-        const int need = mc + std::max(mc / 4, 32) + 2;
-        rows = need <= 8 * 32 ? 8 : need <= 12 * 32 ? 12 : need <= 16 * 32 ? 16 : 0;
-    }
-    if (rows && ctas_per_sm)
-        *ctas_per_sm = std::max(1, std::min(32, FUSED_SMEM_SM / (fused_layout(rows * 32, fused_cells_per_cta(s)).total + 1024)));
-    return rows;
+    FusedGeom g{};
+    const int mc = std::max(s->h_maxcount, 1);
+    const int need = mc + std::max(mc / 4, 32) + 2;
+    g.rows = sim->opt_fused_rows;
+    if (g.rows == 0) g.rows = need <= 8 * 32 ? 8 : need <= 12 * 32 ? 12 : need <= 16 * 32 ? 16 : 0;
+    if (g.rows == 0) return g;
+    g.cpc = fused_cells_per_cta(s);
+    g.stages = sim->opt_fused_stages ? sim->opt_fused_stages : FUSED_STAGES_DEFAULT;
+    g.slots = sim->opt_fused_slots ? std::min(sim->opt_fused_slots, g.rows * 32) : g.rows * 32;
+    g.smem = (size_t)fused_layout(g.slots, g.cpc, g.stages).total;
+    g.ctas_per_sm = std::max(1, std::min(32, FUSED_SMEM_SM / ((int)g.smem + 1024)));
+    return g;
+}
+
+static int fused_rows(const pic_species *s, int *ctas_per_sm)
+{
+    const FusedGeom g = fused_geom(s);
+    if (g.rows && ctas_per_sm) *ctas_per_sm = g.ctas_per_sm;
+    return g.rows;
 }
 
 // One fused push+arrange step, followed by the guarded split chain that redoes the step if the
@@ -624,10 +641,13 @@ static int push_fused(pic_species *s)
     a.st = s->d_st;
     a.k = s->k;
     a.capacity = s->capacity;
-    a.CPC = fused_cells_per_cta(s);
-    const int rows = fused_rows(s, nullptr);
+    const FusedGeom geo = fused_geom(s);
+    a.CPC = geo.cpc;
+    a.SCAP = geo.slots;
+    a.NST = geo.stages;
+    const int rows = geo.rows;
     const int grid = (sim->nc + a.CPC - 1) / a.CPC;
-    const size_t smem = (size_t)fused_layout(rows * 32, a.CPC).total;
+    const size_t smem = geo.smem;
     {
         KernelSpan span(sim, K_FUSED);
         fused_edge_kernel<<<1, 128, 0, sim->stream>>>(a);
@@ -754,7 +774,7 @@ extern "C" int pic_fused_info(pic_species *s, int32_t *active, int32_t *decline_
     if (active) *active = fused_possible(s) ? 1 : 0;
     if (decline_reasons) *decline_reasons = h.abort_reason;
     int ctas = 0;
-    const int cap = 32 * fused_rows(s, &ctas);
+    const int cap = fused_rows(s, &ctas) ? fused_geom(s).slots : 0;
     if (stage_slots) *stage_slots = cap;
     if (ctas_per_sm) *ctas_per_sm = ctas;
     return PIC_OK;
