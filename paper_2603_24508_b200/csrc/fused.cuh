@@ -36,7 +36,7 @@ constexpr int FUSED_MIN_NC = 16;
 constexpr int FUSED_CPC_DEFAULT = 64;  // cells per chunk (per CTA)
 constexpr int FUSED_CPC_MAX = 256;
 constexpr int FUSED_STAGES_DEFAULT = 1;    // stages of the shared-memory ring (1: more CTAs per SM; measured faster than 2)
-constexpr int FUSED_KMAX = 32;         // cells per tile (one lane per cell)
+constexpr int FUSED_KMAX = 31;         // cells per tile (one lane per cell border)
 constexpr int FUSED_DEF = 32;          // deferred right-movers of a tile's last cell
 constexpr int FUSED_XCAP = 256;        // edge kernel: leavers per edge cell
 constexpr int FUSED_SMEM_SM = 233472;  // shared memory per SM (228 KB), 1 KB reserved per CTA
@@ -57,26 +57,27 @@ struct FusedArgs {
     PushConst k;
     long long capacity; // slots allocated in every particle array
     int CPC;
-    int SCAP; // slots per shared-memory stage (<= RMAX*32, even)
+    int SCAP; // largest tile, in slots (<= RMAX*32, even)
     int NST;  // stages of the ring: 1 or 2
 };
 
-// Dynamic shared memory of one fused_kernel CTA (one warp): NST stages of SCAP slots.
+// Dynamic shared memory of one fused_kernel CTA (one warp): NST stages of CAP = RMAX*32 slots.
 struct FusedLayout {
     int stage_bytes; // x, vx, vy, vz [CAP]
-    int off_E, off_offs, off_ps, off_base, off_q, off_mbar, total;
+    int off_E, off_offs, off_cell, off_row, off_base, off_q, off_mbar, total;
 };
 
-__host__ __device__ inline FusedLayout fused_layout(int SCAP, int CPC, int NST)
+__host__ __device__ inline FusedLayout fused_layout(int CAP, int CPC, int NST)
 {
     FusedLayout L;
-    L.stage_bytes = 32 * SCAP;
+    L.stage_bytes = 32 * CAP;
     int o = NST * L.stage_bytes;
     L.off_E = o;    o += 8 * (CPC + 6);
     L.off_offs = o; o += 4 * (CPC + 4);
-    L.off_ps = o;   o += 4 * 3 * (FUSED_KMAX + 2);
-    L.off_base = o; o += 4 * 3 * FUSED_KMAX;
     o = (o + 15) & ~15;
+    L.off_cell = o; o += 8 * (FUSED_KMAX + 1); // {first slot, count} of the tile's cells
+    L.off_row = o;  o += 16 * 16;              // per row: the three class ballots and the running counts before it
+    L.off_base = o; o += 8 * 3 * 32;           // per (class, cell): {slot base, destination cell}
     L.off_q = o;    o += FUSED_DEF * 40;
     L.off_mbar = o; o += 32;
     L.total = o;
@@ -221,7 +222,9 @@ struct FusedItem {
 };
 
 struct FusedCtx { // uniform per CTA
-    int C0, C1, Cm, nc, CAP;
+    int C0, C1, Cm, nc;
+    int CAP; // largest tile, in slots
+    int STR; // slots between the x, vx, vy, vz arrays of a stage
     const int *offs; // offs[c - Cm] = off_old[c] for the chunk's cells and one halo cell on each side
 };
 
@@ -232,7 +235,7 @@ __device__ __forceinline__ int fused_slots(const FusedCtx &X, int a, int b)
 }
 
 // The chunk's work items in order: [halo cell C0-1] tiles of whole cells (greedy: as many cells as
-// fit CAP slots, at most 32) ... [halo cell C1 | virtual end of the grid].
+// fit CAP slots, at most 31) ... [halo cell C1 | virtual end of the grid].
 __device__ __forceinline__ FusedItem fused_next_item(const FusedCtx &X, int &phase, int &cur, int lane, int &bad)
 {
     FusedItem I{0, 0, FK_NONE};
@@ -244,7 +247,7 @@ __device__ __forceinline__ FusedItem fused_next_item(const FusedCtx &X, int &pha
     if (I.kind == FK_NONE && phase == 1) {
         if (cur < X.C1) {
             const int b = cur + 1 + lane;
-            const bool fits = b <= X.C1 && fused_slots(X, cur, b) <= X.CAP;
+            const bool fits = lane < FUSED_KMAX && b <= X.C1 && fused_slots(X, cur, b) <= X.CAP;
             const int nb = __popc(__ballot_sync(FULL, fits)); // fits holds for a prefix of the lanes
             if (nb == 0) {
                 bad |= FA_TILE_OVERFLOW;
@@ -281,14 +284,14 @@ __device__ __forceinline__ void fused_issue(const FusedArgs &a, const FusedCtx &
     if (cnt > 0) {
         const unsigned bytes = 8u * (unsigned)cnt;
         bulk_g2s(stage, a.sx + g0, bytes, mb);
-        bulk_g2s(stage + X.CAP, a.svx + g0, bytes, mb);
-        bulk_g2s(stage + 2 * X.CAP, a.svy + g0, bytes, mb);
-        bulk_g2s(stage + 3 * X.CAP, a.svz + g0, bytes, mb);
+        bulk_g2s(stage + X.STR, a.svx + g0, bytes, mb);
+        bulk_g2s(stage + 2 * X.STR, a.svy + g0, bytes, mb);
+        bulk_g2s(stage + 3 * X.STR, a.svz + g0, bytes, mb);
     }
     if (tail) {
         const int li = pad + n - 1;
         const long long gi = (long long)sA + n - 1;
-        stage[li] = a.sx[gi]; stage[X.CAP + li] = a.svx[gi]; stage[2 * X.CAP + li] = a.svy[gi]; stage[3 * X.CAP + li] = a.svz[gi];
+        stage[li] = a.sx[gi]; stage[X.STR + li] = a.svx[gi]; stage[2 * X.STR + li] = a.svy[gi]; stage[3 * X.STR + li] = a.svz[gi];
     }
 }
 
@@ -300,20 +303,21 @@ __device__ __forceinline__ void fused_issue(const FusedArgs &a, const FusedCtx &
 // EDGE = the tile holds cell 0 or cell nc-1: only there can a particle wrap / be absorbed (class X), can
 // floor(x/dx) need the clamp of reading S8, or can x leave the gather range legitimately.  Elsewhere any
 // of that marks the particle bad (it moved more than one cell, or the grouping is broken).
-// W_[r] = class | (border cell + 1) << 2 | bad << 8, where the border cell is the local cell, 0 - 1 before
-// the tile / for a bad particle, ncell behind the tile.
+// cellinfo[cl] = {first slot, count} of the tile's cells from off_old: a slot outside its cell's range
+// means the grouping is broken.  W_[r] = class | local cell << 2 | bad << 8.
 template <bool PERIODIC, bool EDGE, int RMAX, int R0, int CNT>
-__device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *px, int scap, const double *sEs, int lane, int pad, int n,
-                                              int cA, int ncell, double (&X_)[RMAX], double (&VX_)[RMAX], double (&VY_)[RMAX],
-                                              double (&VZ_)[RMAX], int (&W_)[RMAX], int &hmax)
+__device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *px, const double *sEs, const int2 *cellinfo, int lane,
+                                              int pad, int n, int cA, int ncell, double (&X_)[RMAX], double (&VX_)[RMAX],
+                                              double (&VY_)[RMAX], double (&VZ_)[RMAX], int (&W_)[RMAX], int &hmax)
 {
+    constexpr int CAP = RMAX * 32;
     const int nc = k.nc;
 #pragma unroll
     for (int r = R0; r < R0 + CNT; ++r) {
         const int i = (r << 5) + lane;
         const bool valid = (unsigned)(i - pad) < (unsigned)n;
         const int ic = min(max(i, pad), pad + n - 1);
-        const double x = px[ic], vx = px[scap + ic], vy = px[2 * scap + ic], vz = px[3 * scap + ic];
+        const double x = px[ic], vx = px[CAP + ic], vy = px[2 * CAP + ic], vz = px[3 * CAP + ic];
         const double xs = __dmul_rn(x, k.inv_dx);
         double jf = floor(xs);
         int jc = __double2int_rd(xs);
@@ -325,6 +329,8 @@ __device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *
         const int cl = jc - cA;
         inr = inr && (unsigned)cl < (unsigned)ncell;
         const int j = inr ? jc : cA;
+        const int2 sc = cellinfo[j - cA];
+        const bool inside = (unsigned)(i - sc.x) < (unsigned)sc.y;
         const double E0 = sEs[j], E1 = sEs[j + 1];
         const double w = __dsub_rn(xs, jf);
         const double dE = __dsub_rn(E1, E0);
@@ -365,13 +371,12 @@ __device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *
         } else if (out) {
             g = 3;
         }
-        const bool good = valid && inr && (g < 3 || legit);
+        const bool good = valid && inr && inside && (g < 3 || legit);
         if (!good) g = 3;
         // speed bound for the split path's displacement estimate: largest high word of |v| components
         const int hv = max(max(__double2hiint(nvx) & 0x7fffffff, __double2hiint(wy) & 0x7fffffff), __double2hiint(wz) & 0x7fffffff);
         hmax = max(hmax, (valid && inr) ? hv : 0);
-        const int cle1 = i >= pad + n ? ncell + 1 : (good ? cl + 1 : 0);
-        W_[r] = g | (cle1 << 2) | ((valid && !good) ? 256 : 0);
+        W_[r] = g | ((j - cA) << 2) | ((valid && !good) ? 256 : 0);
         X_[r] = xw; VX_[r] = nvx; VY_[r] = wy; VZ_[r] = wz;
     }
 }
@@ -379,12 +384,12 @@ __device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *
 // Row groups of sweep 1a: four rows at a time while at least four remain likely, then two, then single rows,
 // so that a tile of nrows rows pushes at most one surplus row.
 template <bool PERIODIC, bool EDGE, int RMAX>
-__device__ __forceinline__ void fused_sweep1a_all(const PushConst &k, const double *px, int scap, const double *sEs, int lane, int pad, int n,
-                                                  int nrows, int cA, int ncell, double (&X_)[RMAX], double (&VX_)[RMAX],
+__device__ __forceinline__ void fused_sweep1a_all(const PushConst &k, const double *px, const double *sEs, const int2 *cellinfo, int lane,
+                                                  int pad, int n, int nrows, int cA, int ncell, double (&X_)[RMAX], double (&VX_)[RMAX],
                                                   double (&VY_)[RMAX], double (&VZ_)[RMAX], int (&W_)[RMAX], int &hmax)
 {
 #define FUSED_ROWS(R0, CNT) \
-    if (R0 < nrows) fused_sweep1a<PERIODIC, EDGE, RMAX, R0, CNT>(k, px, scap, sEs, lane, pad, n, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
+    if (R0 < nrows) fused_sweep1a<PERIODIC, EDGE, RMAX, R0, CNT>(k, px, sEs, cellinfo, lane, pad, n, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
     FUSED_ROWS(0, 4)
     if (RMAX == 8) {
         FUSED_ROWS(4, 2) FUSED_ROWS(6, 1) FUSED_ROWS(7, 1)
@@ -397,16 +402,17 @@ __device__ __forceinline__ void fused_sweep1a_all(const PushConst &k, const doub
 }
 
 template <int RMAX, bool PERIODIC>
-__global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
+__global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fused_kernel(FusedArgs a)
 {
     static_assert(RMAX == 8 || RMAX == 12 || RMAX == 16, "row groups of sweep 1a are written for these sizes");
     extern __shared__ __align__(128) unsigned char fused_smem[];
-    constexpr int KP = FUSED_KMAX + 2; // row stride of the prefix samples
-    const FusedLayout L = fused_layout(a.SCAP, a.CPC, a.NST);
+    constexpr int CAP = RMAX * 32;
+    const FusedLayout L = fused_layout(CAP, a.CPC, a.NST);
     double *sE = reinterpret_cast<double *>(fused_smem + L.off_E);
     int *offs = reinterpret_cast<int *>(fused_smem + L.off_offs);
-    int *PS = reinterpret_cast<int *>(fused_smem + L.off_ps);   // PS[class][cl] = class prefix count at the start of cell cl
-    int *bas = reinterpret_cast<int *>(fused_smem + L.off_base); // bas[class*32 + cl]: final slot = bas + class prefix count
+    int2 *cellinfo = reinterpret_cast<int2 *>(fused_smem + L.off_cell); // {first slot, count} of the tile's cells
+    int4 *rowinfo = reinterpret_cast<int4 *>(fused_smem + L.off_row);   // per row: ballots L, S, R; running counts before it
+    int2 *basd = reinterpret_cast<int2 *>(fused_smem + L.off_base);     // [class*32 + cell]: {slot base, destination cell}
     double *qx = reinterpret_cast<double *>(fused_smem + L.off_q), *qvx = qx + FUSED_DEF, *qvy = qx + 2 * FUSED_DEF,
            *qvz = qx + 3 * FUSED_DEF;
     int *qpos = reinterpret_cast<int *>(qx + 4 * FUSED_DEF);
@@ -415,8 +421,8 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
     const unsigned lt = (1u << lane) - 1u;
     DevState *st = a.st;
     const int nc = a.k.nc;
-    int bad = 0; // FA_* bits
-    int mc = 0;  // largest new per-cell count seen by this lane
+    int bad = 0;  // FA_* bits
+    int mc = 0;   // largest new per-cell count seen by this lane
     int hmax = 0; // largest high word of the |v'| components seen by this lane
 
     if (!*(volatile int *)&st->abort) {
@@ -426,6 +432,7 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
         X.Cm = max(X.C0 - 1, 0);
         X.nc = nc;
         X.CAP = a.SCAP;
+        X.STR = CAP;
         X.offs = offs;
         const int Cm = X.Cm, Cp = min(X.C1 + 1, nc);
         for (int idx = lane; idx <= Cp - Cm; idx += 32) offs[idx] = a.off_old[Cm + idx];
@@ -469,72 +476,60 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
             const int n = kind == FK_VIRTUAL ? 0 : offs[cB - Cm] - sA;
             const int pad = sA & 1, gbase = sA - pad;
             const int nrows = n > 0 ? (pad + n + 31) >> 5 : 0;
+            // lane q: first slot of local cell q (q = ncell: the end of the tile), from off_old
+            int st_q = pad + n;
+            if (kind != FK_VIRTUAL && lane <= ncell) {
+                st_q = offs[cA - Cm + lane] - gbase;
+                if (lane < ncell) cellinfo[lane] = make_int2(st_q, offs[cA - Cm + lane + 1] - gbase - st_q);
+            }
+            __syncwarp();
             const bool odd = two && (it & 1);
             double *px = odd ? stage1 : stage0;
             if (n > 0) {
                 if (odd) { mbar_wait(mb1, ph1); ph1 ^= 1u; }
-                else        { mbar_wait(mb0, ph0); ph0 ^= 1u; }
+                else     { mbar_wait(mb0, ph0); ph0 ^= 1u; }
             }
 
             // ---- sweep 1a: push into registers and classify (fused_sweep1a) ----------------------------------
             double X_[RMAX], VX_[RMAX], VY_[RMAX], VZ_[RMAX];
-            int W_[RMAX]; // 1a: class | (border cell + 1) << 2 | bad << 8;  1b: -1, or prefix count << 8 | class*32 + cell
-            if (cA == 0 || cB == nc) fused_sweep1a_all<PERIODIC, true, RMAX>(a.k, px, a.SCAP, sEs, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
-            else fused_sweep1a_all<PERIODIC, false, RMAX>(a.k, px, a.SCAP, sEs, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
+            int W_[RMAX]; // 1a: class | cell << 2 | bad << 8;  1b: -1, or class prefix count << 8 | class*32 + cell
+            if (cA == 0 || cB == nc) fused_sweep1a_all<PERIODIC, true, RMAX>(a.k, px, sEs, cellinfo, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
+            else fused_sweep1a_all<PERIODIC, false, RMAX>(a.k, px, sEs, cellinfo, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
+            __syncwarp();
+            // the stage has been read: refill it with the next item to load
+            if (lane == 0) fused_issue(a, X, two ? I2 : I1, px, odd ? mb1 : mb0);
 
-            // ---- sweep 1b: prefix counts per class (ballot/popc), samples at the cell borders -------------
+            // ---- sweep 1b: prefix counts per class (ballot/popc); the row's ballots are kept for the cell borders ---
             unsigned run = 0; // running class counts of the tile: L | S << 10 | R << 20
-            int lastcl = -1;
 #pragma unroll
             for (int r = 0; r < RMAX; ++r) {
                 if (r < nrows) {
                     const int w = W_[r];
-                    const int g = w & 3, cle = ((w >> 2) & 63) - 1;
+                    const int g = w & 3;
                     if (w & 256) bad |= FA_BAD_PARTICLE;
-                    int prev = __shfl_up_sync(FULL, cle, 1);
-                    if (lane == 0) prev = lastcl;
-                    lastcl = __shfl_sync(FULL, cle, 31);
                     const unsigned mL = __ballot_sync(FULL, g == 0), mS = __ballot_sync(FULL, g == 1), mR = __ballot_sync(FULL, g == 2);
-                    if (cle != prev) {
-                        if (cle > prev) {
-                            // first slot of cell cle (cells prev+1 .. cle-1 are empty): sample the prefix counts and
-                            // check the grouping against off_old
-                            const int i = (r << 5) + lane;
-                            const int bL = (int)(run & 1023u) + __popc(mL & lt), bS = (int)((run >> 10) & 1023u) + __popc(mS & lt),
-                                      bR = (int)(run >> 20) + __popc(mR & lt);
-#pragma unroll 1
-                            for (int q = prev + 1; q <= cle; ++q) {
-                                PS[q] = bL; PS[KP + q] = bS; PS[2 * KP + q] = bR;
-                                if (offs[cA - Cm + q] - gbase != i) bad |= FA_BAD_PARTICLE;
-                            }
-                        } else {
-                            bad |= FA_BAD_PARTICLE;
-                        }
-                    }
+                    if (lane == 0) rowinfo[r] = make_int4((int)mL, (int)mS, (int)mR, (int)run);
                     const unsigned mo = g == 0 ? mL : (g == 1 ? mS : mR);
                     const int mine = (int)((run >> (10 * g)) & 1023u) + __popc(mo & lt);
-                    W_[r] = g < 3 ? (mine << 8) | (g * 32 + cle) : -1;
+                    W_[r] = g < 3 ? (mine << 8) | (g * 32 + ((w >> 2) & 31)) : -1;
                     run += (unsigned)__popc(mL) | ((unsigned)__popc(mS) << 10) | ((unsigned)__popc(mR) << 20);
                 }
             }
-            const int runL = (int)(run & 1023u), runS = (int)((run >> 10) & 1023u), runR = (int)(run >> 20);
-            if (kind != FK_VIRTUAL) {
-                for (int q = lastcl + 1 + lane; q <= ncell; q += 32) {
-                    PS[q] = runL; PS[KP + q] = runS; PS[2 * KP + q] = runR;
-                    if (offs[cA - Cm + q] - gbase != pad + n) bad |= FA_BAD_PARTICLE;
-                }
-            }
             __syncwarp();
-            // the stage has been read: refill it with the item after next
-            if (lane == 0) fused_issue(a, X, two ? I2 : I1, px, odd ? mb1 : mb0);
 
-            // ---- per-cell phase (lane = local cell) -------------------------------------------------
-            int Lc = 0, Sc = 0, Rc = 0, psL = 0, psS = 0, psR = 0;
-            if (kind != FK_VIRTUAL && lane < ncell) {
-                psL = PS[lane]; Lc = PS[lane + 1] - psL;
-                psS = PS[KP + lane]; Sc = PS[KP + lane + 1] - psS;
-                psR = PS[2 * KP + lane]; Rc = PS[2 * KP + lane + 1] - psR;
+            // ---- per-cell phase (lane q = local cell q; lane ncell = the end of the tile) ---------------------
+            // class prefix counts at the first slot of cell q, from the ballots of the row that holds it
+            unsigned ps = run;
+            if ((st_q >> 5) < nrows) {
+                const int4 ri = rowinfo[st_q >> 5];
+                const unsigned below = (1u << (st_q & 31)) - 1u;
+                ps = (unsigned)ri.w + ((unsigned)__popc((unsigned)ri.x & below) | ((unsigned)__popc((unsigned)ri.y & below) << 10) |
+                                       ((unsigned)__popc((unsigned)ri.z & below) << 20));
             }
+            const unsigned c3 = __shfl_down_sync(FULL, ps, 1) - ps; // class counts of cell q (fields cannot borrow)
+            const bool mycell = kind != FK_VIRTUAL && lane < ncell;
+            const int Lc = mycell ? (int)(c3 & 1023u) : 0, Sc = mycell ? (int)((c3 >> 10) & 1023u) : 0, Rc = mycell ? (int)(c3 >> 20) : 0;
+            const int psL = (int)(ps & 1023u), psS = (int)((ps >> 10) & 1023u), psR = (int)(ps >> 20);
             int Rm1 = __shfl_up_sync(FULL, Rc, 1);
             if (lane == 0) Rm1 = pvR;
             int Lp1 = __shfl_down_sync(FULL, Lc, 1);
@@ -542,12 +537,12 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
             const int Lc0 = __shfl_sync(FULL, Lc, 0);
             if (kind == FK_REAL && lane < ncell) {
                 const int c = cA + lane;
-                const int oo = offs[c - Cm], oo1 = offs[c + 1 - Cm];
-                const int pre_c = (a.k.periodic && c == nc - 1) ? OL : 0;
-                const int pre_c1 = (a.k.periodic && c + 1 == nc - 1) ? OL : 0;
-                bas[lane] = oo + (c == 1 ? -OL : shift) - Rm1 - psL;
-                bas[32 + lane] = oo + (c >= 1 ? shift : 0) + Lc + pre_c - psS;
-                bas[64 + lane] = oo1 + shift - Rc + Lp1 + pre_c1 - psR;
+                const int oo = gbase + st_q, oo1 = oo + cellinfo[lane].y;
+                const int pre_c = (PERIODIC && c == nc - 1) ? OL : 0;
+                const int pre_c1 = (PERIODIC && c + 1 == nc - 1) ? OL : 0;
+                basd[lane] = make_int2(oo + (c == 1 ? -OL : shift) - Rm1 - psL, c - 1);
+                basd[32 + lane] = make_int2(oo + (c >= 1 ? shift : 0) + Lc + pre_c - psS, c);
+                basd[64 + lane] = make_int2(oo1 + shift - Rc + Lp1 + pre_c1 - psR, c + 1);
                 if (lane < ncell - 1) { // count / offset of cell c (the tile's last cell waits for the next tile)
                     const int cn = pre_c + Rm1 + Sc + Lp1 + (c == 0 ? AR : 0);
                     a.count_new[c] = cn;
@@ -557,7 +552,7 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
             }
             if (pv_real && lane == 0) { // count / offset of the previous tile's last cell
                 const int c = cA - 1;
-                const int pre_c = (a.k.periodic && c == nc - 1) ? OL : 0;
+                const int pre_c = (PERIODIC && c == nc - 1) ? OL : 0;
                 const int cn = pre_c + pvRR + pvS + Lc0 + (c == 0 ? AR : 0);
                 const int o0 = c == 0 ? 0 : pv_off + shift - pvRR + pvL;
                 a.count_new[c] = cn;
@@ -567,8 +562,8 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
             }
             if (ndef) { // right-movers of the previous tile's last cell: their cell is cA, its L count is known now
                 if (lane < ndef) {
-                    const long long p = (long long)qpos[lane] + Lc0;
-                    if (p < 0 || p >= a.capacity) bad |= FA_BAD_PARTICLE;
+                    const int p = qpos[lane] + Lc0;
+                    if ((unsigned)p >= cap32) bad |= FA_BAD_PARTICLE;
                     else {
                         a.dx[p] = qx[lane]; a.dvx[p] = qvx[lane]; a.dvy[p] = qvy[lane]; a.dvz[p] = qvz[lane];
                         a.dcell[p] = cA;
@@ -580,31 +575,34 @@ __global__ void __launch_bounds__(32) fused_kernel(FusedArgs a)
 
             // ---- sweep 2: every particle straight to its final slot ----------------------------------
             if (kind == FK_REAL) {
-                const int kdef = 64 + ncell - 1; // class R of the tile's last cell
+                const int kdef = 64 + ncell - 1;                                 // class R of the tile's last cell
+                const int rdef = __shfl_sync(FULL, st_q, max(ncell - 1, 0)) >> 5; // first row that can hold it
 #pragma unroll
                 for (int r = 0; r < RMAX; ++r) {
                     if (r < nrows) {
                         const int pk = W_[r];
-                        const int key = pk & 0xff;
                         const bool has = pk >= 0;
-                        const bool defer = has && key == kdef;
-                        const int p = has ? bas[key] + (pk >> 8) : 0;
+                        const int2 bd = basd[pk & 127];
+                        const int p = bd.x + (pk >> 8);
+                        const bool defer = has && (pk & 127) == kdef;
                         const bool inb = (unsigned)p < cap32;
                         if (has && !inb) bad |= FA_BAD_PARTICLE;
                         if (has && !defer && inb) {
                             a.dx[p] = X_[r]; a.dvx[p] = VX_[r]; a.dvy[p] = VY_[r]; a.dvz[p] = VZ_[r];
-                            a.dcell[p] = cA - 1 + (key & 31) + (key >> 5);
+                            a.dcell[p] = bd.y;
                         }
-                        const unsigned md = __ballot_sync(FULL, defer);
-                        if (md) {
-                            if (defer) {
-                                const int q = ndef + __popc(md & lt);
-                                if (q < FUSED_DEF) {
-                                    qx[q] = X_[r]; qvx[q] = VX_[r]; qvy[q] = VY_[r]; qvz[q] = VZ_[r];
-                                    qpos[q] = p;
-                                } else bad |= FA_DEFER_OVERFLOW;
+                        if (r >= rdef) {
+                            const unsigned md = __ballot_sync(FULL, defer);
+                            if (md) {
+                                if (defer) {
+                                    const int q = ndef + __popc(md & lt);
+                                    if (q < FUSED_DEF) {
+                                        qx[q] = X_[r]; qvx[q] = VX_[r]; qvy[q] = VY_[r]; qvz[q] = VZ_[r];
+                                        qpos[q] = p;
+                                    } else bad |= FA_DEFER_OVERFLOW;
+                                }
+                                ndef = min(ndef + __popc(md), FUSED_DEF);
                             }
-                            ndef = min(ndef + __popc(md), FUSED_DEF);
                         }
                     }
                 }

@@ -613,7 +613,7 @@ static FusedGeom fused_geom(const pic_species *s)
     g.cpc = fused_cells_per_cta(s);
     g.stages = sim->opt_fused_stages ? sim->opt_fused_stages : FUSED_STAGES_DEFAULT;
     g.slots = sim->opt_fused_slots ? std::min(sim->opt_fused_slots, g.rows * 32) : g.rows * 32;
-    g.smem = (size_t)fused_layout(g.slots, g.cpc, g.stages).total;
+    g.smem = (size_t)fused_layout(g.rows * 32, g.cpc, g.stages).total;
     g.ctas_per_sm = std::max(1, std::min(32, FUSED_SMEM_SM / ((int)g.smem + 1024)));
     return g;
 }
