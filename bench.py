@@ -298,8 +298,12 @@ def main():
                     "algorithmic_bytes_per_particle": per_particle, "particles_per_launch": n_per_launch,
                     "traffic": committed_traffic(dom, f"config{args.config}"),
                     "kernel_ms_per_step": {k: v[0] / args.steps for k, v in ktimes.items() if v[1]},
-                    "step_algorithmic_GBps": sum(ALG_BYTES[k][0 if all_live else 1] * n_per_launch * v[1]
-                                                 for k, v in ktimes.items() if k in ALG_BYTES) / (ms * 1e-3) / 1e9}
+                    # kernels behind a fused step are guarded no-ops (they return at once): count a kernel's bytes only
+                    # if its launches took at least a tenth of what those bytes cost at the peak
+                    "step_algorithmic_GBps": sum(
+                        ALG_BYTES[k][0 if all_live else 1] * n_per_launch * v[1] for k, v in ktimes.items()
+                        if k in ALG_BYTES and v[1] and v[0] * 1e-3 / v[1] > 0.1 * ALG_BYTES[k][0] * n_per_launch / (peak * 1e9)
+                    ) / (ms * 1e-3) / 1e9}
         roofline["step_frac"] = roofline["step_algorithmic_GBps"] / peak
     pic.pic_destroy(sim)
     del descs, sim

@@ -585,18 +585,32 @@ static int push_split(pic_species *s, bool will_arrange, const int *guard)
     return PIC_OK;
 }
 
-// Rows of 32 slots per tile (the fused_kernel<RMAX> instance) for this species' current state, or 0
-// when a cell may not fit a tile.  A tile must hold at least one cell; maxcount is the bound read
-// at the last sync, so leave room for it to grow.
-static int fused_cells_per_cta(const pic_species *s)
+struct FusedGeom { int rows, slots, stages, cpc, ctas_per_sm; size_t smem; };
+
+// CTAs of fused_kernel<rows> an SM holds: registers (launch bounds of the instance) or shared memory.
+static int fused_ctas_per_sm(int rows, int cpc, int stages)
+{
+    const int by_regs = rows == 8 ? 16 : rows == 12 ? 12 : 8;
+    const int by_smem = FUSED_SMEM_SM / (fused_layout(rows * 32, cpc, stages).total + 1024);
+    return std::max(1, std::min(32, std::min(by_regs, by_smem)));
+}
+
+// Cells per CTA.  Every chunk pushes two halo cells on top of its own, and the grid runs in waves of
+// sm_count * ctas_per_sm CTAs: pick the chunk size that wastes least to halo work and a ragged last wave.
+static int fused_cells_per_cta(const pic_species *s, int rows, int stages)
 {
     const pic_sim *sim = s->sim;
     if (sim->opt_fused_cpc > 0) return sim->opt_fused_cpc;
-    const long long want = sim->nc / ((long long)sim->sm_count * 16);
-    return (int)std::max<long long>(8, std::min<long long>(FUSED_CPC_DEFAULT, want));
+    int best = FUSED_CPC_DEFAULT;
+    double best_score = -1.0;
+    for (int cpc = 2; cpc <= 128; ++cpc) {
+        const double resident = (double)sim->sm_count * fused_ctas_per_sm(rows, cpc, stages);
+        const double chunks = (double)((sim->nc + cpc - 1) / cpc);
+        const double score = chunks / (std::ceil(chunks / resident) * resident) * cpc / (cpc + 2.0);
+        if (score > best_score * 1.0001) { best_score = score; best = cpc; }
+    }
+    return best;
 }
-
-struct FusedGeom { int rows, slots, stages, cpc, ctas_per_sm; size_t smem; };
 
 // Launch geometry of the fused step for this species' current state; rows == 0 when a cell may not fit
 // a tile.  A tile must hold at least one cell; maxcount is the bound read at the last sync, so leave room
@@ -610,11 +624,11 @@ static FusedGeom fused_geom(const pic_species *s)
     g.rows = sim->opt_fused_rows;
     if (g.rows == 0) g.rows = need <= 8 * 32 ? 8 : need <= 12 * 32 ? 12 : need <= 16 * 32 ? 16 : 0;
     if (g.rows == 0) return g;
-    g.cpc = fused_cells_per_cta(s);
     g.stages = sim->opt_fused_stages ? sim->opt_fused_stages : FUSED_STAGES_DEFAULT;
+    g.cpc = fused_cells_per_cta(s, g.rows, g.stages);
     g.slots = sim->opt_fused_slots ? std::min(sim->opt_fused_slots, g.rows * 32) : g.rows * 32;
     g.smem = (size_t)fused_layout(g.rows * 32, g.cpc, g.stages).total;
-    g.ctas_per_sm = std::max(1, std::min(32, FUSED_SMEM_SM / ((int)g.smem + 1024)));
+    g.ctas_per_sm = fused_ctas_per_sm(g.rows, g.cpc, g.stages);
     return g;
 }
 
