@@ -602,8 +602,12 @@ static int fused_cells_per_cta(const pic_species *s, int rows, int stages)
     const pic_sim *sim = s->sim;
     if (sim->opt_fused_cpc > 0) return sim->opt_fused_cpc;
     int best = FUSED_CPC_DEFAULT;
+    {   // many waves: the ragged last wave is noise, keep the measured optimum
+        const double resident = (double)sim->sm_count * fused_ctas_per_sm(rows, best, stages);
+        if ((double)((sim->nc + best - 1) / best) >= 4.0 * resident) return best;
+    }
     double best_score = -1.0;
-    for (int cpc = 2; cpc <= 128; ++cpc) {
+    for (int cpc = 2; cpc <= FUSED_CPC_DEFAULT; ++cpc) {
         const double resident = (double)sim->sm_count * fused_ctas_per_sm(rows, cpc, stages);
         const double chunks = (double)((sim->nc + cpc - 1) / cpc);
         const double score = chunks / (std::ceil(chunks / resident) * resident) * cpc / (cpc + 2.0);
