@@ -173,6 +173,20 @@ def run_reference(args, rank):
     return 0
 
 
+def aggregate_over_ranks(dist, seconds, pushes, device):
+    """Whole-job figures of N independent replicas: (max over ranks of the time, sum over ranks of the pushes).
+    dist is torch.distributed (initialised) or None for a single process.  No data-path collective exists on
+    this path; this is the only exchange, and it happens outside the timed region."""
+    if dist is None:
+        return float(seconds), float(pushes)
+    import torch
+    t = torch.tensor([seconds, pushes], dtype=torch.float64, device=device)
+    tmax = t.clone()
+    dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(tmax[0]), float(t[1])
+
+
 def workload_config(config, inp):
     from paper_2603_24508_b200 import workloads
     c = workloads.CONFIGS[config]
@@ -272,14 +286,7 @@ def main():
     ktimes = {k: pic.pic_kernel_time(sim, k) for k in ("mover", "hist", "scan", "scatter", "general", "fused")}
     info = [pic.pic_arrange_info(sp) for sp in sim.species]
 
-    if dist is not None:
-        t = torch.tensor([ms, pushes], dtype=torch.float64, device=dev)
-        tmax = t.clone()
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        ms_all, pushes_all = float(tmax[0]), float(t[1])
-    else:
-        ms_all, pushes_all = ms, pushes
+    ms_all, pushes_all = aggregate_over_ranks(dist, ms, pushes, dev)
     value = pushes_all / (ms_all * 1e-3)
 
     # roofline of the dominant kernel (this rank)
@@ -335,12 +342,7 @@ def main():
         d2h = n_out * 36 + 16 * len(res)
         n0_e = sum(len(s["x"]) for s in inp["species"])
         e_pushes = 0.5 * (n0_e + n_out) * cfg_steps
-        if dist is not None:
-            t = torch.tensor([t_e2e, e_pushes], dtype=torch.float64, device=dev)
-            tm = t.clone()
-            dist.all_reduce(tm, op=dist.ReduceOp.MAX)
-            dist.all_reduce(t, op=dist.ReduceOp.SUM)
-            t_e2e, e_pushes = float(tm[0]), float(t[1])
+        t_e2e, e_pushes = aggregate_over_ranks(dist, t_e2e, e_pushes, dev)
         e2e = {"value": e_pushes / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d / cfg_steps,
                "d2h_bytes_per_step": d2h / cfg_steps, "steps": cfg_steps, "seconds": t_e2e,
                "call": "pic_run_host (pinned host SoA in, cudaMalloc + H2D + pic_create + pic_push(nsteps) + D2H + free inside)"}
