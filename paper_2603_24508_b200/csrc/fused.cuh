@@ -18,10 +18,10 @@
 // fused_edge_kernel (one small block) pushes cells 0, 1, nc-2, nc-1, publishes OL / AR, counts the
 // walls and writes the wrapped particles.  fused_kernel streams everything else: each 32-thread
 // CTA owns a chunk of CPC consecutive cells, cuts it greedily into tiles of whole cells that fit
-// RMAX rows of 32 slots, stages tile after tile in a two-stage shared-memory ring with TMA bulk
-// copies (cp.async.bulk + mbarrier; the E nodes of the chunk are staged once the same way),
-// pushes each tile into REGISTERS (the stage is refilled at once), ranks with ballot/popc prefix
-// counts per class, and stores every particle straight to its final slot.  Across tiles it
+// RMAX rows of 32 slots, stages tile after tile in shared memory with TMA bulk copies
+// (cp.async.bulk + mbarrier; the E nodes of the chunk are staged once the same way), pushes each
+// tile into REGISTERS (the stage is refilled at once, so the next tile's copies overlap the rest),
+// ranks with ballot/popc prefix counts per class, and stores every particle straight to its final slot.  Across tiles it
 // carries the counts of the previous cell; right-movers of a tile's last cell wait (a few
 // particles, in shared memory) for the next tile's first-cell count.  Chunk ends push one halo
 // cell redundantly instead of talking to the neighbour CTA.  Anything unexpected (a particle
