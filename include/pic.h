@@ -160,13 +160,13 @@ int pic_fused_info(pic_species *sp, int32_t *active, int32_t *decline_reasons, i
 size_t pic_workspace_bytes(int32_t nc, int64_t capacity);
 
 /* Variant switches and tuning knobs, for measurements (profiles/ compares them).  Flags (0/1):
- * "e_stage": 0 = E through the read-only global path, 1 = E window staged in shared memory by
- * TMA bulk copy (default); "fused": 1 = single-pass push+arrange when arrange_every == 1
- * (default), 0 = separate mover / scan / scatter kernels; "kernel_timing": 1 = record CUDA
- * events around every kernel launch (see pic_kernel_time).  Knobs of the fused step:
+ * "fused": 1 = single-pass push+arrange when arrange_every == 1 (default; particles and the E
+ * nodes of each chunk staged in shared memory by TMA bulk copies), 0 = separate mover / scan /
+ * scatter kernels (E through the read-only global path); "kernel_timing": 1 = record CUDA events
+ * around every kernel launch (see pic_kernel_time).  Knobs of the fused step:
  * "fused_cells_per_cta" (cells per chunk, 1..256; 0 = automatic, at most 64), "fused_rows" (rows
  * of 32 slots per tile: 8, 12 or 16; 0 = automatic from the largest per-cell count),
- * "fused_stage_slots" (slots per shared-memory stage, even, <= 32*rows; 0 = 32*rows), "fused_stages"
+ * "fused_stage_slots" (largest tile in slots, even, <= 32*rows; 0 = 32*rows), "fused_stages"
  * (stages of the TMA ring: 1 or 2; 0 = default 1).  Results never depend on any of them.
  * PIC_EINVAL for an unknown key or a value out of range. */
 int pic_set_option(pic_sim *sim, const char *key, int value);

@@ -299,7 +299,8 @@ __device__ __forceinline__ void fused_issue(const FusedArgs &a, const FusedCtx &
 // same sequence of rounded operations as push_core, written as straight-line
 // code without branches or warp collectives so that the rows' dependency chains interleave.  Slots
 // outside the tile (the alignment pad, the tail of the last row, rows behind it inside the group)
-// recompute a clamped slot and are masked out.
+// push whatever the stage holds there (every row lies inside the stage; no address depends on it)
+// and are masked out.
 // EDGE = the tile holds cell 0 or cell nc-1: only there can a particle wrap / be absorbed (class X), can
 // floor(x/dx) need the clamp of reading S8, or can x leave the gather range legitimately.  Elsewhere any
 // of that marks the particle bad (it moved more than one cell, or the grouping is broken).
@@ -316,8 +317,7 @@ __device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *
     for (int r = R0; r < R0 + CNT; ++r) {
         const int i = (r << 5) + lane;
         const bool valid = (unsigned)(i - pad) < (unsigned)n;
-        const int ic = min(max(i, pad), pad + n - 1);
-        const double x = px[ic], vx = px[CAP + ic], vy = px[2 * CAP + ic], vz = px[3 * CAP + ic];
+        const double x = px[i], vx = px[CAP + i], vy = px[2 * CAP + i], vz = px[3 * CAP + i];
         const double xs = __dmul_rn(x, k.inv_dx);
         double jf = floor(xs);
         int jc = __double2int_rd(xs);
@@ -535,6 +535,7 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
             int Lp1 = __shfl_down_sync(FULL, Lc, 1);
             if (lane >= ncell - 1) Lp1 = 0; // last cell: added when the next tile knows it
             const int Lc0 = __shfl_sync(FULL, Lc, 0);
+            bool oob = false;
             if (kind == FK_REAL && lane < ncell) {
                 const int c = cA + lane;
                 const int oo = gbase + st_q, oo1 = oo + cellinfo[lane].y;
@@ -543,6 +544,13 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
                 basd[lane] = make_int2(oo + (c == 1 ? -OL : shift) - Rm1 - psL, c - 1);
                 basd[32 + lane] = make_int2(oo + (c >= 1 ? shift : 0) + Lc + pre_c - psS, c);
                 basd[64 + lane] = make_int2(oo1 + shift - Rc + Lp1 + pre_c1 - psR, c + 1);
+                // slot ranges of the three classes of this cell (ranks are below the class counts): all stores of
+                // sweep 2 stay inside the arrays, or the tile is declined before any of them is issued
+                const int bL = oo + (c == 1 ? -OL : shift) - Rm1, bS = oo + (c >= 1 ? shift : 0) + Lc + pre_c,
+                          bR = oo1 + shift - Rc + Lp1 + pre_c1;
+                oob = (Lc && ((unsigned)bL >= cap32 || (unsigned)(bL + Lc - 1) >= cap32)) ||
+                      (Sc && ((unsigned)bS >= cap32 || (unsigned)(bS + Sc - 1) >= cap32)) ||
+                      (Rc && ((unsigned)bR >= cap32 || (unsigned)(bR + Rc - 1) >= cap32));
                 if (lane < ncell - 1) { // count / offset of cell c (the tile's last cell waits for the next tile)
                     const int cn = pre_c + Rm1 + Sc + Lp1 + (c == 0 ? AR : 0);
                     a.count_new[c] = cn;
@@ -574,7 +582,9 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
             __syncwarp();
 
             // ---- sweep 2: every particle straight to its final slot ----------------------------------
-            if (kind == FK_REAL) {
+            const bool tile_oob = __any_sync(FULL, oob);
+            if (tile_oob) bad |= FA_BAD_PARTICLE;
+            if (kind == FK_REAL && !tile_oob) {
                 const int kdef = 64 + ncell - 1;                                 // class R of the tile's last cell
                 const int rdef = __shfl_sync(FULL, st_q, max(ncell - 1, 0)) >> 5; // first row that can hold it
 #pragma unroll
@@ -585,9 +595,7 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
                         const int2 bd = basd[pk & 127];
                         const int p = bd.x + (pk >> 8);
                         const bool defer = has && (pk & 127) == kdef;
-                        const bool inb = (unsigned)p < cap32;
-                        if (has && !inb) bad |= FA_BAD_PARTICLE;
-                        if (has && !defer && inb) {
+                        if (has && !defer) {
                             a.dx[p] = X_[r]; a.dvx[p] = VX_[r]; a.dvy[p] = VY_[r]; a.dvz[p] = VZ_[r];
                             a.dcell[p] = bd.y;
                         }

@@ -77,7 +77,7 @@ struct pic_sim {
     double Emax = 0; // max |E_node|
     std::vector<pic_species *> sp;
     unsigned long long launches = 0;
-    int opt_e_stage = 1, opt_fused = 1, opt_timing = 0;
+    int opt_fused = 1, opt_timing = 0;
     int opt_fused_cpc = 0, opt_fused_rows = 0, opt_fused_slots = 0, opt_fused_stages = 0; // tuning knobs of the fused step (0 = automatic)
     int sm_count = 148;
     // per-kernel device timing (option "kernel_timing"): event pairs recorded around launches
@@ -421,8 +421,7 @@ extern "C" int pic_set_option(pic_sim *sim, const char *key, int value)
 {
     if (!sim || !key) return PIC_EINVAL;
     const bool flag = value == 0 || value == 1;
-    if (!strcmp(key, "e_stage") && flag) sim->opt_e_stage = value;
-    else if (!strcmp(key, "kernel_timing") && flag) sim->opt_timing = value;
+    if (!strcmp(key, "kernel_timing") && flag) sim->opt_timing = value;
     else if (!strcmp(key, "fused") && flag) sim->opt_fused = value;
     else if (!strcmp(key, "fused_cells_per_cta") && value >= 0 && value <= FUSED_CPC_MAX) sim->opt_fused_cpc = value;
     else if (!strcmp(key, "fused_stage_slots") && value >= 0 && value <= 512 && value % 2 == 0) sim->opt_fused_slots = value;

@@ -13,9 +13,9 @@ from parity_util import compare, make_pair, run_bulk, run_stepwise
 pytestmark = pytest.mark.gpu
 
 VARIANTS = [
-    pytest.param({"fused": 0, "e_stage": 0}, id="split-ldg"),
-    pytest.param({"fused": 0, "e_stage": 1}, id="split-tma"),
-    pytest.param({"fused": 1, "e_stage": 1}, id="fused"),
+    pytest.param({"fused": 0}, id="split"),
+    pytest.param({"fused": 1}, id="fused"),
+    pytest.param({"fused": 1, "fused_stages": 2}, id="fused-2stage"),
 ]
 
 
