@@ -132,7 +132,9 @@ int pic_set_field(pic_sim *sim, const double *E_nodes_host);
  * particles included).  Syncs. */
 int pic_n_slots(pic_species *sp, int64_t *n);
 
-/* Which buffer set (0 or 1) holds the current state.  Does not sync. */
+/* Which buffer set (0 or 1) holds the current state.  Syncs if fused steps are still unchecked (a
+ * declined fused step is redone by the split kernels here, as in every synchronising call);
+ * read the caller-owned buffers only after this or another synchronising call. */
 int pic_active_buffer(pic_species *sp, int *which);
 
 /* Per-cell counts (nc) and exclusive offsets (nc+1, offset[nc] = n_live) of the last

@@ -25,8 +25,9 @@
 // carries the counts of the previous cell; right-movers of a tile's last cell wait (a few
 // particles, in shared memory) for the next tile's first-cell count.  Chunk ends push one halo
 // cell redundantly instead of talking to the neighbour CTA.  Anything unexpected (a particle
-// moving two cells, a cell larger than a tile) aborts the whole step: the source buffers are
-// untouched, and the guarded split kernels launched right behind (mover / scan / scatter) redo it.
+// moving two cells, a cell larger than a tile) declines the whole step: the source buffers are
+// untouched, the step's id is recorded, later fused launches exit at once, and the host redoes
+// the declined steps with the split kernels (mover / scan / scatter) at its next synchronising call.
 #pragma once
 #include "pic_device.cuh"
 
@@ -59,6 +60,7 @@ struct FusedArgs {
     int CPC;
     int SCAP; // largest tile, in slots (<= RMAX*32, even)
     int NST;  // stages of the ring: 1 or 2
+    int step_id; // low 31 bits of the species' step counter before this step
 };
 
 // Dynamic shared memory of one fused_kernel CTA (one warp): NST stages of CAP = RMAX*32 slots.
@@ -661,7 +663,9 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
                 st->used_general = 0;
                 st->run_split = 0;
             } else {
-                st->run_split = 1;
+                // declined: nothing of the state was touched (outputs went to the other buffer set); remember which
+                // step it was, every later fused launch exits at once, the host redoes the steps (pic.cu: verify_fused)
+                if (!st->fused_disabled) st->fail_step = a.step_id;
                 st->fused_disabled = 1;
             }
             st->n_next = 0;

@@ -52,6 +52,9 @@ struct pic_species {
     int h_maxcount = 0;                // bound of the largest per-cell count at the last sync (sizes the fused tiles)
     int h_abort_reason = 0;
     bool fused_off = false;            // the device reported a declined fused step (sticky)
+    // fused steps enqueued but not yet verified (verify_fused): how many, and the host state when the run began
+    long long unv_steps = 0, unv_steps0 = 0;
+    int unv_cur0 = 0, unv_off0 = 0;
     // host-side conservative bound on cell displacement since the last arrange (decides whether the
     // general-path kernels need to be enqueued at all)
     double vkick = 0;                  // 2*|h|*max|E|
@@ -220,6 +223,7 @@ static int run_maxcount(pic_species *s, int which, const int *guard)
 }
 
 static int fused_rows(const pic_species *s, int *ctas_per_sm);
+static int verify_fused(pic_species *s);
 
 static bool fused_possible(const pic_species *s)
 {
@@ -405,6 +409,8 @@ extern "C" pic_species *pic_species_at(pic_sim *sim, int i)
 extern "C" int pic_set_field(pic_sim *sim, const double *E)
 {
     if (!sim || !E) return PIC_EINVAL;
+    for (pic_species *s : sim->sp) // steps already enqueued must have run (or be redone) with the old field
+        if (int rc = verify_fused(s)) return rc;
     double emax = 0;
     for (int j = 0; j <= sim->nc; ++j) {
         if (!std::isfinite(E[j])) return PIC_EINVAL;
@@ -531,6 +537,7 @@ static int arrange_split(pic_species *s, bool hist_ready, const int *guard, bool
 extern "C" int pic_arrange(pic_species *s)
 {
     if (!s) return PIC_EINVAL;
+    if (int rc = verify_fused(s)) return rc;
     return arrange_split(s, false, nullptr, false);
 }
 
@@ -642,8 +649,10 @@ static int fused_rows(const pic_species *s, int *ctas_per_sm)
     return g.rows;
 }
 
-// One fused push+arrange step, followed by the guarded split chain that redoes the step if the
-// fused kernels declined on the device (DevState::run_split).
+// One fused push+arrange step.  Nothing is enqueued behind it to catch a declined step: the device records
+// the first step that declined and turns every later fused launch into a no-op, and verify_fused() -- run by
+// every synchronising call and before any non-fused work -- rewinds the host bookkeeping to that step and
+// redoes the rest with the split kernels.
 static int push_fused(pic_species *s)
 {
     pic_sim *sim = s->sim;
@@ -662,9 +671,15 @@ static int push_fused(pic_species *s)
     a.CPC = geo.cpc;
     a.SCAP = geo.slots;
     a.NST = geo.stages;
+    a.step_id = (int)(s->steps & 0x7fffffff);
     const int rows = geo.rows;
     const int grid = (sim->nc + a.CPC - 1) / a.CPC;
     const size_t smem = geo.smem;
+    if (s->unv_steps == 0) {
+        s->unv_steps0 = s->steps;
+        s->unv_cur0 = s->cur;
+        s->unv_off0 = s->cur_off;
+    }
     {
         KernelSpan span(sim, K_FUSED);
         fused_edge_kernel<<<1, 128, 0, sim->stream>>>(a);
@@ -675,12 +690,52 @@ static int push_fused(pic_species *s)
         kern<<<grid, 32, smem, sim->stream>>>(a);
         if (int rc = launch_check(sim, "fused_kernel")) return rc;
     }
-    // fallback chain, all guarded by run_split; it leaves the same host-visible state behind
-    const int *guard = &s->d_st->run_split;
-    s->h_wsum = std::min<long long>(s->h_wsum + host_step_bound(s), 1LL << 40);
+    s->unv_steps++;
     s->h_steps_since_sync++;
-    if (int rc = push_split(s, true, guard)) return rc;
-    if (int rc = arrange_split(s, true, guard, true)) return rc; // flips cur / cur_off, marks fresh
+    s->cur = dst;
+    s->cur_off = on;
+    s->counts_fresh = true;
+    s->all_live = true;
+    s->reset_w = true;
+    s->h_wsum = 0;
+    s->h_grouped = true;
+    return PIC_OK;
+}
+
+// Check the fused steps enqueued since the last check.  If one declined, the device state is the one before
+// that step (later fused launches did nothing): rewind the host bookkeeping to it and redo the remaining steps
+// through the split path.  Syncs when there is anything to check.
+static int verify_fused(pic_species *s)
+{
+    if (s->unv_steps == 0) return PIC_OK;
+    DevState h;
+    CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, s->sim->stream));
+    CU(cudaStreamSynchronize(s->sim->stream));
+    const long long run = s->unv_steps;
+    s->unv_steps = 0;
+    if (!h.fused_disabled) return PIC_OK;
+    s->fused_off = true;
+    const long long k = ((long long)h.fail_step - (s->unv_steps0 & 0x7fffffff)) & 0x7fffffff; // steps that completed
+    if (k >= run) {
+        snprintf(g_err, sizeof g_err, "fused step bookkeeping: declined step %d outside the unverified run", h.fail_step);
+        return PIC_ESTATE;
+    }
+    s->cur = s->unv_cur0 ^ (int)(k & 1);
+    s->cur_off = s->unv_off0 ^ (int)(k & 1);
+    s->steps = s->unv_steps0 + k;
+    s->counts_fresh = true;
+    s->all_live = true;
+    s->reset_w = true;
+    s->h_wsum = 0;
+    s->h_grouped = true;
+    s->h_vmax = std::sqrt((double)bits_to_float(h.vmax2));
+    s->h_steps_since_sync = 0;
+    s->h_maxcount = h.maxcount;
+    for (long long left = run - k; left > 0;) {
+        const int chunk = (int)std::min<long long>(left, 1 << 20);
+        if (int rc = pic_push(s, chunk)) return rc;
+        left -= chunk;
+    }
     return PIC_OK;
 }
 
@@ -695,6 +750,7 @@ extern "C" int pic_push(pic_species *s, int nsteps)
             s->steps++;
             continue;
         }
+        if (int rc = verify_fused(s)) return rc; // the split kernels need the true state (total step count unchanged)
         if (int rc = push_split(s, will_arrange, nullptr)) return rc;
         s->steps++;
         if (will_arrange)
@@ -708,6 +764,7 @@ extern "C" int pic_push(pic_species *s, int nsteps)
 // ------------------------------------------------------------------------------------------
 static int read_state(pic_species *s, DevState &h)
 {
+    if (int rc = verify_fused(s)) return rc;
     CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, s->sim->stream));
     CU(cudaStreamSynchronize(s->sim->stream));
     if (h.n >= 0 && h.n <= s->n_ub) s->n_ub = h.n;
@@ -748,6 +805,7 @@ extern "C" int pic_n_slots(pic_species *s, int64_t *n)
 extern "C" int pic_active_buffer(pic_species *s, int *which)
 {
     if (!s || !which) return PIC_EINVAL;
+    if (int rc = verify_fused(s)) return rc;
     *which = s->cur;
     return PIC_OK;
 }
@@ -762,6 +820,7 @@ extern "C" int pic_step_count(pic_species *s, int64_t *steps)
 extern "C" int pic_cell_counts(pic_species *s, int32_t *count_host, int32_t *offset_host)
 {
     if (!s) return PIC_EINVAL;
+    if (int rc = verify_fused(s)) return rc;
     if (!s->counts_fresh) return PIC_ESTATE;
     const int nc = s->sim->nc;
     if (count_host)

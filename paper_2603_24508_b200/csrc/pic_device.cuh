@@ -27,8 +27,8 @@ struct DevState {
     int status;       // ERR_* bits
     int need_general; // fast arranger declined (w_acc too large); the general path must run
     int used_general; // the last arrange ran the general path
-    int run_split;      // set by a fused step: 1 = it declined, the guarded split kernels behind it must run
-    int fused_disabled; // sticky: a fused step has declined; later fused launches exit at once
+    int run_split;      // unused (kept for layout)
+    int fused_disabled; // sticky: a fused step has declined (fail_step says which); later fused launches exit at once
     unsigned long long wall[2];      // cumulative absorbed at x<0 / x>=L
     unsigned long long wall_pend[2]; // fused step in flight: absorbed, not yet committed
     unsigned vmax2, vmax2_next;      // float bits (rounded up) of max |v|^2: current state / step in flight
@@ -39,7 +39,8 @@ struct DevState {
     int f_OL, f_AR;                  // fused step in flight: leavers of cell 0 downwards / wrapped arrivals in cell 0
     int ntiles, ntiles_next;         // tiles of the current partition (fused.cuh) / of the one being written
     int maxcount, maxcount_next;     // upper bound of the largest per-cell count: current state / step in flight
-    int pad[2];
+    int fail_step;                   // step id (FusedArgs::step_id) of the first fused step that declined
+    int pad[1];
 };
 
 // Per-species Boris constants (computed once on the host) and grid.

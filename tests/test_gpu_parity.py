@@ -295,3 +295,38 @@ def test_fused_empty_cells_and_sparse_density():
     assert (states[0].count == 0).any()
     info = pic.pic_fused_info(sim.species[0])
     assert info["decline_reasons"] == 0, info
+
+
+def test_fused_declined_mid_run_is_redone_at_the_next_sync():
+    """Fused steps are enqueued without a fallback behind them; a step that declines freezes the state and is
+    redone (with all later steps) by the split kernels at the next synchronising call.  Here one particle turns
+    fast enough to jump two cells only after a few gyration steps, in the middle of one pic_push(sp, 20)."""
+    inp = workloads.make(1, nc=512, ppc=40)
+    s = inp["species"][0]
+    for k in ("vx", "vy", "vz"):
+        s[k] = s[k].copy()
+    p = 7777
+    s["vx"][p], s["vy"][p], s["vz"][p] = 0.0, 0.0, 26.0
+    # oracle: first step at which that particle moves two cells or more
+    probe = oracle.State(s["x"][p:p + 1], s["vx"][p:p + 1], s["vy"][p:p + 1], s["vz"][p:p + 1], s["cell"][p:p + 1], nc=inp["nc"],
+                         dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E=inp["E"], qm=s["qm"], B=inp["B"], arrange_every=0)
+    first = None
+    for k in range(1, 21):
+        c0 = int(probe.cell[0])
+        probe.push(1)
+        d = abs(int(probe.cell[0]) - c0)
+        if min(d, inp["nc"] - d) >= 2:
+            first = k
+            break
+    assert first is not None and 2 <= first <= 15, first
+    sim, (st,) = make_pair(inp, options={"fused": 1})
+    sp = sim.species[0]
+    pic.pic_push(sp, 20)
+    st.push(20)
+    compare(sp, st, where="bulk 20 with a declined fused step inside", counts=True, nc=inp["nc"])
+    info = pic.pic_fused_info(sp)
+    assert info["decline_reasons"] & 1 and info["active"] == 0, info
+    assert pic.pic_step_count(sp) == 20
+    pic.pic_push(sp, 5)
+    st.push(5)
+    compare(sp, st, where="after the switch to the split path", counts=True, nc=inp["nc"])
