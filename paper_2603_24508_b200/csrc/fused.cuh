@@ -133,7 +133,7 @@ __device__ __forceinline__ int fused_classify(const PushConst &k, int j, const P
 __global__ void __launch_bounds__(128) fused_edge_kernel(FusedArgs a)
 {
     __shared__ double qx[2][FUSED_XCAP], qvx[2][FUSED_XCAP], qvy[2][FUSED_XCAP], qvz[2][FUSED_XCAP];
-    __shared__ int cL[4], cS[4], cR[4], cX[4];
+    __shared__ int cL[4], cR[4], cX[4];
     __shared__ int s_bad;
     DevState *st = a.st;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(128) fused_edge_kernel(FusedArgs a)
     }
     bad = (int)__reduce_or_sync(FULL, (unsigned)bad);
     if (lane == 0) {
-        cL[warp] = nL; cS[warp] = nS; cR[warp] = nR; cX[warp] = nX;
+        cL[warp] = nL; cR[warp] = nR; cX[warp] = nX;
         if (bad) atomicOr(&s_bad, bad);
     }
     __syncthreads();
@@ -679,19 +679,12 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
 }
 
 // Largest per-cell count of an offset array (sizes the fused tiles; only ever raises the bound).
-__global__ void maxcount_kernel(const int *__restrict__ off, int nc, DevState *st, const int *guard)
+__global__ void maxcount_kernel(const int *__restrict__ off, int nc, DevState *st)
 {
-    if (guard && !*guard) return;
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     int cn = c < nc ? off[c + 1] - off[c] : 0;
     cn = __reduce_max_sync(FULL, cn);
     if ((threadIdx.x & 31) == 0 && cn > *(volatile int *)&st->maxcount) atomicMax(&st->maxcount, cn);
-}
-
-__global__ void zero_guarded_kernel(int *__restrict__ p, int n, const int *guard)
-{
-    if (guard && !*guard) return;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) p[i] = 0;
 }
 
 } // namespace pic

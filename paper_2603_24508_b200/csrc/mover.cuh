@@ -13,7 +13,6 @@ struct MoverArgs {
     const double *E;  // nc+1 nodes
     int *count;       // per-cell histogram of the new cells (HIST only), pre-zeroed
     DevState *st;
-    const int *guard; // if not NULL: the kernel returns at once unless *guard != 0
     PushConst k;
 };
 
@@ -22,7 +21,6 @@ constexpr int MOVER_THREADS = 256;
 template <bool READ_CELL, bool HIST>
 __global__ void __launch_bounds__(MOVER_THREADS) mover_kernel(MoverArgs a)
 {
-    if (a.guard && !*a.guard) return;
     __shared__ int s_max;
     __shared__ unsigned s_vmax;
     if (threadIdx.x == 0) { s_max = 0; s_vmax = 0; }
@@ -32,8 +30,7 @@ __global__ void __launch_bounds__(MOVER_THREADS) mover_kernel(MoverArgs a)
     const int lane = threadIdx.x & 31;
     int dmax = 0, nleft = 0, nright = 0, bad = 0;
     float vm2 = 0.f; // upper bound of max |v'|^2 (feeds the next step's displacement bound)
-    // one pair of neighbouring particles per thread and iteration; the grid normally covers the array in
-    // one iteration (the guarded fallback launch uses a small grid and strides)
+    // one pair of neighbouring particles per thread and iteration (the grid covers the array in one iteration)
     const long long pairs = ((long long)n + 1) / 2;
     for (long long pb = (long long)blockIdx.x * MOVER_THREADS; pb < pairs; pb += (long long)gridDim.x * MOVER_THREADS) {
     const long long i0 = 2 * (pb + threadIdx.x);

@@ -214,11 +214,11 @@ static float bits_to_float(unsigned u)
 }
 
 // raise DevState::maxcount to the largest per-cell count of the offsets in slot `which`
-static int run_maxcount(pic_species *s, int which, const int *guard)
+static int run_maxcount(pic_species *s, int which)
 {
     pic_sim *sim = s->sim;
     const int nc = sim->nc;
-    maxcount_kernel<<<(nc + 255) / 256, 256, 0, sim->stream>>>(s->d_off[which], nc, s->d_st, guard);
+    maxcount_kernel<<<(nc + 255) / 256, 256, 0, sim->stream>>>(s->d_off[which], nc, s->d_st);
     return launch_check(sim, "maxcount_kernel");
 }
 
@@ -322,7 +322,7 @@ static int create_species(pic_sim *sim, const pic_species_desc &d, pic_species *
     CU(cudaMemcpyAsync(s->d_st, &h, sizeof h, cudaMemcpyHostToDevice, sim->stream));
     CU(cudaStreamSynchronize(sim->stream));
     if (grouped) { // largest per-cell count: sizes the tiles of the fused step
-        if (int rc = run_maxcount(s, 0, nullptr)) return rc;
+        if (int rc = run_maxcount(s, 0)) return rc;
         CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, sim->stream));
         CU(cudaStreamSynchronize(sim->stream));
         s->h_maxcount = h.maxcount;
@@ -474,10 +474,8 @@ extern "C" int pic_launch_count(pic_sim *sim, uint64_t *launches)
 // ------------------------------------------------------------------------------------------
 // arrange (split path): [histogram] -> scan -> destination-driven scatter [-> general path]
 // ------------------------------------------------------------------------------------------
-// guard: NULL = run; else a device flag, every kernel returns at once unless it is non-zero (the
-// fallback chain enqueued behind a fused step).  after_mover: a mover step ran since the last
-// fold, so the scan's fold also commits its speed bound.
-static int arrange_split(pic_species *s, bool hist_ready, const int *guard, bool after_mover)
+// after_mover: a mover step ran since the last fold, so the scan's fold also commits its speed bound.
+static int arrange_split(pic_species *s, bool hist_ready, bool after_mover)
 {
     pic_sim *sim = s->sim;
     const int nc = sim->nc;
@@ -492,7 +490,7 @@ static int arrange_split(pic_species *s, bool hist_ready, const int *guard, bool
             if (int rc = launch_check(sim, "hist_kernel")) return rc;
         }
     }
-    ScanFold fold{s->d_st, (s->reset_w || guard) ? 1 : 0, 1, after_mover ? 1 : 0, guard};
+    ScanFold fold{s->d_st, s->reset_w ? 1 : 0, 1, after_mover ? 1 : 0, nullptr};
     if (int rc = run_scan(s, s->d_count[on], s->d_off[on], nc, fold)) return rc;
 
     ScatterArgs a{};
@@ -501,7 +499,6 @@ static int arrange_split(pic_species *s, bool hist_ready, const int *guard, bool
     a.off_old = s->d_off[oo]; a.count_new = s->d_count[on]; a.off_new = s->d_off[on];
     a.st = s->d_st; a.nc = nc; a.periodic = sim->periodic;
     a.w_limit = FAST_W_LIMIT;
-    a.guard = guard;
     {
         long long want = ((long long)nc + SCATTER_THREADS / 32 - 1) / (SCATTER_THREADS / 32);
         int blocks = (int)std::min<long long>(want, (long long)sim->sm_count * 64);
@@ -522,7 +519,7 @@ static int arrange_split(pic_species *s, bool hist_ready, const int *guard, bool
         if (int rc = general_arrange(ga, sim->stream, sim->sm_count, &sim->launches)) return rc == PIC_ECUDA ? cuda_fail(cudaGetLastError(), "general_arrange") : rc;
     }
     if (s->sim->opt_fused && s->arrange_every == 1)
-        if (int rc = run_maxcount(s, on, guard)) return rc;
+        if (int rc = run_maxcount(s, on)) return rc;
 
     s->cur = dst;
     s->cur_off = on;
@@ -538,7 +535,7 @@ extern "C" int pic_arrange(pic_species *s)
 {
     if (!s) return PIC_EINVAL;
     if (int rc = verify_fused(s)) return rc;
-    return arrange_split(s, false, nullptr, false);
+    return arrange_split(s, false, false);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -550,37 +547,27 @@ static void launch_mover(pic_species *s, const MoverArgs &a, int blocks)
     mover_kernel<RC, H><<<blocks, MOVER_THREADS, 0, s->sim->stream>>>(a);
 }
 
-static int push_split(pic_species *s, bool will_arrange, const int *guard)
+static int push_split(pic_species *s, bool will_arrange)
 {
     pic_sim *sim = s->sim;
     const int nc = sim->nc;
     const int on = s->cur_off ^ 1;
-    if (will_arrange) {
-        if (guard) {
-            zero_guarded_kernel<<<sim->sm_count, 256, 0, sim->stream>>>(s->d_count[on], nc, guard);
-            if (int r = launch_check(sim, "zero_guarded_kernel")) return r;
-        } else {
-            CU(cudaMemsetAsync(s->d_count[on], 0, sizeof(int) * (size_t)nc, sim->stream));
-        }
-    }
+    if (will_arrange) CU(cudaMemsetAsync(s->d_count[on], 0, sizeof(int) * (size_t)nc, sim->stream));
     if (s->n_ub > 0) {
         MoverArgs a{};
         a.x = s->x[s->cur]; a.vx = s->vx[s->cur]; a.vy = s->vy[s->cur]; a.vz = s->vz[s->cur];
         a.cell = s->cell[s->cur];
-        a.E = sim->d_E; a.count = s->d_count[on]; a.st = s->d_st; a.k = s->k; a.guard = guard;
+        a.E = sim->d_E; a.count = s->d_count[on]; a.st = s->d_st; a.k = s->k;
         long long pairs = (s->n_ub + 1) / 2;
         int blocks = (int)((pairs + MOVER_THREADS - 1) / MOVER_THREADS);
-        if (guard) blocks = std::min(blocks, sim->sm_count * 8); // fallback behind a fused step: strides if it runs
         const bool rc = !s->all_live;
         KernelSpan span(sim, K_MOVER);
         if (rc) { if (will_arrange) launch_mover<true, true>(s, a, blocks); else launch_mover<true, false>(s, a, blocks); }
         else    { if (will_arrange) launch_mover<false, true>(s, a, blocks); else launch_mover<false, false>(s, a, blocks); }
         if (int r = launch_check(sim, "mover_kernel")) return r;
     }
-    if (!guard) {
-        s->h_wsum = std::min<long long>(s->h_wsum + host_step_bound(s), 1LL << 40);
-        s->h_steps_since_sync++;
-    }
+    s->h_wsum = std::min<long long>(s->h_wsum + host_step_bound(s), 1LL << 40);
+    s->h_steps_since_sync++;
     if (!sim->periodic) s->all_live = false;
     s->counts_fresh = false;
     if (!will_arrange) {
@@ -751,10 +738,10 @@ extern "C" int pic_push(pic_species *s, int nsteps)
             continue;
         }
         if (int rc = verify_fused(s)) return rc; // the split kernels need the true state (total step count unchanged)
-        if (int rc = push_split(s, will_arrange, nullptr)) return rc;
+        if (int rc = push_split(s, will_arrange)) return rc;
         s->steps++;
         if (will_arrange)
-            if (int rc = arrange_split(s, true, nullptr, true)) return rc;
+            if (int rc = arrange_split(s, true, true)) return rc;
     }
     return PIC_OK;
 }
