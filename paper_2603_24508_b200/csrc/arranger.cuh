@@ -75,6 +75,7 @@ struct ScatterArgs {
     const int *count_new; // nc
     const int *off_new;   // nc+1
     DevState *st;
+    const int *only_if; // if not NULL: the kernel returns at once unless *only_if != 0
     int nc, periodic, w_limit;
 };
 
@@ -102,6 +103,7 @@ __device__ __forceinline__ int scatter_range(const ScatterArgs &a, int c, int ba
 
 __global__ void __launch_bounds__(SCATTER_THREADS) scatter_fast_kernel(ScatterArgs a)
 {
+    if (a.only_if && !*a.only_if) return;
     const int W = a.st->w_acc;
     if (W > a.w_limit) {
         if (blockIdx.x == 0 && threadIdx.x == 0) a.st->need_general = 1;

@@ -14,6 +14,7 @@
 #include "scan.cuh"
 #include "arranger.cuh"
 #include "general.cuh"
+#include "tilesort.cuh"
 #include "fused.cuh"
 
 using namespace pic;
@@ -80,7 +81,7 @@ struct pic_sim {
     double Emax = 0; // max |E_node|
     std::vector<pic_species *> sp;
     unsigned long long launches = 0;
-    int opt_fused = 1, opt_timing = 0;
+    int opt_fused = 1, opt_timing = 0, opt_tile_scatter = 1;
     int opt_fused_cpc = 0, opt_fused_rows = 0, opt_fused_slots = 0, opt_fused_stages = 0; // tuning knobs of the fused step (0 = automatic)
     int sm_count = 148;
     // per-kernel device timing (option "kernel_timing"): event pairs recorded around launches
@@ -137,7 +138,7 @@ extern "C" size_t pic_workspace_bytes(int32_t nc, int64_t capacity)
 {
     (void)nc;
     if (capacity < 0) return 0;
-    return general_workspace_bytes((long long)capacity);
+    return std::max(general_workspace_bytes((long long)capacity), ts_workspace_bytes((long long)capacity));
 }
 
 static void free_species(pic_species *s)
@@ -427,7 +428,8 @@ extern "C" int pic_set_option(pic_sim *sim, const char *key, int value)
 {
     if (!sim || !key) return PIC_EINVAL;
     const bool flag = value == 0 || value == 1;
-    if (!strcmp(key, "kernel_timing") && flag) sim->opt_timing = value;
+    if (!strcmp(key, "tile_scatter") && flag) sim->opt_tile_scatter = value;
+    else if (!strcmp(key, "kernel_timing") && flag) sim->opt_timing = value;
     else if (!strcmp(key, "fused") && flag) sim->opt_fused = value;
     else if (!strcmp(key, "fused_cells_per_cta") && value >= 0 && value <= FUSED_CPC_MAX) sim->opt_fused_cpc = value;
     else if (!strcmp(key, "fused_stage_slots") && value >= 0 && value <= 512 && value % 2 == 0) sim->opt_fused_slots = value;
@@ -500,9 +502,29 @@ static int arrange_split(pic_species *s, bool hist_ready, bool after_mover)
     a.st = s->d_st; a.nc = nc; a.periodic = sim->periodic;
     a.w_limit = FAST_W_LIMIT;
     {
+        KernelSpan span(sim, K_SCATTER);
+        // tile-ranked stable scatter (tilesort.cuh) when the caller gave a workspace; the destination-driven
+        // scatter behind it runs only if a tile declined (or instead of it without a workspace)
+        const bool tiles = sim->opt_tile_scatter && s->ws && s->ws_bytes >= ts_workspace_bytes(s->n_ub) && s->n_ub > 0;
+        if (tiles) {
+            TileArgs t{};
+            t.sx = a.sx; t.svx = a.svx; t.svy = a.svy; t.svz = a.svz; t.scell = a.scell;
+            t.dx = a.dx; t.dvx = a.dvx; t.dvy = a.dvy; t.dvz = a.dvz; t.dcell = a.dcell;
+            t.off_old = a.off_old; t.off_new = a.off_new; t.st = s->d_st;
+            t.nc = nc; t.periodic = sim->periodic; t.w_limit = FAST_W_LIMIT;
+            const int nt = (int)ts_ntiles(s->n_ub);
+            t.tinfo = reinterpret_cast<int2 *>(s->ws);
+            t.thist = reinterpret_cast<int *>(static_cast<char *>(s->ws) + (((size_t)(nt + 1) * sizeof(int2) + 255) & ~(size_t)255));
+            tile_hist_kernel<<<nt, TS_THREADS, 0, sim->stream>>>(t);
+            if (int rc = launch_check(sim, "tile_hist_kernel")) return rc;
+            tile_base_kernel<<<(nc + 255) / 256, 256, 0, sim->stream>>>(t);
+            if (int rc = launch_check(sim, "tile_base_kernel")) return rc;
+            tile_scatter_kernel<<<nt, TS_THREADS, (TS_WARPS + 1) * TS_WIN * sizeof(int), sim->stream>>>(t);
+            if (int rc = launch_check(sim, "tile_scatter_kernel")) return rc;
+            a.only_if = &s->d_st->tile_declined;
+        }
         long long want = ((long long)nc + SCATTER_THREADS / 32 - 1) / (SCATTER_THREADS / 32);
         int blocks = (int)std::min<long long>(want, (long long)sim->sm_count * 64);
-        KernelSpan span(sim, K_SCATTER);
         scatter_fast_kernel<<<blocks, SCATTER_THREADS, 0, sim->stream>>>(a);
         if (int rc = launch_check(sim, "scatter_fast_kernel")) return rc;
     }

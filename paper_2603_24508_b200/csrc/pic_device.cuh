@@ -40,7 +40,7 @@ struct DevState {
     int ntiles, ntiles_next;         // tiles of the current partition (fused.cuh) / of the one being written
     int maxcount, maxcount_next;     // upper bound of the largest per-cell count: current state / step in flight
     int fail_step;                   // step id (FusedArgs::step_id) of the first fused step that declined
-    int pad[1];
+    int tile_declined;               // tilesort.cuh: a tile's window was too wide; scatter_fast_kernel takes the arrange
 };
 
 // Per-species Boris constants (computed once on the host) and grid.

@@ -44,6 +44,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_exclusive_kernel(const int 
         fold.st->step_max = 0;
         fold.st->need_general = 0;
         fold.st->used_general = 0;
+        fold.st->tile_declined = 0;
         if (fold.set_vmax) {
             fold.st->vmax2 = fold.st->vmax2_next;
             fold.st->vmax2_next = 0;

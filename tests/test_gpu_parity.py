@@ -14,6 +14,7 @@ pytestmark = pytest.mark.gpu
 
 VARIANTS = [
     pytest.param({"fused": 0}, id="split"),
+    pytest.param({"fused": 0, "tile_scatter": 0}, id="split-destscatter"),
     pytest.param({"fused": 1}, id="fused"),
     pytest.param({"fused": 1, "fused_stages": 2}, id="fused-2stage"),
 ]
@@ -330,3 +331,31 @@ def test_fused_declined_mid_run_is_redone_at_the_next_sync():
     pic.pic_push(sp, 5)
     st.push(5)
     compare(sp, st, where="after the switch to the split path", counts=True, nc=inp["nc"])
+
+
+@pytest.mark.parametrize("boundary", [workloads.PERIODIC, workloads.ABSORBING])
+def test_tile_scatter_declines_on_sparse_tiles(boundary):
+    """About one particle per cell: a tile of 2,048 slots spans more cells than a window holds, the
+    tile-ranked scatter declines and the destination-driven scatter takes the arrange (same result)."""
+    rng = np.random.default_rng(21)
+    nc = 6000
+    cell = np.sort(rng.integers(0, nc, 7000)).astype(np.int32)
+    x = cell + rng.random(len(cell))
+    x = np.where(np.floor(x) != cell, np.nextafter(cell + 1.0, 0), x)
+    v = 3.0 * rng.standard_normal((3, len(cell)))
+    E = rng.uniform(-0.2, 0.2, nc + 1)
+    if boundary == workloads.PERIODIC:
+        E[nc] = E[0]
+    inp = dict(nc=nc, dx=1.0, dt=0.1, boundary=boundary, E=E, B=np.array([1.0, 1.0, 0.0]), arrange_every=3,
+               species=[dict(qm=-1.0, x=x, vx=v[0], vy=v[1], vz=v[2], cell=cell)])
+    run_stepwise(inp, 12, options={"fused": 0})
+
+
+def test_tile_scatter_wraps_and_large_displacements():
+    """Periodic grid, arrange every 7 steps with fast particles: windows that straddle the ends of the grid."""
+    inp = workloads.make(5, nc=1024, n_total=200000)
+    inp["boundary"] = workloads.PERIODIC
+    inp["E"][inp["nc"]] = inp["E"][0]
+    inp["arrange_every"] = 7
+    sim, _ = run_stepwise(inp, 28, options={"fused": 0})
+    assert pic.pic_arrange_info(sim.species[0])[1] == 0
