@@ -229,25 +229,36 @@ __global__ void __launch_bounds__(TS_THREADS) tile_scatter_kernel(TileArgs a)
         }
     }
     __syncthreads();
-    // sweep B: rank inside the group in slot order, copy
+    // sweep B: rank inside the group in slot order, copy.  The source fields of four rows are loaded ahead of
+    // the ranking so that their latency overlaps it.
 #pragma unroll
-    for (int r = 0; r < TS_ROWS; ++r) {
-        const long long i = base + r * 32 + lane;
-        const unsigned live = __ballot_sync(FULL, bin[r] >= 0);
-        if (bin[r] >= 0) {
-            const unsigned m = __match_any_sync(live, bin[r]);
-            const int d = wc[bin[r]] + __popc(m & lt);
-            __syncwarp(live);
-            if ((m & lt) == 0) wc[bin[r]] += __popc(m);
-            int c = cmin + bin[r];
-            if (c >= a.nc) c -= a.nc;
-            a.dx[d] = a.sx[i];
-            a.dvx[d] = a.svx[i];
-            a.dvy[d] = a.svy[i];
-            a.dvz[d] = a.svz[i];
-            a.dcell[d] = c;
+    for (int r0 = 0; r0 < TS_ROWS; r0 += 4) {
+        double x[4], vx[4], vy[4], vz[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const long long i = base + (r0 + q) * 32 + lane;
+            if (bin[r0 + q] >= 0) { x[q] = a.sx[i]; vx[q] = a.svx[i]; vy[q] = a.svy[i]; vz[q] = a.svz[i]; }
+            else { x[q] = vx[q] = vy[q] = vz[q] = 0.0; }
         }
-        __syncwarp();
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int bq = bin[r0 + q];
+            const unsigned live = __ballot_sync(FULL, bq >= 0);
+            if (bq >= 0) {
+                const unsigned m = __match_any_sync(live, bq);
+                const int d = wc[bq] + __popc(m & lt);
+                __syncwarp(live);
+                if ((m & lt) == 0) wc[bq] += __popc(m);
+                int c = cmin + bq;
+                if (c >= a.nc) c -= a.nc;
+                a.dx[d] = x[q];
+                a.dvx[d] = vx[q];
+                a.dvy[d] = vy[q];
+                a.dvz[d] = vz[q];
+                a.dcell[d] = c;
+            }
+            __syncwarp();
+        }
     }
 }
 
