@@ -34,6 +34,8 @@ def lib():
                                     C.c_int32, C.c_double, C.c_double, C.c_int32, dp, C.c_double, dp, u64p,
                                     ip, ip]
         _lib.oracle_run.restype = C.c_int
+        _lib.oracle_deposit.argtypes = [C.c_int64, dp, ip, C.c_int32, C.c_double, C.c_int32, C.c_double, dp]
+        _lib.oracle_deposit.restype = C.c_int
     return _lib
 
 
@@ -118,10 +120,25 @@ class State:
             dst[:nl] = src[:nl]
         self.n = int(nl)
 
+    def deposit(self, weight=1.0):
+        """charge density on the nc+1 nodes from the current state (oracle_deposit)."""
+        return deposit(self.x[:self.n], self.cell[:self.n], self.nc, self.dx, self.boundary, weight)
+
     def live(self):
         """the five arrays over [0,n)."""
         n = self.n
         return self.x[:n], self.vx[:n], self.vy[:n], self.vz[:n], self.cell[:n]
+
+
+def deposit(x, cell, nc, dx, boundary, weight=1.0):
+    """oracle_deposit -> rho on nc+1 nodes."""
+    xa = np.ascontiguousarray(x, dtype=np.float64)
+    ca = np.ascontiguousarray(cell, dtype=np.int32)
+    rho = np.zeros(nc + 1)
+    rc = lib().oracle_deposit(len(xa), _d(xa), _i(ca), int(nc), float(dx), int(boundary), float(weight), _d(rho))
+    if rc:
+        raise RuntimeError(f"oracle_deposit failed rc={rc}")
+    return rho
 
 
 def arrange_arrays(x, vx, vy, vz, cell, nc):

@@ -216,3 +216,43 @@ int oracle_run(int32_t nsteps, int32_t arrange_every, int64_t *step_count, int64
     }
     return 0;
 }
+
+/* Charge deposition, phase (ii) of the PIC cycle ("deposition to the grid, which maps particle
+ * charges and currents to the mesh"), with the same linear (cloud-in-cell) weighting
+ * as the gather (BASELINE.json north_star).  The paper prints no
+ * formula; the reading (S20-S22): node j of nc+1 nodes receives
+ *     rho[j] = weight * ( sum over live particles in cell j   of (1 - w_i)
+ *                       + sum over live particles in cell j-1 of  w_i     ),
+ * with xs = x*inv_dx, jf = floor(xs) (clamped to nc-1 as in the mover, reading S8), w = xs - jf;
+ * `weight` (charge per macro-particle over dx, sign included) is the caller's business; on a
+ * periodic grid nodes 0 and nc are the same point and both carry the sum of the two; at
+ * absorbing walls the boundary nodes keep their half-cell sums (no correction).  Particles are
+ * visited in index order, each adding (1-w) to node j and then w to node j+1; the node sums are
+ * multiplied by weight at the end.  Flagged-dead particles (cell < 0) are skipped.
+ * Pins (tests/test_oracle_deposit.py): single particle, total charge, first moment (dipole),
+ * one particle per cell centre, linearity, periodic fold, numpy.add.at brute force. */
+int oracle_deposit(int64_t n, const double *x, const int32_t *cell, int32_t nc, double dx,
+                   int32_t boundary, double weight, double *rho)
+{
+    if (n < 0 || nc < 1 || !(dx > 0.0)) return -1;
+    const double inv_dx = 1.0 / dx;
+    for (int32_t j = 0; j <= nc; ++j) rho[j] = 0.0;
+    for (int64_t i = 0; i < n; ++i) {
+        if (cell[i] < 0) continue;
+        const double xs = x[i] * inv_dx;
+        double jf = floor(xs);
+        if (!(jf >= 0.0) || jf > (double)nc) return -2;
+        int32_t j = (int32_t)jf;
+        if (j > nc - 1) { j = nc - 1; jf = (double)j; }
+        const double w = xs - jf;
+        const double w0 = 1.0 - w;
+        rho[j] = rho[j] + w0;
+        rho[j + 1] = rho[j + 1] + w;
+    }
+    if (boundary == ORACLE_PERIODIC) {
+        rho[0] = rho[0] + rho[nc];
+        rho[nc] = rho[0];
+    }
+    for (int32_t j = 0; j <= nc; ++j) rho[j] = rho[j] * weight;
+    return 0;
+}
