@@ -125,6 +125,18 @@ int pic_arrange(pic_species *sp);
  * arranger was needed but the workspace is too small). */
 int pic_wall_flux(pic_species *sp, pic_wall_flux_t *out);
 
+/* Charge deposition on the arranged state: PIC phase (ii), "deposition to the grid, which maps
+ * particle charges ... to the mesh", with the linear (cloud-in-cell) weights of the
+ * gather.  rho_dev: DEVICE, nc+1 doubles, caller-owned:
+ *   rho[j] (+)= weight * ( sum over particles in cell j of (1-w) + sum over particles in cell j-1 of w ),
+ * w = x/dx - floor(x/dx); on a periodic grid nodes 0 and nc carry the same (summed) value; no
+ * correction at absorbing walls.  weight: charge per macro-particle over dx, sign included.
+ * accumulate: 0 overwrites rho, 1 adds to it (several species).  Asynchronous on the stream, except
+ * that unchecked fused steps are checked first (which syncs).  PIC_ESTATE unless the state is
+ * arranged (right after an arranging step or pic_arrange): the reduction runs per cell over the
+ * arranged slots.  Deterministic (fixed summation tree); agrees with a sequential sum to rounding. */
+int pic_deposit(pic_species *sp, double weight, double *rho_dev, int accumulate);
+
 /* Replace E (HOST, nc+1 doubles, copied; stream-ordered). */
 int pic_set_field(pic_sim *sim, const double *E_nodes_host);
 
@@ -176,7 +188,7 @@ int pic_set_option(pic_sim *sim, const char *key, int value);
 /* Device time of one kernel class since the previous query of that class, measured with CUDA
  * event pairs recorded on the sim's stream around each of its launches while option
  * "kernel_timing" is 1 (default 0: nothing is recorded).  kernel is one of "mover", "hist",
- * "scan", "scatter", "general", "fused".  *ms_total = summed milliseconds, *spans = number of
+ * "scan", "scatter", "general", "fused", "deposit".  *ms_total = summed milliseconds, *spans = number of
  * timed launches (either may be NULL).  Syncs.  PIC_EINVAL for an unknown name. */
 int pic_kernel_time(pic_sim *sim, const char *kernel, double *ms_total, uint64_t *spans);
 

@@ -21,7 +21,7 @@ EXPORTS = [
     "pic_create", "pic_species_at", "pic_push", "pic_arrange", "pic_wall_flux", "pic_set_field", "pic_n_slots",
     "pic_active_buffer", "pic_cell_counts", "pic_step_count", "pic_arrange_info", "pic_workspace_bytes",
     "pic_set_option", "pic_launch_count", "pic_sync", "pic_destroy", "pic_strerror", "pic_last_error",
-    "pic_run_host", "pic_kernel_time", "pic_fused_info",
+    "pic_run_host", "pic_kernel_time", "pic_fused_info", "pic_deposit",
 ]
 
 
@@ -89,6 +89,7 @@ def lib():
         L.pic_launch_count.argtypes = [vp, C.POINTER(C.c_uint64)]
         L.pic_kernel_time.argtypes = [vp, C.c_char_p, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
         L.pic_fused_info.argtypes = [vp, i32p, i32p, i32p, i32p]
+        L.pic_deposit.argtypes = [vp, C.c_double, vp, C.c_int]
         L.pic_sync.argtypes = [vp]
         L.pic_destroy.argtypes = [vp]
         L.pic_destroy.restype = None
@@ -138,8 +139,8 @@ class Species:
 class Sim:
     """Handle of a simulation (pic_sim*)."""
 
-    def __init__(self, handle, species, keep):
-        self.handle, self.species, self._keep = handle, species, keep
+    def __init__(self, handle, species, keep, nc=None, stream=None):
+        self.handle, self.species, self._keep, self.nc, self.stream = handle, species, keep, nc, stream
 
     def __del__(self):
         try:
@@ -203,7 +204,7 @@ def pic_create(*, nc, dx, dt, boundary, E_nodes, B, species, stream=None):
     torch.cuda.current_stream().synchronize()  # uploads in make_species ran on torch's current stream
     h = C.c_void_p()
     _check(lib().pic_create(C.byref(g), descs, len(species), C.byref(h)), "pic_create")
-    sim = Sim(h, [], keep)
+    sim = Sim(h, [], keep, nc=int(nc), stream=stream)
     for i, s in enumerate(species):
         sim.species.append(Species(sim, C.c_void_p(lib().pic_species_at(h, i)), s["bufs"], wss[i]))
     return sim
@@ -262,6 +263,18 @@ def pic_arrange_info(sp):
     w, g = C.c_int32(), C.c_int32()
     _check(lib().pic_arrange_info(sp.handle, C.byref(w), C.byref(g)), "pic_arrange_info")
     return w.value, g.value
+
+
+def pic_deposit(sp, weight, rho=None, accumulate=False):
+    """pic_deposit: charge density on the nc+1 nodes (torch float64 device tensor; allocated if None)."""
+    import torch
+    nc = sp.sim.nc
+    if rho is None:
+        rho = torch.zeros(nc + 1, dtype=torch.float64, device=sp.bufs[0][0].device)
+        sp.sim.stream.wait_stream(torch.cuda.current_stream())
+    assert rho.dtype == torch.float64 and rho.numel() == nc + 1 and rho.is_contiguous()
+    _check(lib().pic_deposit(sp.handle, float(weight), C.c_void_p(rho.data_ptr()), 1 if accumulate else 0), "pic_deposit")
+    return rho
 
 
 def pic_fused_info(sp):

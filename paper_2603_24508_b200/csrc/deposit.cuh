@@ -1,0 +1,64 @@
+// deposit.cuh -- charge deposition on the arranged state (PIC phase (ii); SURVEY.md
+// section 8(f) rank 1): linear (cloud-in-cell) weights, the transpose of the
+// mover's gather.  Because the particles of cell c occupy the slots [offset[c], offset[c+1]) the
+// scatter-add becomes a segmented reduction: one warp per cell sums (1-w) and w over its particles
+// (lane-strided partial sums, then a fixed shuffle tree: no atomics, bitwise deterministic), and one
+// thread per node adds the two cells that touch it.  8 B read per particle.
+#pragma once
+#include "pic_device.cuh"
+
+namespace pic {
+
+constexpr int DEP_THREADS = 256;
+
+struct DepositArgs {
+    const double *x;
+    const int *off;  // nc+1 offsets of the arranged state
+    double2 *cs;     // per cell: {sum (1-w), sum w}
+    int nc;
+    double inv_dx;
+};
+
+__global__ void __launch_bounds__(DEP_THREADS) deposit_cell_kernel(DepositArgs a)
+{
+    const int lane = threadIdx.x & 31;
+    const long long c = ((long long)blockIdx.x * DEP_THREADS + threadIdx.x) >> 5;
+    if (c >= a.nc) return;
+    const int s0 = a.off[c], s1 = a.off[c + 1];
+    const double cf = (double)c; // = floor(x*inv_dx), clamped to nc-1, for every particle of the cell (invariant)
+    double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
+    int i = s0 + lane;
+    for (; i + 32 < s1; i += 64) { // two loads in flight per lane
+        const double xa = a.x[i], xb = a.x[i + 32];
+        const double wa = __dsub_rn(__dmul_rn(xa, a.inv_dx), cf), wb = __dsub_rn(__dmul_rn(xb, a.inv_dx), cf);
+        a0 += 1.0 - wa; a1 += wa;
+        b0 += 1.0 - wb; b1 += wb;
+    }
+    if (i < s1) {
+        const double w = __dsub_rn(__dmul_rn(a.x[i], a.inv_dx), cf);
+        a0 += 1.0 - w; a1 += w;
+    }
+    a0 += b0; a1 += b1;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a0 += __shfl_xor_sync(FULL, a0, o);
+        a1 += __shfl_xor_sync(FULL, a1, o);
+    }
+    if (lane == 0) a.cs[c] = make_double2(a0, a1);
+}
+
+// rho[j] = weight * (sum (1-w) over cell j + sum w over cell j-1); nodes 0 and nc of a periodic grid are one
+// point and carry the same sum.  accumulate: add to rho instead of overwriting it (several species).
+__global__ void deposit_node_kernel(const double2 *__restrict__ cs, int nc, int periodic, double weight, int accumulate,
+                                    double *__restrict__ rho)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j > nc) return;
+    double v;
+    if (periodic && (j == 0 || j == nc)) v = cs[0].x + cs[nc - 1].y;
+    else v = (j < nc ? cs[j].x : 0.0) + (j > 0 ? cs[j - 1].y : 0.0);
+    const double out = __dmul_rn(v, weight);
+    rho[j] = accumulate ? rho[j] + out : out;
+}
+
+} // namespace pic

@@ -15,6 +15,7 @@
 #include "arranger.cuh"
 #include "general.cuh"
 #include "tilesort.cuh"
+#include "deposit.cuh"
 #include "fused.cuh"
 
 using namespace pic;
@@ -32,8 +33,8 @@ static int cuda_fail(cudaError_t e, const char *what)
         if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
     } while (0)
 
-enum { K_MOVER = 0, K_HIST, K_SCAN, K_SCATTER, K_GENERAL, K_FUSED, K_COUNT };
-static const char *const K_NAMES[K_COUNT] = {"mover", "hist", "scan", "scatter", "general", "fused"};
+enum { K_MOVER = 0, K_HIST, K_SCAN, K_SCATTER, K_GENERAL, K_FUSED, K_DEPOSIT, K_COUNT };
+static const char *const K_NAMES[K_COUNT] = {"mover", "hist", "scan", "scatter", "general", "fused", "deposit"};
 
 struct pic_species {
     pic_sim *sim = nullptr;
@@ -50,6 +51,7 @@ struct pic_species {
     unsigned long long *d_scan = nullptr;
     size_t scan_words = 0;
     // fused push+arrange step (fused.cuh)
+    double2 *d_cs = nullptr;           // deposition: per-cell partial sums (allocated at the first pic_deposit)
     int h_maxcount = 0;                // bound of the largest per-cell count at the last sync (sizes the fused tiles)
     int h_abort_reason = 0;
     bool fused_off = false;            // the device reported a declined fused step (sticky)
@@ -147,6 +149,7 @@ static void free_species(pic_species *s)
     cudaFree(s->d_st);
     for (int b = 0; b < 2; ++b) { cudaFree(s->d_count[b]); cudaFree(s->d_off[b]); }
     cudaFree(s->d_scan);
+    cudaFree(s->d_cs);
     delete s;
 }
 
@@ -838,6 +841,31 @@ extern "C" int pic_cell_counts(pic_species *s, int32_t *count_host, int32_t *off
         CU(cudaMemcpyAsync(offset_host, s->d_off[s->cur_off], sizeof(int) * ((size_t)nc + 1), cudaMemcpyDeviceToHost, s->sim->stream));
     CU(cudaStreamSynchronize(s->sim->stream));
     return PIC_OK;
+}
+
+extern "C" int pic_deposit(pic_species *s, double weight, double *rho_dev, int accumulate)
+{
+    if (!s || !rho_dev || !std::isfinite(weight)) return PIC_EINVAL;
+    if (int rc = verify_fused(s)) return rc;
+    if (!s->counts_fresh || !s->all_live) return PIC_ESTATE;
+    pic_sim *sim = s->sim;
+    const int nc = sim->nc;
+    if (!s->d_cs) {
+        cudaError_t e = cudaMalloc(&s->d_cs, sizeof(double2) * (size_t)nc);
+        if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? PIC_ENOMEM : cuda_fail(e, "cudaMalloc deposition sums");
+    }
+    DepositArgs a{};
+    a.x = s->x[s->cur];
+    a.off = s->d_off[s->cur_off];
+    a.cs = s->d_cs;
+    a.nc = nc;
+    a.inv_dx = s->k.inv_dx;
+    KernelSpan span(sim, K_DEPOSIT);
+    const long long threads = (long long)nc * 32;
+    deposit_cell_kernel<<<(unsigned)((threads + DEP_THREADS - 1) / DEP_THREADS), DEP_THREADS, 0, sim->stream>>>(a);
+    if (int rc = launch_check(sim, "deposit_cell_kernel")) return rc;
+    deposit_node_kernel<<<(nc + 1 + 255) / 256, 256, 0, sim->stream>>>(s->d_cs, nc, sim->periodic, weight, accumulate ? 1 : 0, rho_dev);
+    return launch_check(sim, "deposit_node_kernel");
 }
 
 extern "C" int pic_arrange_info(pic_species *s, int32_t *w_bound, int32_t *used_general)

@@ -359,3 +359,72 @@ def test_tile_scatter_wraps_and_large_displacements():
     inp["arrange_every"] = 7
     sim, _ = run_stepwise(inp, 28, options={"fused": 0})
     assert pic.pic_arrange_info(sim.species[0])[1] == 0
+
+
+DEP_RTOL = 1e-12  # north_star tolerance; the GPU sums each cell with a fixed tree, the oracle sequentially
+
+
+def _check_deposit(sp, st, weight, where):
+    rho = pic.pic_deposit(sp, weight).cpu().numpy()
+    ref = st.deposit(weight)
+    scale = np.maximum(np.abs(ref), abs(weight))
+    assert np.all(np.abs(rho - ref) <= DEP_RTOL * scale), f"{where}: deposition differs, max {np.max(np.abs(rho - ref) / scale)}"
+    return rho
+
+
+@pytest.mark.parametrize("config,kw,fused", [(1, {}, 1), (2, dict(nc=2048), 1), (4, dict(nc=4099), 0), (5, dict(nc=4096), 1)])
+def test_deposit_matches_oracle(config, kw, fused):
+    """pic_deposit on the arranged state after every arranging step: all nodes within 1e-12 relative
+    (to max(|rho_j|, |weight|)); total charge = weight * n_live."""
+    inp = workloads.make(config, **kw)
+    sim, states = make_pair(inp, options={"fused": fused})
+    ae = inp["arrange_every"]
+    for step in range(1, 21):
+        for sp, st in zip(sim.species, states):
+            pic.pic_push(sp, 1)
+            st.push(1)
+        if step % ae == 0:
+            for sp, st in zip(sim.species, states):
+                rho = _check_deposit(sp, st, -0.75, f"config {config} step {step}")
+                tot = rho[:-1].sum() if inp["boundary"] == workloads.PERIODIC else rho.sum()
+                assert abs(tot - (-0.75) * st.n) <= 1e-10 * 0.75 * st.n
+    pic.pic_sync(sim)
+
+
+def test_deposit_two_species_accumulate_and_state_errors():
+    inp = workloads.make(3, nc=1000)
+    sim, states = make_pair(inp)
+    for sp, st in zip(sim.species, states):
+        pic.pic_push(sp, 3)
+        st.push(3)
+    rho = pic.pic_deposit(sim.species[0], -1.0)
+    rho = pic.pic_deposit(sim.species[1], +1.0, rho=rho, accumulate=True).cpu().numpy()
+    ref = states[0].deposit(-1.0) + states[1].deposit(+1.0)
+    scale = np.maximum(np.abs(states[0].deposit(-1.0)), 1.0)
+    assert np.all(np.abs(rho - ref) <= 1e-12 * scale)
+    # not arranged -> PIC_ESTATE
+    inp5 = workloads.make(5, nc=512)
+    sim5, _ = make_pair(inp5)
+    pic.pic_push(sim5.species[0], 1)
+    with pytest.raises(pic.PicError) as e:
+        pic.pic_deposit(sim5.species[0], 1.0)
+    assert e.value.status == pic.PIC_ESTATE
+
+
+def test_deposit_empty_cells_tiny_and_dx():
+    rng = np.random.default_rng(13)
+    nc, dx = 40, 0.37
+    cell = np.sort(rng.choice(nc, size=25, replace=True)).astype(np.int32)
+    x = (cell + rng.random(len(cell))) * dx
+    ok = np.minimum(np.floor(x * (1.0 / dx)), nc - 1) == cell
+    x, cell = x[ok], cell[ok]
+    v = rng.standard_normal((3, len(x)))
+    for boundary in (workloads.PERIODIC, workloads.ABSORBING):
+        E = np.zeros(nc + 1)
+        inp = dict(nc=nc, dx=dx, dt=0.05, boundary=boundary, E=E, B=np.array([0.0, 1.0, 0.0]), arrange_every=1,
+                   species=[dict(qm=-1.0, x=x, vx=v[0], vy=v[1], vz=v[2], cell=cell)])
+        sim, (st,) = make_pair(inp)
+        _check_deposit(sim.species[0], st, 2.5, "initial state")
+        pic.pic_push(sim.species[0], 4)
+        st.push(4)
+        _check_deposit(sim.species[0], st, 2.5, "after 4 steps")
