@@ -47,6 +47,7 @@ FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 #   scatter : read all five (36), write all five (36)
 #   fused   : read x,vx,vy,vz (32), write all five (36)
 ALG_BYTES = {"mover": (68, 72), "scatter": (72, 72), "fused": (68, 68), "hist": (4, 4)}
+DEPOSIT_BYTES = 8  # pic_deposit reads x only
 
 
 def env_rank():
@@ -211,6 +212,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the CPU-oracle baseline leg")
+    ap.add_argument("--no-deposit", action="store_true", help="skip the separate timing of pic_deposit")
     ap.add_argument("--option", action="append", default=[], help="pic_set_option key=value (e.g. fused=0)")
     ap.add_argument("--scale", type=float, default=1.0, help="scale nc (debug only; the line is then not a bench value)")
     args = ap.parse_args()
@@ -312,6 +314,22 @@ def main():
                         if k in ALG_BYTES and v[1] and v[0] * 1e-3 / v[1] > 0.1 * ALG_BYTES[k][0] * n_per_launch / (peak * 1e9)
                     ) / (ms * 1e-3) / 1e9}
         roofline["step_frac"] = roofline["step_algorithmic_GBps"] / peak
+    # the next row of the path, measured beside the step, outside its timed region:
+    # charge deposition on the arranged state, 20 calls per species, device time from the library's event pairs
+    deposit = None
+    if ae == 1 and not args.no_deposit:
+        pic.pic_kernel_time(sim, "deposit")
+        rho = None
+        for _ in range(20):
+            for si, sp in enumerate(sim.species):
+                rho = pic.pic_deposit(sp, -1.0 if si == 0 else 1.0, rho=rho, accumulate=si > 0)
+        dms, dn = pic.pic_kernel_time(sim, "deposit")
+        if dn:
+            d_ms = dms / dn
+            d_gbs = DEPOSIT_BYTES * n_per_launch / (d_ms * 1e-3) / 1e9
+            deposit = {"ms_per_call": d_ms, "calls": int(dn), "algorithmic_bytes_per_particle": DEPOSIT_BYTES,
+                       "achieved": d_gbs, "unit": "GB/s", "frac": d_gbs / peak, "particles_per_call": n_per_launch,
+                       "total_charge_check": float(rho[:-1].sum().item() if all_live else rho.sum().item())}
     pic.pic_destroy(sim)
     del descs, sim
     torch.cuda.empty_cache()
@@ -359,7 +377,7 @@ def main():
                 "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic", "config": workload_config(args.config, inp),
                 "clocks": sampler.result(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-                "cpu_baseline": cpu,
+                "cpu_baseline": cpu, "deposit": deposit,
                 "path": {"arranger": ["general" if g else "fast" for (_, g) in info],
                          "options": args.option, "numpy": np.__version__}}
         if args.scale != 1.0:

@@ -26,19 +26,21 @@ __global__ void __launch_bounds__(DEP_THREADS) deposit_cell_kernel(DepositArgs a
     if (c >= a.nc) return;
     const int s0 = a.off[c], s1 = a.off[c + 1];
     const double cf = (double)c; // = floor(x*inv_dx), clamped to nc-1, for every particle of the cell (invariant)
-    double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
-    int i = s0 + lane;
-    for (; i + 32 < s1; i += 64) { // two loads in flight per lane
-        const double xa = a.x[i], xb = a.x[i + 32];
-        const double wa = __dsub_rn(__dmul_rn(xa, a.inv_dx), cf), wb = __dsub_rn(__dmul_rn(xb, a.inv_dx), cf);
-        a0 += 1.0 - wa; a1 += wa;
-        b0 += 1.0 - wb; b1 += wb;
+    double a0 = 0.0, a1 = 0.0;
+    // four loads in flight per lane: a cell of up to 128 particles is fetched in one round trip
+    for (int i = s0 + lane; i < s1; i += 128) {
+        double xv[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) xv[q] = i + 32 * q < s1 ? a.x[i + 32 * q] : 0.0;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            if (i + 32 * q < s1) {
+                const double w = __dsub_rn(__dmul_rn(xv[q], a.inv_dx), cf);
+                a0 += 1.0 - w;
+                a1 += w;
+            }
+        }
     }
-    if (i < s1) {
-        const double w = __dsub_rn(__dmul_rn(a.x[i], a.inv_dx), cf);
-        a0 += 1.0 - w; a1 += w;
-    }
-    a0 += b0; a1 += b1;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         a0 += __shfl_xor_sync(FULL, a0, o);
