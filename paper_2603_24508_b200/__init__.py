@@ -271,9 +271,10 @@ def pic_deposit(sp, weight, rho=None, accumulate=False):
     nc = sp.sim.nc
     if rho is None:
         rho = torch.zeros(nc + 1, dtype=torch.float64, device=sp.bufs[0][0].device)
-        sp.sim.stream.wait_stream(torch.cuda.current_stream())
+    sp.sim.stream.wait_stream(torch.cuda.current_stream())
     assert rho.dtype == torch.float64 and rho.numel() == nc + 1 and rho.is_contiguous()
     _check(lib().pic_deposit(sp.handle, float(weight), C.c_void_p(rho.data_ptr()), 1 if accumulate else 0), "pic_deposit")
+    torch.cuda.current_stream().wait_stream(sp.sim.stream)  # rho is produced on the sim's stream
     return rho
 
 

@@ -47,6 +47,11 @@ def test_fullsize_first_steps_elementwise(config, steps, check_every):
     pic.pic_sync(sim)
     for sp in sim.species:
         assert pic.pic_arrange_info(sp)[1] == 0, "full-size run fell to the general arranger"
+    if steps % ae == 0:  # arranged state: charge deposition at full size against the oracle (1e-12)
+        for sp, st in zip(sim.species, states):
+            rho = pic.pic_deposit(sp, -1.0).cpu().numpy()
+            ref = st.deposit(-1.0)
+            assert np.all(np.abs(rho - ref) <= 1e-12 * np.maximum(np.abs(ref), 1.0)), f"config {config}: deposition differs"
     pic.pic_destroy(sim)
 
 

@@ -428,3 +428,18 @@ def test_deposit_empty_cells_tiny_and_dx():
         pic.pic_push(sim.species[0], 4)
         st.push(4)
         _check_deposit(sim.species[0], st, 2.5, "after 4 steps")
+
+
+def test_neutral_species_qm_zero():
+    """Neutral species (`nmove` / `narrj`) are the same kernels with q/m = 0: ballistic motion,
+    same arranger; three species side by side as in the paper's ionisation case (e-, D+, D)."""
+    inp = workloads.make(3, nc=600)
+    neutral = dict(inp["species"][1])
+    neutral["qm"] = 0.0
+    neutral["name"] = "D"
+    inp["species"].append(neutral)
+    sim, states = run_stepwise(inp, 20, check_every=5)
+    v0 = neutral["vx"]
+    assert np.array_equal(np.sort(states[2].vx[:states[2].n]), np.sort(v0)[:states[2].n]) or states[2].n < len(v0)
+    for sp in sim.species:
+        assert pic.pic_fused_info(sp)["decline_reasons"] == 0

@@ -358,3 +358,22 @@ def test_single_call_equals_step_by_step():
     for p, q in zip(a.live(), b.live()):
         assert np.array_equal(p, q)
     assert np.array_equal(a.wall, b.wall)
+
+
+def test_neutral_species_is_ballistic():
+    """q/m = 0 (the paper's neutral species, `nmove`): no gather, no rotation -- v is untouched
+    bit for bit and x advances by the separately rounded product vx*dt each step, whatever E and B are."""
+    rng = np.random.default_rng(77)
+    nc, n, dt = 50, 300, 0.1
+    x0 = rng.random(n) * nc
+    v0 = rng.standard_normal((3, n))
+    cell = np.floor(x0).astype(np.int32)
+    st = oracle.State(x0, v0[0], v0[1], v0[2], cell, nc=nc, dx=1.0, dt=dt, boundary=oracle.PERIODIC,
+                      E=rng.uniform(-5, 5, nc + 1), qm=0.0, B=np.array([3.0, -2.0, 7.0]), arrange_every=0)
+    x = x0.copy()
+    for _ in range(25):
+        st.push_only()
+        x = x + v0[0] * dt
+        x = np.where(x >= nc, x - nc, np.where(x < 0, x + nc, x))
+    assert np.array_equal(st.vx, v0[0]) and np.array_equal(st.vy, v0[1]) and np.array_equal(st.vz, v0[2])
+    assert np.array_equal(st.x, x)
