@@ -311,7 +311,7 @@ __device__ __forceinline__ void fused_issue(const FusedArgs &a, const FusedCtx &
 template <bool PERIODIC, bool EDGE, int RMAX, int R0, int CNT>
 __device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *px, const double *sEs, const int2 *cellinfo, int lane,
                                               int pad, int n, int cA, int ncell, double (&X_)[RMAX], double (&VX_)[RMAX],
-                                              double (&VY_)[RMAX], double (&VZ_)[RMAX], int (&W_)[RMAX], int &hmax)
+                                              double (&VY_)[RMAX], double (&VZ_)[RMAX], int (&W_)[RMAX])
 {
     constexpr int CAP = RMAX * 32;
     const int nc = k.nc;
@@ -375,9 +375,6 @@ __device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *
         }
         const bool good = valid && inr && inside && (g < 3 || legit);
         if (!good) g = 3;
-        // speed bound for the split path's displacement estimate: largest high word of |v| components
-        const int hv = max(max(__double2hiint(nvx) & 0x7fffffff, __double2hiint(wy) & 0x7fffffff), __double2hiint(wz) & 0x7fffffff);
-        hmax = max(hmax, (valid && inr) ? hv : 0);
         W_[r] = g | ((j - cA) << 2) | ((valid && !good) ? 256 : 0);
         X_[r] = xw; VX_[r] = nvx; VY_[r] = wy; VZ_[r] = wz;
     }
@@ -388,10 +385,10 @@ __device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *
 template <bool PERIODIC, bool EDGE, int RMAX>
 __device__ __forceinline__ void fused_sweep1a_all(const PushConst &k, const double *px, const double *sEs, const int2 *cellinfo, int lane,
                                                   int pad, int n, int nrows, int cA, int ncell, double (&X_)[RMAX], double (&VX_)[RMAX],
-                                                  double (&VY_)[RMAX], double (&VZ_)[RMAX], int (&W_)[RMAX], int &hmax)
+                                                  double (&VY_)[RMAX], double (&VZ_)[RMAX], int (&W_)[RMAX])
 {
 #define FUSED_ROWS(R0, CNT) \
-    if (R0 < nrows) fused_sweep1a<PERIODIC, EDGE, RMAX, R0, CNT>(k, px, sEs, cellinfo, lane, pad, n, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
+    if (R0 < nrows) fused_sweep1a<PERIODIC, EDGE, RMAX, R0, CNT>(k, px, sEs, cellinfo, lane, pad, n, cA, ncell, X_, VX_, VY_, VZ_, W_);
     FUSED_ROWS(0, 4)
     if (RMAX == 8) {
         FUSED_ROWS(4, 2) FUSED_ROWS(6, 1) FUSED_ROWS(7, 1)
@@ -425,7 +422,6 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
     const int nc = a.k.nc;
     int bad = 0;  // FA_* bits
     int mc = 0;   // largest new per-cell count seen by this lane
-    int hmax = 0; // largest high word of the |v'| components seen by this lane
 
     if (!*(volatile int *)&st->abort) {
         FusedCtx X;
@@ -495,8 +491,8 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
             // ---- sweep 1a: push into registers and classify (fused_sweep1a) ----------------------------------
             double X_[RMAX], VX_[RMAX], VY_[RMAX], VZ_[RMAX];
             int W_[RMAX]; // 1a: class | cell << 2 | bad << 8;  1b: -1, or class prefix count << 8 | class*32 + cell
-            if (cA == 0 || cB == nc) fused_sweep1a_all<PERIODIC, true, RMAX>(a.k, px, sEs, cellinfo, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
-            else fused_sweep1a_all<PERIODIC, false, RMAX>(a.k, px, sEs, cellinfo, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_, hmax);
+            if (cA == 0 || cB == nc) fused_sweep1a_all<PERIODIC, true, RMAX>(a.k, px, sEs, cellinfo, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_);
+            else fused_sweep1a_all<PERIODIC, false, RMAX>(a.k, px, sEs, cellinfo, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_);
             __syncwarp();
             // the stage has been read: refill it with the next item to load
             if (lane == 0) fused_issue(a, X, two ? I2 : I1, px, odd ? mb1 : mb0);
@@ -636,16 +632,11 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
     // ---- CTA epilogue; the last CTA commits or rolls back the step ----------------------------------
     bad = (int)__reduce_or_sync(FULL, (unsigned)bad);
     mc = __reduce_max_sync(FULL, mc);
-    // |v'|^2 <= 3 b^2 with b the smallest double whose high word exceeds every component's
-    hmax = __reduce_max_sync(FULL, hmax);
-    const double vb = __hiloint2double(hmax + 1, 0);
-    const unsigned vmw = hmax ? __float_as_uint(__double2float_ru(3.0 * vb * vb)) : 0u;
     if (lane == 0) {
         if (bad) {
             atomicExch(&st->abort, 1);
             atomicOr(&st->abort_reason, bad);
         }
-        if (vmw > *(volatile unsigned *)&st->vmax2_next) atomicMax(&st->vmax2_next, vmw);
         if (mc > *(volatile int *)&st->maxcount_next) atomicMax(&st->maxcount_next, mc);
         __threadfence();
         const unsigned d = atomicAdd(&st->done, 1u);
@@ -655,7 +646,8 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
                 st->n = *(volatile int *)&st->n_next;
                 st->wall[0] += *(volatile unsigned long long *)&st->wall_pend[0];
                 st->wall[1] += *(volatile unsigned long long *)&st->wall_pend[1];
-                st->vmax2 = *(volatile unsigned *)&st->vmax2_next;
+                st->vmax2 = 0x7f800000u; // speed bound unknown after a fused step (+inf): the split path, should it
+                                         // take over, enqueues its general arranger until its mover has measured one
                 st->maxcount = *(volatile int *)&st->maxcount_next;
                 st->w_acc = 0;
                 st->step_max = 0;
