@@ -443,3 +443,61 @@ def test_neutral_species_qm_zero():
     assert np.array_equal(np.sort(states[2].vx[:states[2].n]), np.sort(v0)[:states[2].n]) or states[2].n < len(v0)
     for sp in sim.species:
         assert pic.pic_fused_info(sp)["decline_reasons"] == 0
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_random_api_sequences(seed):
+    """Random interleavings of pic_push(k), pic_arrange, pic_set_field, pic_wall_flux, pic_deposit and full state
+    comparisons, for every arrange_every rule, both boundaries, with and without a particle that makes the fused
+    step decline somewhere in the middle: the host bookkeeping (buffer parity, step counter, deferred check of
+    fused steps, wall counter intervals) must stay in lock-step with the oracle."""
+    rng = np.random.default_rng(1000 + seed)
+    boundary = workloads.PERIODIC if seed % 2 == 0 else workloads.ABSORBING
+    ae = (1, 1, 3, 0, 1, 2)[seed]
+    nc, ppc = 257, 24
+    cell = np.repeat(np.arange(nc, dtype=np.int32), ppc)
+    x = cell + rng.random(len(cell))
+    x = np.where(np.floor(x) != cell, np.nextafter(cell + 1.0, 0), x)
+    v = rng.standard_normal((3, len(cell)))
+    if seed in (1, 4):
+        v[2, 1234] = 24.0  # turns into vx > 10 after a few gyrations: a two-cell jump, the fused step declines
+    def field():
+        E = rng.uniform(-0.3, 0.3, nc + 1)
+        if boundary == workloads.PERIODIC:
+            E[nc] = E[0]
+        return E
+    inp = dict(nc=nc, dx=1.0, dt=0.1, boundary=boundary, E=field(), B=np.array([1.4, 1.4, 0.3]), arrange_every=ae,
+               species=[dict(qm=-1.0, x=x, vx=v[0], vy=v[1], vz=v[2], cell=cell)])
+    sim, (st,) = make_pair(inp)
+    sp = sim.species[0]
+    arranged = False  # the oracle fills count / offset at its first arrange only
+    last_flux_steps = 0
+    for op_i in range(40):
+        op = rng.choice(["push", "push", "push", "arrange", "field", "flux", "deposit", "compare"])
+        if op == "push":
+            k = int(rng.integers(1, 5))
+            pic.pic_push(sp, k)
+            st.push(k)
+            arranged = ae > 0 and st.steps % ae == 0
+        elif op == "arrange":
+            pic.pic_arrange(sp)
+            st.arrange()
+            arranged = True
+        elif op == "field":
+            E = field()
+            pic.pic_set_field(sim, E)
+            st.E = np.ascontiguousarray(E)
+        elif op == "flux":
+            wf = pic.pic_wall_flux(sp)
+            assert (wf["left_total"], wf["right_total"]) == (int(st.wall[0]), int(st.wall[1]))
+            assert wf["steps_recent"] == st.steps - last_flux_steps and wf["steps_total"] == st.steps
+            last_flux_steps = st.steps
+        elif op == "deposit" and arranged:
+            _check_deposit(sp, st, 1.5, f"seed {seed} op {op_i}")
+        elif op == "compare":
+            wf = compare(sp, st, where=f"seed {seed} op {op_i}", counts=arranged, nc=nc)
+            last_flux_steps = st.steps
+    compare(sp, st, where=f"seed {seed} end", counts=arranged, nc=nc)
+    pic.pic_sync(sim)
+    if seed in (1, 4) and st.steps >= 12:
+        assert pic.pic_fused_info(sp)["decline_reasons"] & 1, "the fast particle should have made a fused step decline"
