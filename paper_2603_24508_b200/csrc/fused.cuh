@@ -308,7 +308,7 @@ __device__ __forceinline__ void fused_issue(const FusedArgs &a, const FusedCtx &
 // of that marks the particle bad (it moved more than one cell, or the grouping is broken).
 // cellinfo[cl] = {first slot, count} of the tile's cells from off_old: a slot outside its cell's range
 // means the grouping is broken.  W_[r] = class | local cell << 2 | bad << 8.
-template <bool PERIODIC, bool EDGE, int RMAX, int R0, int CNT>
+template <bool PERIODIC, bool EDGE, bool BZ0, int RMAX, int R0, int CNT>
 __device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *px, const double *sEs, const int2 *cellinfo, int lane,
                                               int pad, int n, int cA, int ncell, double (&X_)[RMAX], double (&VX_)[RMAX],
                                               double (&VY_)[RMAX], double (&VZ_)[RMAX], int (&W_)[RMAX])
@@ -339,12 +339,24 @@ __device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *
         const double Ep = __dadd_rn(E0, __dmul_rn(w, dE));
         const double hE = __dmul_rn(k.h, Ep);
         const double ux = __dadd_rn(vx, hE), uy = vy, uz = vz;
-        const double qx = __dadd_rn(ux, __dsub_rn(__dmul_rn(uy, k.tz), __dmul_rn(uz, k.ty)));
-        const double qy = __dadd_rn(uy, __dsub_rn(__dmul_rn(uz, k.tx), __dmul_rn(ux, k.tz)));
-        const double qz = __dadd_rn(uz, __dsub_rn(__dmul_rn(ux, k.ty), __dmul_rn(uy, k.tx)));
-        const double wx = __dadd_rn(ux, __dsub_rn(__dmul_rn(qy, k.sz), __dmul_rn(qz, k.sy)));
-        const double wy = __dadd_rn(uy, __dsub_rn(__dmul_rn(qz, k.sx), __dmul_rn(qx, k.sz)));
-        const double wz = __dadd_rn(uz, __dsub_rn(__dmul_rn(qx, k.sy), __dmul_rn(qy, k.sx)));
+        double qx, qy, qz, wx, wy, wz;
+        if (BZ0) {
+            // Bz = 0 (so tz = sz = 0): the products with tz / sz are exact zeros and a + (0 - b) == a - b, a + (b - 0) == a + b
+            // bit for bit (only the sign of a zero can differ)
+            qx = __dsub_rn(ux, __dmul_rn(uz, k.ty));
+            qy = __dadd_rn(uy, __dmul_rn(uz, k.tx));
+            qz = __dadd_rn(uz, __dsub_rn(__dmul_rn(ux, k.ty), __dmul_rn(uy, k.tx)));
+            wx = __dsub_rn(ux, __dmul_rn(qz, k.sy));
+            wy = __dadd_rn(uy, __dmul_rn(qz, k.sx));
+            wz = __dadd_rn(uz, __dsub_rn(__dmul_rn(qx, k.sy), __dmul_rn(qy, k.sx)));
+        } else {
+            qx = __dadd_rn(ux, __dsub_rn(__dmul_rn(uy, k.tz), __dmul_rn(uz, k.ty)));
+            qy = __dadd_rn(uy, __dsub_rn(__dmul_rn(uz, k.tx), __dmul_rn(ux, k.tz)));
+            qz = __dadd_rn(uz, __dsub_rn(__dmul_rn(ux, k.ty), __dmul_rn(uy, k.tx)));
+            wx = __dadd_rn(ux, __dsub_rn(__dmul_rn(qy, k.sz), __dmul_rn(qz, k.sy)));
+            wy = __dadd_rn(uy, __dsub_rn(__dmul_rn(qz, k.sx), __dmul_rn(qx, k.sz)));
+            wz = __dadd_rn(uz, __dsub_rn(__dmul_rn(qx, k.sy), __dmul_rn(qy, k.sx)));
+        }
         const double nvx = __dadd_rn(wx, hE);
         const double xn = __dadd_rn(x, __dmul_rn(nvx, k.dt));
         double xw = xn;
@@ -382,13 +394,13 @@ __device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *
 
 // Row groups of sweep 1a: four rows at a time while at least four remain likely, then two, then single rows,
 // so that a tile of nrows rows pushes at most one surplus row.
-template <bool PERIODIC, bool EDGE, int RMAX>
+template <bool PERIODIC, bool EDGE, bool BZ0, int RMAX>
 __device__ __forceinline__ void fused_sweep1a_all(const PushConst &k, const double *px, const double *sEs, const int2 *cellinfo, int lane,
                                                   int pad, int n, int nrows, int cA, int ncell, double (&X_)[RMAX], double (&VX_)[RMAX],
                                                   double (&VY_)[RMAX], double (&VZ_)[RMAX], int (&W_)[RMAX])
 {
 #define FUSED_ROWS(R0, CNT) \
-    if (R0 < nrows) fused_sweep1a<PERIODIC, EDGE, RMAX, R0, CNT>(k, px, sEs, cellinfo, lane, pad, n, cA, ncell, X_, VX_, VY_, VZ_, W_);
+    if (R0 < nrows) fused_sweep1a<PERIODIC, EDGE, BZ0, RMAX, R0, CNT>(k, px, sEs, cellinfo, lane, pad, n, cA, ncell, X_, VX_, VY_, VZ_, W_);
     FUSED_ROWS(0, 4)
     if (RMAX == 8) {
         FUSED_ROWS(4, 2) FUSED_ROWS(6, 1) FUSED_ROWS(7, 1)
@@ -400,7 +412,7 @@ __device__ __forceinline__ void fused_sweep1a_all(const PushConst &k, const doub
 #undef FUSED_ROWS
 }
 
-template <int RMAX, bool PERIODIC>
+template <int RMAX, bool PERIODIC, bool BZ0>
 __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fused_kernel(FusedArgs a)
 {
     static_assert(RMAX == 8 || RMAX == 12 || RMAX == 16, "row groups of sweep 1a are written for these sizes");
@@ -491,8 +503,8 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
             // ---- sweep 1a: push into registers and classify (fused_sweep1a) ----------------------------------
             double X_[RMAX], VX_[RMAX], VY_[RMAX], VZ_[RMAX];
             int W_[RMAX]; // 1a: class | cell << 2 | bad << 8;  1b: -1, or class prefix count << 8 | class*32 + cell
-            if (cA == 0 || cB == nc) fused_sweep1a_all<PERIODIC, true, RMAX>(a.k, px, sEs, cellinfo, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_);
-            else fused_sweep1a_all<PERIODIC, false, RMAX>(a.k, px, sEs, cellinfo, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_);
+            if (cA == 0 || cB == nc) fused_sweep1a_all<PERIODIC, true, BZ0, RMAX>(a.k, px, sEs, cellinfo, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_);
+            else fused_sweep1a_all<PERIODIC, false, BZ0, RMAX>(a.k, px, sEs, cellinfo, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_);
             __syncwarp();
             // the stage has been read: refill it with the next item to load
             if (lane == 0) fused_issue(a, X, two ? I2 : I1, px, odd ? mb1 : mb0);

@@ -339,12 +339,11 @@ static int create_species(pic_sim *sim, const pic_species_desc &d, pic_species *
     {
         static bool attr_set = false;
         if (!attr_set) {
-            CU(cudaFuncSetAttribute(fused_kernel<8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-            CU(cudaFuncSetAttribute(fused_kernel<12, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-            CU(cudaFuncSetAttribute(fused_kernel<16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-            CU(cudaFuncSetAttribute(fused_kernel<8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-            CU(cudaFuncSetAttribute(fused_kernel<12, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-            CU(cudaFuncSetAttribute(fused_kernel<16, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+            void (*kerns[])(FusedArgs) = {fused_kernel<8, true, true>,   fused_kernel<12, true, true>,   fused_kernel<16, true, true>,
+                                          fused_kernel<8, false, true>,  fused_kernel<12, false, true>,  fused_kernel<16, false, true>,
+                                          fused_kernel<8, true, false>,  fused_kernel<12, true, false>,  fused_kernel<16, true, false>,
+                                          fused_kernel<8, false, false>, fused_kernel<12, false, false>, fused_kernel<16, false, false>};
+            for (auto kfn : kerns) CU(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
             attr_set = true;
         }
     }
@@ -696,9 +695,12 @@ static int push_fused(pic_species *s)
         KernelSpan span(sim, K_FUSED);
         fused_edge_kernel<<<1, 128, 0, sim->stream>>>(a);
         if (int rc = launch_check(sim, "fused_edge_kernel")) return rc;
-        void (*kern)(FusedArgs) =
-            sim->periodic ? (rows == 8 ? fused_kernel<8, true> : rows == 12 ? fused_kernel<12, true> : fused_kernel<16, true>)
-                          : (rows == 8 ? fused_kernel<8, false> : rows == 12 ? fused_kernel<12, false> : fused_kernel<16, false>);
+        const bool bz0 = s->k.tz == 0.0 && s->k.sz == 0.0; // B in the x-y plane: the kernel drops the exact-zero products
+        void (*kern)(FusedArgs);
+#define PIC_FUSED_PICK(P, Z) (rows == 8 ? fused_kernel<8, P, Z> : rows == 12 ? fused_kernel<12, P, Z> : fused_kernel<16, P, Z>)
+        if (sim->periodic) kern = bz0 ? PIC_FUSED_PICK(true, true) : PIC_FUSED_PICK(true, false);
+        else kern = bz0 ? PIC_FUSED_PICK(false, true) : PIC_FUSED_PICK(false, false);
+#undef PIC_FUSED_PICK
         kern<<<grid, 32, smem, sim->stream>>>(a);
         if (int rc = launch_check(sim, "fused_kernel")) return rc;
     }
