@@ -1,6 +1,6 @@
 /*
  * oracle.c -- plain, slow, obviously-correct CPU oracle for the BIT1-style particle
- * mover and arranger (the grey box of Fig. 1; phases (i)+(iv) of the PIC
+ * mover, arranger and charge deposition (the grey box of Fig. 1; phases (i)+(iv) of the PIC
  * cycle; `move0`/`moveb`, `arrj`, `rempar2`).
  *
  * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
@@ -24,6 +24,9 @@
  *       force in extended precision, gather vs numpy.interp, wall/wrap edge cases.
  *   oracle_arrange : P8 O(N^2) rank brute force and numpy stable argsort, P9 count /
  *       offset invariants, P10 idempotence, the tiny printed pin of SURVEY 8(c).
+ *   oracle_deposit : single particle (exact 3/4, 1/4), total charge, first moment, one particle
+ *       per cell centre, periodic fold, linearity, numpy add.at brute force, clamp (S8)
+ *       (tests/test_oracle_deposit.py).
  *   Parity with BIT1's own output is UNPINNED (no code, no printed values in the paper).
  */
 #include <math.h>
