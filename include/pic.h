@@ -165,7 +165,9 @@ int pic_arrange_info(pic_species *sp, int32_t *w_bound, int32_t *used_general);
  * with an arrange would take it.  *decline_reasons: OR of the reasons any fused step has been
  * redone by the split kernels so far (1 = a particle moved more than one cell or broke the
  * grouping, 2 = a cell did not fit a tile, 4 / 8 = a boundary list overflowed);
- * 0 means every fused step so far completed.  *stage_slots, *ctas_per_sm: the launch geometry
+ * 0 means every fused step so far completed.  After a decline the split kernels carry on; the
+ * fused path is tried again once a synchronising call finds the state arranged and the last
+ * step's displacements within one cell, 16 or more steps later.  *stage_slots, *ctas_per_sm: the launch geometry
  * the next fused step would use.  Any pointer may be NULL.  Syncs. */
 int pic_fused_info(pic_species *sp, int32_t *active, int32_t *decline_reasons, int32_t *stage_slots,
                    int32_t *ctas_per_sm);

@@ -40,6 +40,7 @@ constexpr int FUSED_STAGES_DEFAULT = 1;    // stages of the shared-memory ring (
 constexpr int FUSED_KMAX = 31;         // cells per tile (one lane per cell border)
 constexpr int FUSED_DEF = 32;          // deferred right-movers of a tile's last cell
 constexpr int FUSED_XCAP = 256;        // edge kernel: leavers per edge cell
+constexpr int FUSED_RETRY_STEPS = 16;  // split steps after a decline before the fused path is tried again
 constexpr int FUSED_SMEM_SM = 233472;  // shared memory per SM (228 KB), 1 KB reserved per CTA
 
 constexpr int FA_BAD_PARTICLE = 1; // moved more than one cell / left the gather range / broke the grouping

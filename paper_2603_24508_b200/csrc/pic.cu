@@ -57,6 +57,7 @@ struct pic_species {
     bool fused_off = false;            // the device reported a declined fused step (sticky)
     // fused steps enqueued but not yet verified (verify_fused): how many, and the host state when the run began
     long long unv_steps = 0, unv_steps0 = 0;
+    long long declined_at = 0;         // step count when the last decline was detected
     int unv_cur0 = 0, unv_off0 = 0;
     // host-side conservative bound on cell displacement since the last arrange (decides whether the
     // general-path kernels need to be enqueued at all)
@@ -729,6 +730,7 @@ static int verify_fused(pic_species *s)
     s->unv_steps = 0;
     if (!h.fused_disabled) return PIC_OK;
     s->fused_off = true;
+    s->declined_at = s->unv_steps0 + run;
     const long long k = ((long long)h.fail_step - (s->unv_steps0 & 0x7fffffff)) & 0x7fffffff; // steps that completed
     if (k >= run) {
         snprintf(g_err, sizeof g_err, "fused step bookkeeping: declined step %d outside the unverified run", h.fail_step);
@@ -787,6 +789,15 @@ static int read_state(pic_species *s, DevState &h)
     if (h.fused_disabled) s->fused_off = true;
     s->h_maxcount = h.maxcount;
     s->h_abort_reason = h.abort_reason;
+    // A declined fused path comes back once the cause is gone: the state is arranged, the split mover's last
+    // step moved no particle by more than one cell, and some steps have passed since the decline.
+    if (s->fused_off && s->arrange_every == 1 && s->counts_fresh && h.w_acc <= 1 && h.status == 0 &&
+        s->steps - s->declined_at >= FUSED_RETRY_STEPS && !(h.abort_reason & (FA_DEFER_OVERFLOW | FA_EDGE_OVERFLOW))) {
+        const int zero = 0;
+        CU(cudaMemcpyAsync(&s->d_st->fused_disabled, &zero, sizeof zero, cudaMemcpyHostToDevice, s->sim->stream));
+        CU(cudaStreamSynchronize(s->sim->stream));
+        s->fused_off = false;
+    }
     return PIC_OK;
 }
 

@@ -501,3 +501,31 @@ def test_random_api_sequences(seed):
     pic.pic_sync(sim)
     if seed in (1, 4) and st.steps >= 12:
         assert pic.pic_fused_info(sp)["decline_reasons"] & 1, "the fast particle should have made a fused step decline"
+
+
+def test_fused_path_comes_back_after_the_cause_is_gone():
+    """One particle far too fast for the fused step (2.5 cells per step) on an absorbing grid: the fused step
+    declines, the split kernels carry the run, the particle is absorbed at the wall, and 16 steps later a
+    synchronising call switches the fused path back on.  Parity throughout."""
+    inp = workloads.make(2, nc=256, ppc=40)
+    s = inp["species"][0]
+    for k in ("vx", "vy", "vz"):
+        s[k] = s[k].copy()
+    p = 40 * 200 + 3  # a particle in cell 200 heading for the right wall
+    s["vx"][p], s["vy"][p], s["vz"][p] = 25.0, 0.0, 0.0
+    inp["B"] = np.array([2.0, 0.0, 0.0])  # B along x: vx is not rotated away
+    sim, (st,) = make_pair(inp, options={"fused": 1})
+    sp = sim.species[0]
+    seen_off = seen_back = False
+    for step in range(1, 71):
+        pic.pic_push(sp, 1)
+        st.push(1)
+        if step % 5 == 0:
+            compare(sp, st, where=f"step {step}", counts=True, nc=inp["nc"])
+            info = pic.pic_fused_info(sp)
+            if info["active"] == 0:
+                seen_off = True
+            elif seen_off:
+                seen_back = True
+    assert seen_off and seen_back, "fused path should have declined and then come back"
+    assert pic.pic_fused_info(sp)["decline_reasons"] & 1
