@@ -413,6 +413,16 @@ __device__ __forceinline__ void fused_sweep1a_all(const PushConst &k, const doub
 #undef FUSED_ROWS
 }
 
+// Row groups shared by the three sweeps: rows 4 by 4 while at least four more can follow, then 2, 1, 1 (for RMAX = 8:
+// {0-3} {4,5} {6} {7}).  A group runs if its first row is inside the tile; rows of it behind the tile are masked
+// out (class X, nothing stored), so that a group is straight-line code whose rows interleave.
+__host__ __device__ constexpr int fused_ngroups(int rmax) { return rmax / 4 + 2; }
+__host__ __device__ constexpr int fused_group_start(int rmax, int gi)
+{
+    return gi < rmax / 4 - 1 ? 4 * gi : 4 * (rmax / 4 - 1) + (gi == rmax / 4 - 1 ? 0 : (gi == rmax / 4 ? 2 : 3));
+}
+__host__ __device__ constexpr int fused_group_count(int rmax, int gi) { return gi < rmax / 4 - 1 ? 4 : (gi == rmax / 4 - 1 ? 2 : 1); }
+
 template <int RMAX, bool PERIODIC, bool BZ0>
 __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fused_kernel(FusedArgs a)
 {
@@ -513,17 +523,20 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
             // ---- sweep 1b: prefix counts per class (ballot/popc); the row's ballots are kept for the cell borders ---
             unsigned run = 0; // running class counts of the tile: L | S << 10 | R << 20
 #pragma unroll
-            for (int r = 0; r < RMAX; ++r) {
-                if (r < nrows) {
-                    const int w = W_[r];
-                    const int g = w & 3;
-                    if (w & 256) bad |= FA_BAD_PARTICLE;
-                    const unsigned mL = __ballot_sync(FULL, g == 0), mS = __ballot_sync(FULL, g == 1), mR = __ballot_sync(FULL, g == 2);
-                    if (lane == 0) rowinfo[r] = make_int4((int)mL, (int)mS, (int)mR, (int)run);
-                    const unsigned mo = g == 0 ? mL : (g == 1 ? mS : mR);
-                    const int mine = (int)((run >> (10 * g)) & 1023u) + __popc(mo & lt);
-                    W_[r] = g < 3 ? (mine << 8) | (g * 32 + ((w >> 2) & 31)) : -1;
-                    run += (unsigned)__popc(mL) | ((unsigned)__popc(mS) << 10) | ((unsigned)__popc(mR) << 20);
+            for (int gi = 0; gi < fused_ngroups(RMAX); ++gi) {
+                if (fused_group_start(RMAX, gi) < nrows) {
+#pragma unroll
+                    for (int r = fused_group_start(RMAX, gi); r < fused_group_start(RMAX, gi) + fused_group_count(RMAX, gi); ++r) {
+                        const int w = W_[r];
+                        const int g = w & 3;
+                        if (w & 256) bad |= FA_BAD_PARTICLE;
+                        const unsigned mL = __ballot_sync(FULL, g == 0), mS = __ballot_sync(FULL, g == 1), mR = __ballot_sync(FULL, g == 2);
+                        if (lane == 0) rowinfo[r] = make_int4((int)mL, (int)mS, (int)mR, (int)run);
+                        const unsigned mo = g == 0 ? mL : (g == 1 ? mS : mR);
+                        const int mine = (int)((run >> (10 * g)) & 1023u) + __popc(mo & lt);
+                        W_[r] = g < 3 ? (mine << 8) | (g * 32 + ((w >> 2) & 31)) : -1;
+                        run += (unsigned)__popc(mL) | ((unsigned)__popc(mS) << 10) | ((unsigned)__popc(mR) << 20);
+                    }
                 }
             }
             __syncwarp();
@@ -599,28 +612,31 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
                 const int kdef = 64 + ncell - 1;                                 // class R of the tile's last cell
                 const int rdef = __shfl_sync(FULL, st_q, max(ncell - 1, 0)) >> 5; // first row that can hold it
 #pragma unroll
-                for (int r = 0; r < RMAX; ++r) {
-                    if (r < nrows) {
-                        const int pk = W_[r];
-                        const bool has = pk >= 0;
-                        const int2 bd = basd[pk & 127];
-                        const int p = bd.x + (pk >> 8);
-                        const bool defer = has && (pk & 127) == kdef;
-                        if (has && !defer) {
-                            a.dx[p] = X_[r]; a.dvx[p] = VX_[r]; a.dvy[p] = VY_[r]; a.dvz[p] = VZ_[r];
-                            a.dcell[p] = bd.y;
-                        }
-                        if (r >= rdef) {
-                            const unsigned md = __ballot_sync(FULL, defer);
-                            if (md) {
-                                if (defer) {
-                                    const int q = ndef + __popc(md & lt);
-                                    if (q < FUSED_DEF) {
-                                        qx[q] = X_[r]; qvx[q] = VX_[r]; qvy[q] = VY_[r]; qvz[q] = VZ_[r];
-                                        qpos[q] = p;
-                                    } else bad |= FA_DEFER_OVERFLOW;
+                for (int gi = 0; gi < fused_ngroups(RMAX); ++gi) {
+                    if (fused_group_start(RMAX, gi) < nrows) {
+#pragma unroll
+                        for (int r = fused_group_start(RMAX, gi); r < fused_group_start(RMAX, gi) + fused_group_count(RMAX, gi); ++r) {
+                            const int pk = W_[r];
+                            const bool has = pk >= 0;
+                            const int2 bd = basd[pk & 127];
+                            const int p = bd.x + (pk >> 8);
+                            const bool defer = has && (pk & 127) == kdef;
+                            if (has && !defer) {
+                                a.dx[p] = X_[r]; a.dvx[p] = VX_[r]; a.dvy[p] = VY_[r]; a.dvz[p] = VZ_[r];
+                                a.dcell[p] = bd.y;
+                            }
+                            if (r >= rdef) {
+                                const unsigned md = __ballot_sync(FULL, defer);
+                                if (md) {
+                                    if (defer) {
+                                        const int q = ndef + __popc(md & lt);
+                                        if (q < FUSED_DEF) {
+                                            qx[q] = X_[r]; qvx[q] = VX_[r]; qvy[q] = VY_[r]; qvz[q] = VZ_[r];
+                                            qpos[q] = p;
+                                        } else bad |= FA_DEFER_OVERFLOW;
+                                    }
+                                    ndef = min(ndef + __popc(md), FUSED_DEF);
                                 }
-                                ndef = min(ndef + __popc(md), FUSED_DEF);
                             }
                         }
                     }
