@@ -180,7 +180,7 @@ size_t pic_workspace_bytes(int32_t nc, int64_t capacity);
  * nodes of each chunk staged in shared memory by TMA bulk copies), 0 = separate mover / scan /
  * scatter kernels (E through the read-only global path); "kernel_timing": 1 = record CUDA events
  * around every kernel launch (see pic_kernel_time).  Knobs of the fused step:
- * "fused_cells_per_cta" (cells per chunk, 1..256; 0 = automatic, at most 64), "fused_rows" (rows
+ * "fused_cells_per_cta" (cells per chunk, 1..256; 0 = automatic: 32 on large grids), "fused_rows" (rows
  * of 32 slots per tile: 8, 12 or 16; 0 = automatic from the largest per-cell count),
  * "fused_stage_slots" (largest tile in slots, even, <= 32*rows; 0 = 32*rows), "fused_stages"
  * (stages of the TMA ring: 1 or 2; 0 = default 1).  Results never depend on any of them.

@@ -34,7 +34,8 @@
 namespace pic {
 
 constexpr int FUSED_MIN_NC = 16;
-constexpr int FUSED_CPC_DEFAULT = 64;  // cells per chunk (per CTA)
+constexpr int FUSED_CPC_DEFAULT = 32;  // cells per chunk (per CTA) on grids of many waves (measured optimum at config 4)
+constexpr int FUSED_CPC_SEARCH = 64;   // largest chunk the per-launch search considers on smaller grids
 constexpr int FUSED_CPC_MAX = 256;
 constexpr int FUSED_STAGES_DEFAULT = 1;    // stages of the shared-memory ring (1: more CTAs per SM; measured faster than 2)
 constexpr int FUSED_KMAX = 31;         // cells per tile (one lane per cell border)

@@ -625,7 +625,7 @@ static int fused_cells_per_cta(const pic_species *s, int rows, int stages)
         if ((double)((sim->nc + best - 1) / best) >= 4.0 * resident) return best;
     }
     double best_score = -1.0;
-    for (int cpc = 2; cpc <= FUSED_CPC_DEFAULT; ++cpc) {
+    for (int cpc = 2; cpc <= FUSED_CPC_SEARCH; ++cpc) {
         const double resident = (double)sim->sm_count * fused_ctas_per_sm(rows, cpc, stages);
         const double chunks = (double)((sim->nc + cpc - 1) / cpc);
         const double score = chunks / (std::ceil(chunks / resident) * resident) * cpc / (cpc + 2.0);
