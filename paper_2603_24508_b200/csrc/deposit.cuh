@@ -1,7 +1,7 @@
 // deposit.cuh -- charge deposition on the arranged state (PIC phase (ii); SURVEY.md
 // section 8(f) rank 1): linear (cloud-in-cell) weights, the transpose of the
 // mover's gather.  Because the particles of cell c occupy the slots [offset[c], offset[c+1]) the
-// scatter-add becomes a segmented reduction: one warp per cell sums (1-w) and w over its particles
+// scatter-add becomes a segmented reduction: half a warp (or a warp) per cell sums (1-w) and w over its particles
 // (lane-strided partial sums, then a fixed shuffle tree: no atomics, bitwise deterministic), and one
 // thread per node adds the two cells that touch it.  8 B read per particle.
 #pragma once
@@ -19,22 +19,25 @@ struct DepositArgs {
     double inv_dx;
 };
 
+// LPC lanes per cell (16: half a warp; 32 for very large cells): the lanes stride
+// over the cell's particles with eight loads in flight each (8*LPC particles per round trip), then a fixed
+// shuffle tree inside the lane group.
+template <int LPC>
 __global__ void __launch_bounds__(DEP_THREADS) deposit_cell_kernel(DepositArgs a)
 {
-    const int lane = threadIdx.x & 31;
-    const long long c = ((long long)blockIdx.x * DEP_THREADS + threadIdx.x) >> 5;
-    if (c >= a.nc) return;
-    const int s0 = a.off[c], s1 = a.off[c + 1];
+    const int sub = threadIdx.x & (LPC - 1);
+    const long long c = ((long long)blockIdx.x * DEP_THREADS + threadIdx.x) / LPC;
+    const bool live = c < a.nc;
+    const int s0 = live ? a.off[c] : 0, s1 = live ? a.off[c + 1] : 0;
     const double cf = (double)c; // = floor(x*inv_dx), clamped to nc-1, for every particle of the cell (invariant)
     double a0 = 0.0, a1 = 0.0;
-    // four loads in flight per lane: a cell of up to 128 particles is fetched in one round trip
-    for (int i = s0 + lane; i < s1; i += 128) {
-        double xv[4];
+    for (int i = s0 + sub; i < s1; i += 8 * LPC) {
+        double xv[8];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) xv[q] = i + 32 * q < s1 ? a.x[i + 32 * q] : 0.0;
+        for (int q = 0; q < 8; ++q) xv[q] = i + LPC * q < s1 ? a.x[i + LPC * q] : 0.0;
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            if (i + 32 * q < s1) {
+        for (int q = 0; q < 8; ++q) {
+            if (i + LPC * q < s1) {
                 const double w = __dsub_rn(__dmul_rn(xv[q], a.inv_dx), cf);
                 a0 += 1.0 - w;
                 a1 += w;
@@ -42,11 +45,11 @@ __global__ void __launch_bounds__(DEP_THREADS) deposit_cell_kernel(DepositArgs a
         }
     }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
+    for (int o = LPC / 2; o > 0; o >>= 1) {
         a0 += __shfl_xor_sync(FULL, a0, o);
         a1 += __shfl_xor_sync(FULL, a1, o);
     }
-    if (lane == 0) a.cs[c] = make_double2(a0, a1);
+    if (live && sub == 0) a.cs[c] = make_double2(a0, a1);
 }
 
 // rho[j] = weight * (sum (1-w) over cell j + sum w over cell j-1); nodes 0 and nc of a periodic grid are one
