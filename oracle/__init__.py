@@ -15,6 +15,33 @@ PERIODIC = 0
 ABSORBING = 1
 
 _lib = None
+_lib_omp = None
+
+
+def lib_omp():
+    """The threaded twin (oracle/oracle_omp.c): same results as lib(), bit for bit, on all host cores."""
+    global _lib_omp
+    if _lib_omp is None:
+        _lib_omp = C.CDLL(_build.build_omp())
+        dp, ip, u64p = C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_uint64)
+        i64p = C.POINTER(C.c_int64)
+        _lib_omp.oracle_omp_max_threads.argtypes = []
+        _lib_omp.oracle_omp_max_threads.restype = C.c_int
+        _lib_omp.oracle_omp_push.argtypes = [C.c_int64, dp, dp, dp, dp, ip, C.c_int32, C.c_double, C.c_double,
+                                             C.c_int32, dp, C.c_double, dp, u64p, C.c_int32]
+        _lib_omp.oracle_omp_push.restype = C.c_int
+        _lib_omp.oracle_omp_arrange.argtypes = [C.c_int64, dp, dp, dp, dp, ip, dp, dp, dp, dp, ip, C.c_int32, ip, ip,
+                                                C.c_int32]
+        _lib_omp.oracle_omp_arrange.restype = C.c_int64
+        _lib_omp.oracle_omp_run.argtypes = [C.c_int32, C.c_int32, i64p, i64p, dp, dp, dp, dp, ip, dp, dp, dp, dp, ip,
+                                            C.c_int32, C.c_double, C.c_double, C.c_int32, dp, C.c_double, dp, u64p,
+                                            ip, ip, C.c_int32]
+        _lib_omp.oracle_omp_run.restype = C.c_int
+    return _lib_omp
+
+
+def omp_max_threads():
+    return int(lib_omp().oracle_omp_max_threads())
 
 
 def lib():
@@ -60,7 +87,10 @@ def boris_constants(qm, dt, dx, B):
 class State:
     """Host-side species state driven by the oracle: x, vx, vy, vz (f64), cell (i32), n."""
 
-    def __init__(self, x, vx, vy, vz, cell, *, nc, dx, dt, boundary, E, qm, B, arrange_every=0):
+    def __init__(self, x, vx, vy, vz, cell, *, nc, dx, dt, boundary, E, qm, B, arrange_every=0, threads=None):
+        """threads=None: the single-thread oracle (oracle.c, the authority).  threads=k >= 1 (0 = all cores):
+        its threaded twin (oracle_omp.c), pinned bit-identical to it by tests/test_oracle_omp.py."""
+        self.threads = threads
         self.cap = len(x)
         self.x = np.array(x, dtype=np.float64)
         self.vx = np.array(vx, dtype=np.float64)
@@ -90,20 +120,25 @@ class State:
         t = self._tmpbufs()
         steps = C.c_int64(self.steps)
         n = C.c_int64(self.n)
-        rc = lib().oracle_run(nsteps, self.arrange_every, C.byref(steps), C.byref(n),
-                              _d(self.x), _d(self.vx), _d(self.vy), _d(self.vz), _i(self.cell),
-                              _d(t[0]), _d(t[1]), _d(t[2]), _d(t[3]), _i(t[4]),
-                              self.nc, self.dx, self.dt, self.boundary, _d(self.E), self.qm, _d(self.B),
-                              self.wall.ctypes.data_as(C.POINTER(C.c_uint64)), _i(self.count), _i(self.offset))
+        args = (nsteps, self.arrange_every, C.byref(steps), C.byref(n),
+                _d(self.x), _d(self.vx), _d(self.vy), _d(self.vz), _i(self.cell),
+                _d(t[0]), _d(t[1]), _d(t[2]), _d(t[3]), _i(t[4]),
+                self.nc, self.dx, self.dt, self.boundary, _d(self.E), self.qm, _d(self.B),
+                self.wall.ctypes.data_as(C.POINTER(C.c_uint64)), _i(self.count), _i(self.offset))
+        if self.threads is None:
+            rc = lib().oracle_run(*args)
+        else:
+            rc = lib_omp().oracle_omp_run(*args, int(self.threads))
         if rc:
             raise RuntimeError(f"oracle_run failed rc={rc}")
         self.steps, self.n = steps.value, n.value
 
     def push_only(self):
         """one bare mover step, no arrange, over slots [0,n) (oracle_push)."""
-        rc = lib().oracle_push(self.n, _d(self.x), _d(self.vx), _d(self.vy), _d(self.vz), _i(self.cell),
-                               self.nc, self.dx, self.dt, self.boundary, _d(self.E), self.qm, _d(self.B),
-                               self.wall.ctypes.data_as(C.POINTER(C.c_uint64)))
+        args = (self.n, _d(self.x), _d(self.vx), _d(self.vy), _d(self.vz), _i(self.cell),
+                self.nc, self.dx, self.dt, self.boundary, _d(self.E), self.qm, _d(self.B),
+                self.wall.ctypes.data_as(C.POINTER(C.c_uint64)))
+        rc = lib().oracle_push(*args) if self.threads is None else lib_omp().oracle_omp_push(*args, int(self.threads))
         if rc:
             raise RuntimeError(f"oracle_push failed rc={rc}")
         self.steps += 1
@@ -111,9 +146,9 @@ class State:
     def arrange(self):
         """explicit arrange (oracle_arrange); does not touch the step counter."""
         t = self._tmpbufs()
-        nl = lib().oracle_arrange(self.n, _d(self.x), _d(self.vx), _d(self.vy), _d(self.vz), _i(self.cell),
-                                  _d(t[0]), _d(t[1]), _d(t[2]), _d(t[3]), _i(t[4]), self.nc,
-                                  _i(self.count), _i(self.offset))
+        args = (self.n, _d(self.x), _d(self.vx), _d(self.vy), _d(self.vz), _i(self.cell),
+                _d(t[0]), _d(t[1]), _d(t[2]), _d(t[3]), _i(t[4]), self.nc, _i(self.count), _i(self.offset))
+        nl = lib().oracle_arrange(*args) if self.threads is None else lib_omp().oracle_omp_arrange(*args, int(self.threads))
         if nl < 0:
             raise RuntimeError("oracle_arrange failed")
         for dst, src in zip((self.x, self.vx, self.vy, self.vz, self.cell), t):

@@ -64,7 +64,9 @@ void oracle_boris_constants(double qm, double dt, double dx, const double *B, do
  * E has nc+1 node values, node j at x_j = j*dx.  wall[0] += absorbed at x<0,
  * wall[1] += absorbed at x>=L (half-open domain [0,L), reading S6).
  * Returns 0, or -1 if a live particle's gather cell falls outside [0,nc-1]
- * (precondition 0 <= x < L violated). */
+ * (precondition 0 <= x < L violated) or differs from its stored cell index (SURVEY 8(c):
+ * "j == cell by invariant (oracle asserts)" -- a harness that hands over a stale cell array is
+ * caught here; the state is left as it was up to that particle). */
 int oracle_push(int64_t n, double *x, double *vx, double *vy, double *vz, int32_t *cell,
                 int32_t nc, double dx, double dt, int32_t boundary, const double *E,
                 double qm, const double *B, uint64_t *wall)
@@ -88,6 +90,8 @@ int oracle_push(int64_t n, double *x, double *vx, double *vy, double *vz, int32_
             j = nc - 1;
             jf = (double)j;
         }
+        if (cell[i] != j)
+            return -1; /* invariant cell == min(floor(x/dx), nc-1) broken */
         double w = xs - jf;
         double dE = E[j + 1] - E[j];
         double wdE = w * dE;

@@ -1,7 +1,11 @@
 """GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (own
 stream, default options: fused single-pass step where arrange_every == 1, TMA-staged E).
 
-Two kinds of check (task contract, parity at full size):
+Three kinds of check (task contract, parity at full size):
+  * the WHOLE run (every step of the config) element by element -- all five arrays, per-cell counts, offsets,
+    slot count, wall counters -- against the oracle's threaded twin (oracle/oracle_omp.c, pinned bit-identical
+    to the single-thread oracle by tests/test_oracle_omp.py); config 2 also against the single-thread oracle
+    itself;
   * element by element against the oracle for the first steps of every config (the oracle needs
     about a second per 30-40 M pushes, so a few steps of 100 M particles is still seconds);
   * after the config's whole step count: on SAMPLED particles the oracle computes one by one
@@ -126,4 +130,40 @@ def test_fullsize_all_steps_sampled_and_properties(config, margin):
             assert (wf["left_total"], wf["right_total"]) == (int(sw.wall[0]), int(sw.wall[1]))
         else:
             assert wf["left_total"] == 0 and wf["right_total"] == 0
+    pic.pic_destroy(sim)
+
+
+# ---- the whole run, element by element (north_star: "arranged order bit-exact ... on all five configs") ----------
+@pytest.mark.parametrize("config,single_thread_too", [(2, True), (3, False), (4, False), (5, False)])
+def test_fullsize_whole_run_elementwise(config, single_thread_too):
+    """Every step of the config at full size, in bench.py's launch configuration, one pic_push(nsteps) per species
+    (as the e2e leg) -- then the final state against the oracle's: the five arrays bit for bit over [0, n_live),
+    counts, offsets, walls.  A wrong rank inside a cell at any step changes the final order, so this covers the
+    stable order the sampled test below cannot see."""
+    inp = workloads.make(config)
+    nc, steps, ae = inp["nc"], inp["steps"], inp["arrange_every"]
+    assert steps % ae == 0
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        sim, _ = make_pair(inp, stream=stream)
+    del _
+    for sp in sim.species:
+        pic.pic_push(sp, steps)
+    pic.pic_sync(sim)
+    for si, (sp, s) in enumerate(zip(sim.species, inp["species"])):
+        kw = dict(nc=nc, dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E=inp["E"], qm=s["qm"], B=inp["B"],
+                  arrange_every=ae)
+        st = oracle.State(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], threads=0, **kw)
+        st.push(steps)
+        compare(sp, st, where=f"config {config} full size, all {steps} steps, species {si} (threaded oracle)",
+                counts=True, nc=nc)
+        if single_thread_too:
+            st1 = oracle.State(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], **kw)
+            st1.push(steps)
+            for a, b in zip(st1.live(), st.live()):
+                assert np.array_equal(a, b), "threaded oracle differs from the single-thread oracle"
+            assert np.array_equal(st1.wall, st.wall) and np.array_equal(st1.offset, st.offset)
+        assert pic.pic_arrange_info(sp)[1] == 0, "full-size run fell to the general arranger"
+        assert pic.pic_fused_info(sp)["decline_reasons"] == 0, "a fused step declined at full size"
+        del st
     pic.pic_destroy(sim)

@@ -377,3 +377,25 @@ def test_neutral_species_is_ballistic():
         x = np.where(x >= nc, x - nc, np.where(x < 0, x + nc, x))
     assert np.array_equal(st.vx, v0[0]) and np.array_equal(st.vy, v0[1]) and np.array_equal(st.vz, v0[2])
     assert np.array_equal(st.x, x)
+
+
+def test_stale_cell_index_is_rejected():
+    """"j == cell by invariant (oracle asserts)".  A harness that hands the oracle a cell array
+    that no longer matches floor(x/dx) must be caught, not silently pushed."""
+    st = make([2.5, 7.25], [[0.1, 0, 0], [0.2, 0, 0]], nc=16)
+    st.cell[1] = 6  # x = 7.25 sits in cell 7
+    x_before = st.x.copy()
+    with pytest.raises(RuntimeError):
+        st.push_only()
+    assert st.x[1] == x_before[1], "the offending particle must be left untouched"
+    ok = make([2.5, 7.25], [[0.1, 0, 0], [0.2, 0, 0]], nc=16)
+    ok.push_only()  # the same input with the right cells passes
+
+
+def test_P7_file_is_what_its_generator_writes(golden_dir):
+    """tests/golden/boris_worked_example.txt is the output of the committed scalar-float script beside it."""
+    import subprocess
+    import sys
+    r = subprocess.run([sys.executable, os.path.join(golden_dir, "make_boris_worked_example.py"), "--check"],
+                       capture_output=True, text=True)
+    assert r.returncode == 0, r.stdout + r.stderr
