@@ -21,10 +21,14 @@ library's stream.  `e2e`: the same metric through the C-ABI call pic_run_host wi
 (pinned) buffers, H2D + the config's full step count + D2H inside the timed region.
 `roofline`: the dominant kernel's algorithmic bytes / its mean launch duration measured with
 CUDA events inside the timed region (pic_kernel_time), against MEASURED_PEAKS.json.
-`cpu_baseline`: the CPU oracle (oracle/, as it stands, 1 thread) on a bounded sample.
+`cpu_baseline`: the CPU oracle (oracle/, as it stands) on the full-size workload for a reduced step
+count: single thread (the authority), and `threaded`: its bit-identical OpenMP twin on all host cores.
+`fused_path`: how many timed steps took the fused kernel / were redone by the split kernels; a
+decline inside the timed region marks the line "invalid" and the exit code is 3.
 
 --impl reference: there is no reference implementation to install (the paper ships no code);
-per the task contract this arm times the CPU oracle on the host cores.
+per the task contract this arm times the CPU oracle (threaded twin, all host cores) on the full-size
+workload for a bounded number of steps.
 """
 import argparse
 import json
@@ -123,20 +127,29 @@ class ClockSampler(threading.Thread):
 # ----------------------------------------------------------------------------------------------
 # CPU oracle legs (cpu_baseline of the main line; the whole of --impl reference)
 # ----------------------------------------------------------------------------------------------
-def oracle_sample(config, nc_sample, steps):
-    """Time the oracle, as it stands (1 thread), on the first nc_sample cells' worth of the workload.
-    Returns (pushes/s, seconds, pushes, description)."""
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def oracle_run(inp, steps, threads):
+    """Time `steps` steps of the oracle, as it stands, on the FULL workload `inp` (every species): threads=None is
+    oracle/oracle.c (single thread, the authority), threads=0 its threaded twin oracle/oracle_omp.c on all host
+    cores (pinned bit-identical to it by tests/test_oracle_omp.py).  Returns (pushes/s, seconds, pushes, cores)."""
     import oracle
-    from paper_2603_24508_b200 import workloads
-    kw = dict(nc=nc_sample)
-    inp = workloads.make(config, **kw)
     states = []
     for s in inp["species"]:
         states.append(oracle.State(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], nc=inp["nc"], dx=inp["dx"], dt=inp["dt"],
                                    boundary=inp["boundary"], E=inp["E"], qm=s["qm"], B=inp["B"],
-                                   arrange_every=inp["arrange_every"]))
+                                   arrange_every=inp["arrange_every"], threads=threads))
     oracle.lib()
-    n0 = sum(st.n for st in states)
+    cores = 1 if threads is None else oracle.omp_max_threads()
     t0 = time.perf_counter()
     pushes = 0
     for _ in range(steps):
@@ -144,32 +157,60 @@ def oracle_sample(config, nc_sample, steps):
             pushes += st.n
             st.push(1)
     dt = time.perf_counter() - t0
-    desc = (f"config {config} recipe on {nc_sample} cells ({n0} particles, all species), {steps} steps, "
-            f"arrange every {inp['arrange_every']}, oracle/oracle.c single thread")
-    return pushes / dt, dt, pushes, desc
+    return pushes / dt, dt, pushes, cores
 
 
-SAMPLE_CELLS = {1: 1024, 2: 25000, 3: 10000, 4: 40000, 5: 20000}  # ~4 M particles each (config 1: all of it)
+# oracle steps timed by the cpu_baseline leg: the full-size workload with a reduced step count (SURVEY.md section
+# 8(d): ">= 5 steps"; config 5 takes 10 so that one arrange is inside); configs 1 and 2 run their whole step count
+CPU_STEPS = {1: 200, 2: 100, 3: 5, 4: 5, 5: 10}
+
+
+def sample_text(config, inp, steps, what):
+    n0 = sum(len(s["x"]) for s in inp["species"])
+    return (f"BASELINE.json configs[{config - 1}] at full size ({n0} particles, {inp['nc']} cells, all species), "
+            f"{steps} of its {inp['steps']} steps, arrange every {inp['arrange_every']}, {what}")
+
+
+def cpu_baseline_block(config, inp):
+    steps = min(CPU_STEPS[config], inp["steps"])
+    v1, dt1, _, _ = oracle_run(inp, steps, None)
+    vt, dtt, _, cores = oracle_run(inp, steps, 0)
+    return {"value": v1, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt1,
+            "sample": sample_text(config, inp, steps, "oracle/oracle.c single thread"),
+            "threaded": {"value": vt, "unit": UNIT, "cores": cores, "kind": "oracle (threaded twin, bit-identical)",
+                         "seconds": dtt, "cpu_model": cpu_model(),
+                         "sample": sample_text(config, inp, steps, f"oracle/oracle_omp.c on {cores} threads")},
+            "host_cores_available": os.cpu_count(), "same_config": True}
 
 
 def run_reference(args, rank):
+    """--impl reference: no reference code exists (the paper ships none); per the task contract this arm is the CPU
+    oracle on the host cores: its threaded twin on all cores, on the full-size workload, for a bounded step count."""
     if rank != 0:
         return 0
-    steps_total = max(1, args.steps)
-    nc_s = SAMPLE_CELLS[args.config]
+    from paper_2603_24508_b200 import workloads
+    kw = {}
+    if args.scale != 1.0:
+        kw["nc"] = max(8, int(workloads.CONFIGS[args.config]["nc"] * args.scale))
+    inp = workloads.make(args.config, **kw)
+    n0 = sum(len(s["x"]) for s in inp["species"])
+    # each "step" of this arm = one oracle step over the whole workload; bound the CPU time to about a minute
+    steps = max(1, min(args.steps, inp["steps"], int(6e9 // max(n0, 1)) or 1))
     for _ in range(max(0, min(args.warmup, 1))):
-        oracle_sample(args.config, max(64, nc_s // 16), 1)
-    # each "step" of this arm = one oracle step over the bounded sample; cap the total CPU time
-    steps = min(steps_total, 50)
-    v, dt, pushes, desc = oracle_sample(args.config, nc_s, steps)
+        oracle_run(workloads.make(args.config, nc=max(64, inp["nc"] // 64)), 1, 0)
+    v, dt, pushes, cores = oracle_run(inp, steps, 0)
+    desc = sample_text(args.config, inp, steps, f"oracle/oracle_omp.c on {cores} threads")
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(args.config, None),
-            "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
+            "config": workload_config(args.config, inp),
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle (threaded twin, bit-identical)",
+                             "sample": desc, "cpu_model": cpu_model(), "same_config": True},
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0,
             "note": "no reference code exists (paper only): this arm is the CPU oracle on the host cores"}
+    if args.scale != 1.0:
+        line["config"]["workload"] += f" SCALED x{args.scale} (debug, not a bench value)"
     print(json.dumps(line), flush=True)
     return 0
 
@@ -262,6 +303,7 @@ def main():
     for k in ("mover", "hist", "scan", "scatter", "general", "fused"):
         pic.pic_kernel_time(sim, k)  # drop warm-up spans
     n_before = sum(pic.pic_n_slots(sp) for sp in sim.species)
+    fused0 = [pic.pic_fused_info(sp) for sp in sim.species]
     launches0 = pic.pic_launch_count(sim)
 
     uuid = str(torch.cuda.get_device_properties(dev).uuid)
@@ -274,6 +316,9 @@ def main():
     e0.record(stream)
     for _ in range(args.steps):
         step()
+    # A fused step that declines on the device is redone by the split kernels in the next synchronising call:
+    # force that call INSIDE the timed region, so that no skipped work can ever be timed as done.
+    pic.pic_sync(sim)
     e1.record(stream)
     torch.cuda.synchronize()
     if dist is not None:
@@ -287,6 +332,20 @@ def main():
     pushes = 0.5 * (n_before + n_after) * args.steps  # n_live changes only by wall absorption (negligible; exact if periodic)
     ktimes = {k: pic.pic_kernel_time(sim, k) for k in ("mover", "hist", "scan", "scatter", "general", "fused")}
     info = [pic.pic_arrange_info(sp) for sp in sim.species]
+    fused1 = [pic.pic_fused_info(sp) for sp in sim.species]
+    # which path the timed steps took: the fused step is expected whenever it was active at the start of the timed
+    # region; every timed step must then have been one completed fused launch, none redone by the split mover
+    expect_fused = all(f["active"] for f in fused0)
+    fused_path = {"expected": bool(expect_fused), "fused_steps": int(ktimes["fused"][1]),
+                  "split_mover_steps": int(ktimes["mover"][1]),
+                  "decline_reasons_before": [f["decline_reasons"] for f in fused0],
+                  "decline_reasons": [f["decline_reasons"] for f in fused1],
+                  "active_after": [f["active"] for f in fused1]}
+    invalid = None
+    if expect_fused and (ktimes["mover"][1] != 0 or ktimes["fused"][1] != args.steps * len(sim.species)
+                         or not all(f["active"] for f in fused1)
+                         or any(a["decline_reasons"] != b["decline_reasons"] for a, b in zip(fused0, fused1))):
+        invalid = "a fused step declined inside the timed region and was redone by the split kernels"
 
     ms_all, pushes_all = aggregate_over_ranks(dist, ms, pushes, dev)
     value = pushes_all / (ms_all * 1e-3)
@@ -368,25 +427,26 @@ def main():
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        v, dt_cpu, _, desc = oracle_sample(args.config, min(SAMPLE_CELLS[args.config], inp["nc"]), 50 if args.config != 1 else 200)
-        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc, "seconds": dt_cpu,
-               "host_cores_available": os.cpu_count()}
+        cpu = cpu_baseline_block(args.config, inp)
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warmup,
                 "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic", "config": workload_config(args.config, inp),
                 "clocks": sampler.result(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-                "cpu_baseline": cpu, "deposit": deposit,
+                "cpu_baseline": cpu, "deposit": deposit, "fused_path": fused_path,
                 "path": {"arranger": ["general" if g else "fast" for (_, g) in info],
                          "options": args.option, "numpy": np.__version__}}
         if args.scale != 1.0:
             line["config"]["scaled_nc"] = inp["nc"]
             line["config"]["workload"] += f" SCALED x{args.scale} (debug, not a bench value)"
+        if invalid:
+            line["invalid"] = True
+            line["invalid_reason"] = invalid
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
-    return 0
+    return 3 if invalid else 0
 
 
 if __name__ == "__main__":

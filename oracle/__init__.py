@@ -190,3 +190,65 @@ def arrange_arrays(x, vx, vy, vz, cell, nc):
     if nl < 0:
         raise RuntimeError("oracle_arrange failed")
     return o[0][:nl], o[1][:nl], o[2][:nl], o[3][:nl], co[:nl], count, offset, int(nl)
+
+
+# ---- field solve (oracle/oracle_field.c): smoother, Poisson solve, E from phi -------------------------------------
+_lib_field = None
+
+
+def lib_field():
+    global _lib_field
+    if _lib_field is None:
+        _lib_field = C.CDLL(_build.build_field())
+        dp = C.POINTER(C.c_double)
+        _lib_field.oracle_smooth.argtypes = [C.c_int32, C.c_int32, C.c_int32, dp, dp]
+        _lib_field.oracle_poisson.argtypes = [C.c_int32, C.c_double, C.c_int32, dp, dp]
+        _lib_field.oracle_efield.argtypes = [C.c_int32, C.c_double, C.c_int32, dp, dp]
+        _lib_field.oracle_field_solve.argtypes = [C.c_int32, C.c_double, C.c_int32, C.c_int32, dp, dp, dp, dp]
+        for f in (_lib_field.oracle_smooth, _lib_field.oracle_poisson, _lib_field.oracle_efield,
+                  _lib_field.oracle_field_solve):
+            f.restype = C.c_int
+    return _lib_field
+
+
+def _nodes(a, nc):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    assert a.shape == (nc + 1,)
+    return a
+
+
+def smooth(rho, nc, boundary, passes=1):
+    """oracle_smooth -> filtered rho on nc+1 nodes."""
+    out = np.zeros(nc + 1)
+    rc = lib_field().oracle_smooth(int(nc), int(boundary), int(passes), _d(_nodes(rho, nc)), _d(out))
+    if rc:
+        raise RuntimeError(f"oracle_smooth failed rc={rc}")
+    return out
+
+
+def poisson(rho, nc, dx, boundary):
+    """oracle_poisson -> phi on nc+1 nodes."""
+    phi = np.zeros(nc + 1)
+    rc = lib_field().oracle_poisson(int(nc), float(dx), int(boundary), _d(_nodes(rho, nc)), _d(phi))
+    if rc:
+        raise RuntimeError(f"oracle_poisson failed rc={rc}")
+    return phi
+
+
+def efield(phi, nc, dx, boundary):
+    """oracle_efield -> E on nc+1 nodes."""
+    E = np.zeros(nc + 1)
+    rc = lib_field().oracle_efield(int(nc), float(dx), int(boundary), _d(_nodes(phi, nc)), _d(E))
+    if rc:
+        raise RuntimeError(f"oracle_efield failed rc={rc}")
+    return E
+
+
+def field_solve(rho, nc, dx, boundary, passes=0):
+    """oracle_field_solve: smooth -> Poisson -> E.  -> (rho_smoothed, phi, E)."""
+    rs, phi, E = np.zeros(nc + 1), np.zeros(nc + 1), np.zeros(nc + 1)
+    rc = lib_field().oracle_field_solve(int(nc), float(dx), int(boundary), int(passes), _d(_nodes(rho, nc)), _d(rs),
+                                        _d(phi), _d(E))
+    if rc:
+        raise RuntimeError(f"oracle_field_solve failed rc={rc}")
+    return rs, phi, E

@@ -41,6 +41,7 @@ constexpr int FUSED_STAGES_DEFAULT = 1;    // stages of the shared-memory ring (
 constexpr int FUSED_KMAX = 31;         // cells per tile (one lane per cell border)
 constexpr int FUSED_DEF = 32;          // deferred right-movers of a tile's last cell
 constexpr int FUSED_XCAP = 256;        // edge kernel: leavers per edge cell
+constexpr int FUSED_TELEMETRY_STEPS = 4; // fused steps between two asynchronous copies of DevState to the host
 constexpr int FUSED_RETRY_STEPS = 16;  // split steps after a decline before the fused path is tried again
 constexpr int FUSED_SMEM_SM = 233472;  // shared memory per SM (228 KB), 1 KB reserved per CTA
 
@@ -659,7 +660,8 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
         }
     }
 
-    // ---- CTA epilogue; the last CTA commits or rolls back the step ----------------------------------
+    // ---- CTA epilogue: report a decline and the largest new per-cell count.  No fence, no arrival counter: the step
+    // is committed or rolled back by fused_commit_kernel, launched behind this kernel on the same stream.
     bad = (int)__reduce_or_sync(FULL, (unsigned)bad);
     mc = __reduce_max_sync(FULL, mc);
     if (lane == 0) {
@@ -668,36 +670,35 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
             atomicOr(&st->abort_reason, bad);
         }
         if (mc > *(volatile int *)&st->maxcount_next) atomicMax(&st->maxcount_next, mc);
-        __threadfence();
-        const unsigned d = atomicAdd(&st->done, 1u);
-        if (d == gridDim.x - 1u) {
-            __threadfence();
-            if (!*(volatile int *)&st->abort) {
-                st->n = *(volatile int *)&st->n_next;
-                st->wall[0] += *(volatile unsigned long long *)&st->wall_pend[0];
-                st->wall[1] += *(volatile unsigned long long *)&st->wall_pend[1];
-                st->vmax2 = 0x7f800000u; // speed bound unknown after a fused step (+inf): the split path, should it
-                                         // take over, enqueues its general arranger until its mover has measured one
-                st->maxcount = *(volatile int *)&st->maxcount_next;
-                st->w_acc = 0;
-                st->step_max = 0;
-                st->need_general = 0;
-                st->used_general = 0;
-                st->run_split = 0;
-            } else {
-                // declined: nothing of the state was touched (outputs went to the other buffer set); remember which
-                // step it was, every later fused launch exits at once, the host redoes the steps (pic.cu: verify_fused)
-                if (!st->fused_disabled) st->fail_step = a.step_id;
-                st->fused_disabled = 1;
-            }
-            st->n_next = 0;
-            st->wall_pend[0] = st->wall_pend[1] = 0;
-            st->vmax2_next = 0;
-            st->maxcount_next = 0;
-            st->done = 0;
-            st->abort = 0;
-        }
     }
+}
+
+// Commit or roll back one fused step (one thread, launched behind fused_kernel; the kernel boundary orders it
+// after every CTA's stores and atomics).
+__global__ void fused_commit_kernel(DevState *st, int step_id)
+{
+    if (!st->abort) {
+        st->n = st->n_next;
+        st->wall[0] += st->wall_pend[0];
+        st->wall[1] += st->wall_pend[1];
+        st->vmax2 = 0x7f800000u; // speed bound unknown after a fused step (+inf): the split path, should it
+                                 // take over, enqueues its general arranger until its mover has measured one
+        st->maxcount = st->maxcount_next;
+        st->w_acc = 0;
+        st->step_max = 0;
+        st->need_general = 0;
+        st->used_general = 0;
+    } else {
+        // declined: nothing of the state was touched (outputs went to the other buffer set); remember which
+        // step it was, every later fused launch exits at once, the host redoes the steps (pic.cu: verify_fused)
+        if (!st->fused_disabled) st->fail_step = step_id;
+        st->fused_disabled = 1;
+    }
+    st->n_next = 0;
+    st->wall_pend[0] = st->wall_pend[1] = 0;
+    st->vmax2_next = 0;
+    st->maxcount_next = 0;
+    st->abort = 0;
 }
 
 // Largest per-cell count of an offset array (sizes the fused tiles; only ever raises the bound).

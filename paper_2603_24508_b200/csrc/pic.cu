@@ -52,7 +52,14 @@ struct pic_species {
     size_t scan_words = 0;
     // fused push+arrange step (fused.cuh)
     double2 *d_cs = nullptr;           // deposition: per-cell partial sums (allocated at the first pic_deposit)
-    int h_maxcount = 0;                // bound of the largest per-cell count at the last sync (sizes the fused tiles)
+    int h_maxcount = 0;                // bound of the largest per-cell count last seen by the host (sizes the fused tiles)
+    // asynchronous telemetry of the fused path: every few fused steps the device state is copied to pinned host
+    // memory without waiting; push_fused reads the latest copy that has landed (the largest per-cell count drifts
+    // over a long pic_push without any synchronising call, and a cell that outgrows the tile declines the step)
+    DevState *h_tel = nullptr;
+    cudaEvent_t tel_ev = nullptr;
+    bool tel_pending = false;
+    long long tel_step = 0;            // fused steps since the last telemetry copy was enqueued
     int h_abort_reason = 0;
     bool fused_off = false;            // the device reported a declined fused step (sticky)
     // fused steps enqueued but not yet verified (verify_fused): how many, and the host state when the run began
@@ -151,6 +158,8 @@ static void free_species(pic_species *s)
     for (int b = 0; b < 2; ++b) { cudaFree(s->d_count[b]); cudaFree(s->d_off[b]); }
     cudaFree(s->d_scan);
     cudaFree(s->d_cs);
+    if (s->h_tel) cudaFreeHost(s->h_tel);
+    if (s->tel_ev) cudaEventDestroy(s->tel_ev);
     delete s;
 }
 
@@ -293,6 +302,8 @@ static int create_species(pic_sim *sim, const pic_species_desc &d, pic_species *
     long long max_scan = std::max<long long>((long long)nc + 1, general_scan_elems(d.capacity));
     s->scan_words = scan_scratch_words(max_scan);
     CU(cudaMalloc(&s->d_scan, s->scan_words * sizeof(unsigned long long)));
+    CU(cudaMallocHost(&s->h_tel, sizeof(DevState)));
+    CU(cudaEventCreateWithFlags(&s->tel_ev, cudaEventDisableTiming));
 
     DevState h{};
     h.n = (int)d.n;
@@ -641,8 +652,14 @@ static FusedGeom fused_geom(const pic_species *s)
 {
     const pic_sim *sim = s->sim;
     FusedGeom g{};
+    // Largest cell a tile must hold: the largest count last seen (telemetry lags a few steps: leave 1/16 + 8), and
+    // never less than the expected maximum of nc Poisson counts of the mean occupancy -- a state that starts with
+    // exactly equal counts (the configs do) reaches that within a few steps.
     const int mc = std::max(s->h_maxcount, 1);
-    const int need = mc + std::max(mc / 4, 32) + 2;
+    const double mean = (double)s->n_ub / (double)sim->nc;
+    const int poisson_max = (int)std::ceil(mean + std::sqrt(2.0 * mean * std::log((double)sim->nc + 1.0)));
+    const int top = std::max(mc, poisson_max);
+    const int need = top + top / 16 + 8 + 2;
     g.rows = sim->opt_fused_rows;
     if (g.rows == 0) g.rows = need <= 8 * 32 ? 8 : need <= 12 * 32 ? 12 : need <= 16 * 32 ? 16 : 0;
     if (g.rows == 0) return g;
@@ -668,6 +685,17 @@ static int fused_rows(const pic_species *s, int *ctas_per_sm)
 static int push_fused(pic_species *s)
 {
     pic_sim *sim = s->sim;
+    if (s->tel_pending) { // has a telemetry copy landed?  (never waits)
+        const cudaError_t q = cudaEventQuery(s->tel_ev);
+        if (q == cudaSuccess) {
+            s->tel_pending = false;
+            if (!s->h_tel->fused_disabled) s->h_maxcount = s->h_tel->maxcount;
+        } else if (q == cudaErrorNotReady) {
+            cudaGetLastError(); // not an error: clear it so that the launch checks below do not see it
+        } else {
+            return cuda_fail(q, "cudaEventQuery telemetry");
+        }
+    }
     const int src = s->cur, dst = s->cur ^ 1;
     const int oo = s->cur_off, on = s->cur_off ^ 1;
     FusedArgs a{};
@@ -704,6 +732,14 @@ static int push_fused(pic_species *s)
 #undef PIC_FUSED_PICK
         kern<<<grid, 32, smem, sim->stream>>>(a);
         if (int rc = launch_check(sim, "fused_kernel")) return rc;
+        fused_commit_kernel<<<1, 1, 0, sim->stream>>>(s->d_st, a.step_id);
+        if (int rc = launch_check(sim, "fused_commit_kernel")) return rc;
+    }
+    if (++s->tel_step >= FUSED_TELEMETRY_STEPS && !s->tel_pending) {
+        CU(cudaMemcpyAsync(s->h_tel, s->d_st, sizeof(DevState), cudaMemcpyDeviceToHost, sim->stream));
+        CU(cudaEventRecord(s->tel_ev, sim->stream));
+        s->tel_pending = true;
+        s->tel_step = 0;
     }
     s->unv_steps++;
     s->h_steps_since_sync++;

@@ -27,13 +27,11 @@ struct DevState {
     int status;       // ERR_* bits
     int need_general; // fast arranger declined (w_acc too large); the general path must run
     int used_general; // the last arrange ran the general path
-    int run_split;      // unused (kept for layout)
     int fused_disabled; // sticky: a fused step has declined (fail_step says which); later fused launches exit at once
     unsigned long long wall[2];      // cumulative absorbed at x<0 / x>=L
     unsigned long long wall_pend[2]; // fused step in flight: absorbed, not yet committed
     unsigned vmax2, vmax2_next;      // float bits (rounded up) of max |v|^2: current state / step in flight
     int n_next;                      // fused step in flight: particle count after it
-    unsigned done;                   // fused step: finished CTAs
     int abort;                       // fused step in flight: some CTA declined
     int abort_reason;                // FA_* bits of every decline so far (diagnostics)
     int f_OL, f_AR;                  // fused step in flight: leavers of cell 0 downwards / wrapped arrivals in cell 0

@@ -1,0 +1,260 @@
+"""Pins for the field-solve oracle (oracle/oracle_field.c: 1-2-1 smoother, 1D Poisson solve, E from phi; PIC phase
+(iii); readings S23-S28 of DESIGN.md section 12).  CPU only.
+
+None of these re-calls the oracle or retypes its elimination: they are closed forms of the discrete operator
+(parabola, sine eigenvectors, the Green's function of a point charge), the defining residual evaluated in extended
+precision, the discrete Gauss law, library routines on small grids (numpy.linalg.solve, scipy solve_banded,
+numpy.convolve), and invariants (gauge, neutralisation, charge conservation of the filter).  A dropped dx^2, a wrong
+sign of rho or E, a shifted node, a centred difference without the 1/2, a wall treated as periodic -- each fails
+at least one of them.
+"""
+import math
+
+import numpy as np
+import pytest
+import scipy.linalg
+
+import oracle
+from oracle import ABSORBING, PERIODIC
+
+LD = np.longdouble
+
+
+def residual_ld(phi, rho, dx, nodes):
+    """(phi[j-1] - 2 phi[j] + phi[j+1])/dx^2 + rho[j] at the given nodes, in extended precision."""
+    p = phi.astype(LD)
+    out = []
+    n = len(phi) - 1
+    for j in nodes:
+        jm, jp = (j - 1) % n, (j + 1) % n  # wraps only matter on the periodic grid (nodes 0..nc-1)
+        out.append((p[jm] - 2 * p[j] + p[jp]) / LD(dx) ** 2 + LD(rho[j]))
+    return np.array(out, dtype=LD)
+
+
+# ------------------------------------------------------------------------------------------------ Poisson, bounded
+@pytest.mark.parametrize("nc,dx,rho0", [(8, 1.0, 1.0), (100, 0.5, -2.5), (1000, 0.125, 0.75)])
+def test_uniform_rho_gives_the_exact_parabola(nc, dx, rho0):
+    phi = oracle.poisson(np.full(nc + 1, rho0), nc, dx, ABSORBING)
+    j = np.arange(nc + 1, dtype=np.float64)
+    want = rho0 * dx * dx * j * (nc - j) / 2.0  # the second difference of a quadratic is exact on the grid
+    assert phi[0] == 0.0 and phi[nc] == 0.0
+    # the elimination runs in long double (S28): the binary64 result is the exact parabola to a few ulp
+    assert np.max(np.abs(phi - want)) <= 4 * np.finfo(np.float64).eps * np.max(np.abs(want))
+
+
+@pytest.mark.parametrize("m", [1, 2, 7])
+def test_dirichlet_sine_modes_are_eigenvectors(m):
+    nc, dx = 64, 0.5
+    j = np.arange(nc + 1)
+    rho = np.sin(math.pi * m * j / nc)
+    lam = (2.0 - 2.0 * math.cos(math.pi * m / nc)) / dx ** 2
+    phi = oracle.poisson(rho, nc, dx, ABSORBING)
+    assert np.max(np.abs(phi - rho / lam)) <= 1e-13 * np.max(np.abs(rho / lam))
+
+
+def test_point_charge_gives_the_piecewise_linear_greens_function():
+    nc, dx, k, q = 50, 0.25, 17, 3.0
+    rho = np.zeros(nc + 1)
+    rho[k] = q
+    phi = oracle.poisson(rho, nc, dx, ABSORBING)
+    j = np.arange(nc + 1, dtype=np.float64)
+    want = q * dx * dx * np.where(j <= k, j * (nc - k), k * (nc - j)) / nc
+    assert np.max(np.abs(phi - want)) <= 1e-13 * want.max()
+    assert phi[0] == 0.0 and phi[nc] == 0.0  # grounded walls (S24)
+
+
+def test_wall_nodes_of_rho_do_not_enter_the_bounded_solve():
+    rng = np.random.default_rng(3)
+    nc = 40
+    rho = rng.normal(size=nc + 1)
+    a = oracle.poisson(rho, nc, 1.0, ABSORBING)
+    rho2 = rho.copy()
+    rho2[0] += 100.0
+    rho2[nc] -= 55.0
+    assert np.array_equal(a, oracle.poisson(rho2, nc, 1.0, ABSORBING))
+
+
+@pytest.mark.parametrize("nc,dx", [(16, 1.0), (257, 0.3), (5000, 1.0)])
+def test_bounded_residual_and_gauss_law(nc, dx):
+    rng = np.random.default_rng(nc)
+    rho = rng.normal(size=nc + 1)
+    phi = oracle.poisson(rho, nc, dx, ABSORBING)
+    res = residual_ld(phi, rho, dx, range(1, nc))
+    scale = np.max(np.abs(phi)) / dx ** 2 + np.max(np.abs(rho))
+    assert float(np.max(np.abs(res))) <= 64 * np.finfo(np.float64).eps * scale
+    # discrete Gauss law on the half nodes: E_{j+1/2} - E_{j-1/2} = rho_j dx, with E_{j+1/2} = -(phi_{j+1}-phi_j)/dx
+    p = phi.astype(LD)
+    Eh = -(p[1:] - p[:-1]) / LD(dx)
+    gauss = (Eh[1:] - Eh[:-1]) - rho[1:nc].astype(LD) * LD(dx)
+    assert float(np.max(np.abs(gauss))) <= 64 * np.finfo(np.float64).eps * scale * dx
+
+
+@pytest.mark.parametrize("nc", [3, 10, 64])
+def test_bounded_solve_matches_library_solvers(nc):
+    rng = np.random.default_rng(100 + nc)
+    dx = 0.7
+    rho = rng.normal(size=nc + 1)
+    phi = oracle.poisson(rho, nc, dx, ABSORBING)
+    m = nc - 1
+    A = 2.0 * np.eye(m) - np.eye(m, k=1) - np.eye(m, k=-1)
+    ref = np.linalg.solve(A, dx * dx * rho[1:nc])
+    assert np.max(np.abs(phi[1:nc] - ref)) <= 1e-12 * np.max(np.abs(ref))
+    ab = np.zeros((3, m))
+    ab[0, 1:] = -1.0
+    ab[1, :] = 2.0
+    ab[2, :-1] = -1.0
+    ref2 = scipy.linalg.solve_banded((1, 1), ab, dx * dx * rho[1:nc])
+    assert np.max(np.abs(phi[1:nc] - ref2)) <= 1e-12 * np.max(np.abs(ref2))
+
+
+# ------------------------------------------------------------------------------------------------ Poisson, periodic
+@pytest.mark.parametrize("m", [1, 3, 16])
+def test_periodic_sine_modes_are_eigenvectors(m):
+    nc, dx = 64, 2.0
+    j = np.arange(nc + 1)
+    rho = np.cos(2 * math.pi * m * j / nc + 0.3)
+    lam = (2.0 - 2.0 * math.cos(2 * math.pi * m / nc)) / dx ** 2
+    phi = oracle.poisson(rho, nc, dx, PERIODIC)
+    assert np.max(np.abs(phi - rho / lam)) <= 1e-12 * np.max(np.abs(rho / lam))
+    assert phi[nc] == phi[0]
+
+
+def test_periodic_neutralisation_gauge_and_residual():
+    rng = np.random.default_rng(8)
+    nc, dx = 300, 0.4
+    rho = rng.normal(size=nc + 1) + 5.0  # a net charge: the uniform background removes it (S25)
+    rho[nc] = rho[0]
+    phi = oracle.poisson(rho, nc, dx, PERIODIC)
+    assert abs(phi[:nc].sum()) <= 1e-12 * np.abs(phi).sum()  # zero mean over the nc distinct nodes
+    assert phi[nc] == phi[0]
+    shifted = oracle.poisson(rho - 5.0, nc, dx, PERIODIC)  # adding a constant to rho changes nothing
+    assert np.max(np.abs(phi - shifted)) <= 1e-11 * np.max(np.abs(phi))
+    rho_n = rho - rho[:nc].mean()
+    res = residual_ld(phi, rho_n, dx, range(0, nc))  # includes node 0, whose equation closes the ring
+    scale = np.max(np.abs(phi)) / dx ** 2 + np.max(np.abs(rho))
+    assert float(np.max(np.abs(res))) <= 1e-12 * scale
+    # translation invariance of the ring: rolling rho rolls phi
+    k = 37
+    rolled = np.empty_like(rho)
+    rolled[:nc] = np.roll(rho[:nc], k)
+    rolled[nc] = rolled[0]
+    phi_r = oracle.poisson(rolled, nc, dx, PERIODIC)
+    assert np.max(np.abs(phi_r[:nc] - np.roll(phi[:nc], k))) <= 1e-10 * np.max(np.abs(phi))
+
+
+def test_periodic_solve_matches_dense_least_norm_solution():
+    rng = np.random.default_rng(21)
+    nc, dx = 24, 1.5
+    rho = rng.normal(size=nc + 1)
+    rho[nc] = rho[0]
+    A = 2.0 * np.eye(nc) - np.roll(np.eye(nc), 1, axis=1) - np.roll(np.eye(nc), -1, axis=1)
+    b = dx * dx * (rho[:nc] - rho[:nc].mean())
+    ref = np.linalg.lstsq(A, b, rcond=None)[0]  # minimum-norm solution = the zero-mean one
+    phi = oracle.poisson(rho, nc, dx, PERIODIC)
+    assert np.max(np.abs(phi[:nc] - ref)) <= 1e-12 * np.max(np.abs(ref))
+
+
+# ------------------------------------------------------------------------------------------------ E from phi
+def test_efield_of_linear_and_quadratic_potentials_bounded():
+    nc, dx, a = 20, 0.5, 3.0
+    j = np.arange(nc + 1, dtype=np.float64)
+    E = oracle.efield(a * j * dx, nc, dx, ABSORBING)  # phi = a x  ->  E = -a everywhere, walls included
+    assert np.max(np.abs(E + a)) <= 1e-14 * a
+    phi = (j * dx) ** 2  # E = -2x in the interior (centred difference exact); one-sided at the walls
+    E = oracle.efield(phi, nc, dx, ABSORBING)
+    assert np.max(np.abs(E[1:nc] + 2.0 * j[1:nc] * dx)) <= 1e-13 * 2 * nc * dx
+    assert abs(E[0] - (-(phi[1] - phi[0]) / dx)) <= 1e-15 and abs(E[0] + dx) <= 1e-14  # -(dx^2)/dx
+    assert abs(E[nc] - (-(phi[nc] - phi[nc - 1]) / dx)) <= 1e-13
+    assert abs(E[nc] + (2 * nc - 1) * dx) <= 1e-13 * nc
+
+
+def test_efield_periodic_wraps_and_mirrors_node_nc():
+    nc, dx = 32, 0.25
+    j = np.arange(nc + 1)
+    phi = np.sin(2 * math.pi * j / nc)
+    phi[nc] = phi[0]
+    E = oracle.efield(phi, nc, dx, PERIODIC)
+    want = -(np.roll(phi[:nc], -1) - np.roll(phi[:nc], 1)) / (2 * dx)
+    assert np.max(np.abs(E[:nc] - want)) <= 1e-14 * np.max(np.abs(want))
+    assert E[nc] == E[0]
+    # sign: E = -dphi/dx, so E at node 0 of sin is negative
+    assert E[0] < 0
+
+
+def test_sign_chain_positive_charge_makes_a_potential_hill():
+    nc = 10
+    rho = np.zeros(nc + 1)
+    rho[5] = 1.0
+    rs, phi, E = oracle.field_solve(rho, nc, 1.0, ABSORBING, passes=0)
+    assert np.array_equal(rs, rho)
+    assert phi[5] == phi.max() > 0.0
+    assert E[3] < 0 < E[7]  # the field points away from a positive charge
+
+
+# ------------------------------------------------------------------------------------------------ smoother
+@pytest.mark.parametrize("boundary", [PERIODIC, ABSORBING])
+@pytest.mark.parametrize("passes", [1, 2, 5])
+def test_filter_conserves_charge_and_constants(boundary, passes):
+    rng = np.random.default_rng(passes)
+    nc = 33 if boundary == ABSORBING else 32
+    rho = rng.normal(size=nc + 1)
+    if boundary == PERIODIC:
+        rho[nc] = rho[0]
+    out = oracle.smooth(rho, nc, boundary, passes)
+    if boundary == PERIODIC:
+        assert abs(out[:nc].sum() - rho[:nc].sum()) <= 1e-13 * np.abs(rho).sum()
+        assert out[nc] == out[0]
+    else:
+        assert abs(out.sum() - rho.sum()) <= 1e-13 * np.abs(rho).sum()
+    c = np.full(nc + 1, 2.75)
+    assert np.array_equal(oracle.smooth(c, nc, boundary, passes), c)
+    # k passes = k single passes
+    it = rho
+    for _ in range(passes):
+        it = oracle.smooth(it, nc, boundary, 1)
+    assert np.array_equal(it, out)
+    assert np.array_equal(oracle.smooth(rho, nc, boundary, 0), rho)
+
+
+def test_filter_annihilates_the_nyquist_mode_on_the_ring():
+    nc = 16
+    rho = np.array([(-1.0) ** j for j in range(nc + 1)])
+    assert rho[nc] == rho[0]
+    assert np.array_equal(oracle.smooth(rho, nc, PERIODIC, 1), np.zeros(nc + 1))
+
+
+def test_filter_delta_responses_and_numpy_convolve():
+    nc = 12
+    d = np.zeros(nc + 1)
+    d[5] = 1.0
+    assert np.array_equal(oracle.smooth(d, nc, ABSORBING, 1)[3:8], [0, 0.25, 0.5, 0.25, 0])
+    w = np.zeros(nc + 1)
+    w[0] = 1.0
+    out = oracle.smooth(w, nc, ABSORBING, 1)
+    assert out[0] == 0.75 and out[1] == 0.25 and out[2:].sum() == 0.0  # reflected quarter (S27)
+    w = np.zeros(nc + 1)
+    w[nc] = 1.0
+    out = oracle.smooth(w, nc, ABSORBING, 1)
+    assert out[nc] == 0.75 and out[nc - 1] == 0.25
+    p = np.zeros(nc + 1)
+    p[0] = p[nc] = 1.0  # one point of the ring
+    out = oracle.smooth(p, nc, PERIODIC, 1)
+    assert out[0] == 0.5 and out[1] == 0.25 and out[nc - 1] == 0.25 and out[nc] == 0.5
+    rng = np.random.default_rng(0)
+    rho = rng.normal(size=nc + 1)
+    ref = np.convolve(rho, [0.25, 0.5, 0.25], mode="same")
+    got = oracle.smooth(rho, nc, ABSORBING, 1)
+    assert np.max(np.abs(got[1:nc] - ref[1:nc])) <= 1e-15
+
+
+def test_field_solve_is_the_composition():
+    rng = np.random.default_rng(4)
+    for boundary in (PERIODIC, ABSORBING):
+        nc, dx = 64, 0.5
+        rho = rng.normal(size=nc + 1)
+        if boundary == PERIODIC:
+            rho[nc] = rho[0]
+        rs, phi, E = oracle.field_solve(rho, nc, dx, boundary, passes=2)
+        assert np.array_equal(rs, oracle.smooth(rho, nc, boundary, 2))
+        assert np.array_equal(phi, oracle.poisson(rs, nc, dx, boundary))
+        assert np.array_equal(E, oracle.efield(phi, nc, dx, boundary))
