@@ -256,6 +256,9 @@ def main():
     ap.add_argument("--no-deposit", action="store_true", help="skip the separate timing of pic_deposit")
     ap.add_argument("--option", action="append", default=[], help="pic_set_option key=value (e.g. fused=0)")
     ap.add_argument("--scale", type=float, default=1.0, help="scale nc (debug only; the line is then not a bench value)")
+    ap.add_argument("--debug-fast-particle", type=float, default=None, metavar="VZ",
+                    help="debug only (tests of the decline guard): give particle 7777 of species 0 the velocity (0, 0, VZ) "
+                         "so that it jumps two cells after a few gyration steps and a fused step declines")
     args = ap.parse_args()
     rank, local_rank, world = env_rank()
     if args.impl == "reference":
@@ -280,6 +283,9 @@ def main():
     if args.scale != 1.0:
         kw["nc"] = max(8, int(workloads.CONFIGS[args.config]["nc"] * args.scale))
     inp = workloads.make(args.config, replica=rank, **kw)
+    if args.debug_fast_particle is not None:
+        s0 = inp["species"][0]
+        s0["vx"][7777], s0["vy"][7777], s0["vz"][7777] = 0.0, 0.0, args.debug_fast_particle
     ae = inp["arrange_every"]
     stream = torch.cuda.Stream(device=dev)
     with torch.cuda.stream(stream):
@@ -440,6 +446,8 @@ def main():
         if args.scale != 1.0:
             line["config"]["scaled_nc"] = inp["nc"]
             line["config"]["workload"] += f" SCALED x{args.scale} (debug, not a bench value)"
+        if args.debug_fast_particle is not None:
+            line["config"]["workload"] += " with an injected fast particle (debug, not a bench value)"
         if invalid:
             line["invalid"] = True
             line["invalid_reason"] = invalid

@@ -137,12 +137,43 @@ int pic_wall_flux(pic_species *sp, pic_wall_flux_t *out);
  * arranged slots.  Deterministic (fixed summation tree); agrees with a sequential sum to rounding. */
 int pic_deposit(pic_species *sp, double weight, double *rho_dev, int accumulate);
 
-/* Replace E (HOST, nc+1 doubles, copied; stream-ordered). */
+/* Replace E from a HOST array (nc+1 doubles, copied).  Steps already enqueued run with the old field.  Syncs (the
+ * caller's array may be pageable, and unchecked fused steps are checked first).  PIC_EINVAL for a non-finite value. */
 int pic_set_field(pic_sim *sim, const double *E_nodes_host);
+
+/* Replace E from a DEVICE array (nc+1 doubles, copied device-to-device on the sim's stream): the field stays
+ * resident on the device between steps ("keep resident"; PAPER.md:148 raw device pointers).
+ * Stream-ordered, no host round trip of the field; the caller's array must be ready on the sim's stream.  max |E|
+ * (the host's bound on what one step can displace a particle) is reduced on the device and read at the next
+ * synchronising call; until then the split arranger also enqueues its (guarded) general path.  Unchecked fused
+ * steps are checked first, which syncs only if there are any. */
+int pic_set_field_device(pic_sim *sim, const double *E_nodes_dev);
+
+/* The field solve, PIC phase (iii): "the field solver, which computes the electric ... fields by solving ...
+ * Poisson's equations" with BIT1's "native Poisson solver ... and smoothing operators".
+ * The paper prints neither; readings S23-S28 of DESIGN.md section 12 (normalised, epsilon_0 = 1):
+ *   1. smooth_passes passes of the 1-2-1 binomial filter rho'[j] = (rho[j-1] + 2 rho[j] + rho[j+1])/4 (periodic:
+ *      wraps over the nc distinct nodes; absorbing walls: the quarter leaving the grid is reflected, charge kept);
+ *   2. (phi[j-1] - 2 phi[j] + phi[j+1])/dx^2 = -rho'[j]; absorbing: phi[0] = phi[nc] = 0; periodic: rho' neutralised
+ *      by a uniform background, phi of zero mean, phi[nc] = phi[0];
+ *   3. E[j] = -(phi[j+1] - phi[j-1])/(2 dx), one-sided at absorbing walls, wrapped on a periodic grid; E replaces
+ *      the sim's field on the device (as pic_set_field_device).
+ * rho_dev: DEVICE, nc+1 doubles (what pic_deposit writes), read only, ready on the sim's stream.  phi_dev: DEVICE,
+ * nc+1 doubles, receives phi, or NULL.  Asynchronous on the stream (unchecked fused steps are checked first).
+ * Deterministic (fixed summation trees); agrees with a sequential elimination to rounding: within 1e-12 of
+ * max |phi|.  PIC_EINVAL: NULL, smooth_passes outside [0, 1024], nc < 2. */
+int pic_solve_field(pic_sim *sim, const double *rho_dev, int smooth_passes, double *phi_dev);
+
+/* Copy the field in force (nc+1 doubles) to a HOST array.  Syncs. */
+int pic_get_field(pic_sim *sim, double *E_nodes_host);
 
 /* Number of slots in use: n_live after an arrange, else n at the last arrange (dead
  * particles included).  Syncs. */
 int pic_n_slots(pic_species *sp, int64_t *n);
+
+/* Number of live particles now: the slots in use minus the particles absorbed at the walls (flagged, still in
+ * their slots) since the last arrange.  Equal to pic_n_slots right after an arrange.  Syncs. */
+int pic_n_live(pic_species *sp, int64_t *n);
 
 /* Which buffer set (0 or 1) holds the current state.  Syncs if fused steps are still unchecked (a
  * declined fused step is redone by the split kernels here, as in every synchronising call);
@@ -178,19 +209,22 @@ size_t pic_workspace_bytes(int32_t nc, int64_t capacity);
 /* Variant switches and tuning knobs, for measurements (profiles/ compares them).  Flags (0/1):
  * "fused": 1 = single-pass push+arrange when arrange_every == 1 (default; particles and the E
  * nodes of each chunk staged in shared memory by TMA bulk copies), 0 = separate mover / scan /
- * scatter kernels (E through the read-only global path); "kernel_timing": 1 = record CUDA events
+ * scatter kernels (E through the read-only global path); "fused_tma": 1 = the fused step stages particles and E by TMA bulk copies (default),
+ * 0 = it reads them with plain read-only global loads (the A/B variant of profiles/); "kernel_timing": 1 = record CUDA events
  * around every kernel launch (see pic_kernel_time).  Knobs of the fused step:
  * "fused_cells_per_cta" (cells per chunk, 1..256; 0 = automatic: 32 on large grids), "fused_rows" (rows
  * of 32 slots per tile: 8, 12 or 16; 0 = automatic from the largest per-cell count),
  * "fused_stage_slots" (largest tile in slots, even, <= 32*rows; 0 = 32*rows), "fused_stages"
- * (stages of the TMA ring: 1 or 2; 0 = default 1).  Results never depend on any of them.
+ * (stages of the TMA ring: 1 or 2; 0 = automatic: 2 under 8-row tiles, else 1), "fused_pdl" (1 = the streaming
+ * kernel is launched with programmatic dependent launch and overlaps its prologue with the edge kernel, default;
+ * 0 = plain stream order).  Results never depend on any of them.
  * PIC_EINVAL for an unknown key or a value out of range. */
 int pic_set_option(pic_sim *sim, const char *key, int value);
 
 /* Device time of one kernel class since the previous query of that class, measured with CUDA
  * event pairs recorded on the sim's stream around each of its launches while option
  * "kernel_timing" is 1 (default 0: nothing is recorded).  kernel is one of "mover", "hist",
- * "scan", "scatter", "general", "fused", "deposit".  *ms_total = summed milliseconds, *spans = number of
+ * "scan", "scatter", "general", "fused", "deposit", "field".  *ms_total = summed milliseconds, *spans = number of
  * timed launches (either may be NULL).  Syncs.  PIC_EINVAL for an unknown name. */
 int pic_kernel_time(pic_sim *sim, const char *kernel, double *ms_total, uint64_t *spans);
 

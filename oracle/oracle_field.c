@@ -31,11 +31,14 @@
  *            filter  ((rho[j-1] + 2*rho[j]) + rho[j+1]) * 0.25   (the products by 2 and 0.25 are exact)
  *            E       (phi[j+1] - phi[j-1]) * (-0.5*inv_dx),  one-sided (phi[1] - phi[0]) * (-inv_dx)
  *        Solve: the textbook Thomas algorithm for  -phi[j-1] + 2 phi[j] - phi[j+1] = dx^2 rho[j], as written
- *        below, with its recurrences carried in `long double` and phi rounded to binary64 at the end.  The
- *        solution of the linear system is what is defined; a sequential elimination in binary64 carries its
- *        own rounding error of order eps*nc relative to max|phi| (measured: 3.7e-13 at nc = 1000 for uniform
- *        rho, i.e. ~4e-10 at the 10^6 nodes of config 4), which would make the oracle, not the kernel, the
- *        larger error at the 1e-12 parity bar.  Inputs and outputs are binary64.
+ *        below, with its recurrences carried in binary128 (`xreal`: __float128 where the compiler has it, i.e.
+ *        x86-64; `long double`, which is binary128, on aarch64) and phi rounded to binary64 at the end.  The
+ *        solution of the linear system is what is defined, and a sequential elimination accumulates its own
+ *        rounding error systematically: in binary64 3.7e-13 of max|phi| at nc = 1000 (uniform rho), and even in
+ *        the 64-bit-mantissa x87 long double 1.8e-13 at nc = 10^5 and 8.7e-12 at nc = 10^6 (measured against an
+ *        extended-precision double prefix sum, which the CUDA path matched to 1e-14).  At the 1e-12 parity bar the
+ *        oracle, not the kernel, would be the larger error; in binary128 its own error is below 1e-25.
+ *        Inputs and outputs are binary64.
  *
  * The solve reaches, up to rounding, a result with a plain definition (the solution of a linear system);
  * the oracle is the textbook sequential elimination.  Pins (tests/test_oracle_field.py, "-m not gpu";
@@ -54,6 +57,15 @@
 
 #define ORACLE_PERIODIC 0
 #define ORACLE_ABSORBING 1
+
+/* the precision the elimination is carried in (S28) */
+#if defined(__SIZEOF_FLOAT128__) && !defined(__aarch64__)
+typedef __float128 xreal;
+#define XABS(v) ((v) < 0 ? -(v) : (v))
+#else
+typedef long double xreal;
+#define XABS(v) fabsl(v)
+#endif
 
 /* S27: `passes` passes of the 1-2-1 filter; in and out have nc+1 entries and may be the same array. */
 int oracle_smooth(int32_t nc, int32_t boundary, int32_t passes, const double *rho_in, double *rho_out)
@@ -90,25 +102,61 @@ int oracle_smooth(int32_t nc, int32_t boundary, int32_t passes, const double *rh
 }
 
 /* Thomas algorithm for  -u[j-1] + 2 u[j] - u[j+1] = r[j],  j = 1..m,  u[0] = u[m+1] = 0.
- * r and u are indexed 1..m (arrays of m+2 entries); cp, dp scratch of m+2 entries.  long double (S28). */
-static void thomas_121(int32_t m, const long double *r, long double *u, long double *cp, long double *dp)
+ * r and u are indexed 1..m (arrays of m+2 entries); cp, dp scratch of m+2 entries.  binary128 (S28). */
+static void thomas_121(int32_t m, const xreal *r, xreal *u, xreal *cp, xreal *dp)
 {
-    u[0] = 0.0L;
-    u[m + 1] = 0.0L;
+    u[0] = (xreal)0.0;
+    u[m + 1] = (xreal)0.0;
     if (m < 1) return;
-    cp[1] = -0.5L;            /* c/b = -1/2 */
-    dp[1] = r[1] * 0.5L;      /* r/b */
+    cp[1] = -(xreal)0.5;            /* c/b = -1/2 */
+    dp[1] = r[1] * (xreal)0.5;      /* r/b */
     for (int32_t j = 2; j <= m; ++j) {
-        long double denom = 2.0L + cp[j - 1]; /* b - a*cp[j-1] with a = -1 */
-        long double num = r[j] + dp[j - 1];   /* r - a*dp[j-1] */
-        cp[j] = -1.0L / denom;
+        xreal denom = (xreal)2.0 + cp[j - 1]; /* b - a*cp[j-1] with a = -1 */
+        xreal num = r[j] + dp[j - 1];   /* r - a*dp[j-1] */
+        cp[j] = -(xreal)1.0 / denom;
         dp[j] = num / denom;
     }
     u[m] = dp[m];
     for (int32_t j = m - 1; j >= 1; --j) {
-        long double t = cp[j] * u[j + 1];
+        xreal t = cp[j] * u[j + 1];
         u[j] = dp[j] - t;
     }
+}
+
+/* Sum of n binary64 values in extended precision with Neumaier's compensation (the running error of every addition
+ * is recovered exactly and added at the end): the result is the exact sum rounded once, for all practical n.
+ * Needed for the mean that neutralises a periodic grid (S25): an error d in that mean leaves a uniform charge d
+ * behind, i.e. a spurious parabola of height d dx^2 nc^2 / 8 in phi -- 1e11 d at the 10^6 nodes of config 4.  A
+ * plain x87 long double loop is not enough: 65,536 equal terms already lose 12 bits (measured: phi = 1.7e-8 instead of
+ * 0 for uniform rho = 0.37, dx = 0.5; pinned by test_uniform_rho_on_a_ring_gives_zero). */
+static xreal sum_compensated(const double *v, int32_t n)
+{
+    xreal s = (xreal)0.0, c = (xreal)0.0;
+    for (int32_t j = 0; j < n; ++j) {
+        const xreal x = (xreal)v[j];
+        const xreal t = s + x;
+        if (XABS(s) >= XABS(x))
+            c += (s - t) + x;
+        else
+            c += (x - t) + s;
+        s = t;
+    }
+    return s + c;
+}
+
+static xreal sum_compensated_ld(const xreal *v, int32_t n)
+{
+    xreal s = (xreal)0.0, c = (xreal)0.0;
+    for (int32_t j = 0; j < n; ++j) {
+        const xreal x = v[j];
+        const xreal t = s + x;
+        if (XABS(s) >= XABS(x))
+            c += (s - t) + x;
+        else
+            c += (x - t) + s;
+        s = t;
+    }
+    return s + c;
 }
 
 /* S23-S25: phi on the nc+1 nodes from rho on the nc+1 nodes. */
@@ -116,29 +164,24 @@ int oracle_poisson(int32_t nc, double dx, int32_t boundary, const double *rho, d
 {
     if (nc < 2 || !(dx > 0.0)) return -1;
     const size_t n1 = (size_t)nc + 2;
-    long double *r = (long double *)malloc(n1 * sizeof(long double));
-    long double *u = (long double *)malloc(n1 * sizeof(long double));
-    long double *cp = (long double *)malloc(n1 * sizeof(long double));
-    long double *dp = (long double *)malloc(n1 * sizeof(long double));
+    xreal *r = (xreal *)malloc(n1 * sizeof(xreal));
+    xreal *u = (xreal *)malloc(n1 * sizeof(xreal));
+    xreal *cp = (xreal *)malloc(n1 * sizeof(xreal));
+    xreal *dp = (xreal *)malloc(n1 * sizeof(xreal));
     if (!r || !u || !cp || !dp) { free(r); free(u); free(cp); free(dp); return -2; }
-    const long double dx2 = (long double)dx * (long double)dx;
-    long double mean = 0.0L;
-    if (boundary == ORACLE_PERIODIC) {
-        long double sum = 0.0L;
-        for (int32_t j = 0; j < nc; ++j) sum = sum + (long double)rho[j];
-        mean = sum / (long double)nc;
-    }
+    const xreal dx2 = (xreal)dx * (xreal)dx;
+    xreal mean = (xreal)0.0;
+    if (boundary == ORACLE_PERIODIC)
+        mean = sum_compensated(rho, nc) / (xreal)nc;
     for (int32_t j = 1; j <= nc - 1; ++j) {
-        long double rj = (long double)rho[j] - mean; /* mean = 0 on a bounded grid */
+        xreal rj = (xreal)rho[j] - mean; /* mean = 0 on a bounded grid */
         r[j] = dx2 * rj;
     }
     /* bounded: phi[0] = phi[nc] = 0.  periodic: the gauge phi[0] = 0 first (the equation at node 0 then holds
      * by itself because the neutralised rho sums to zero), the mean is removed below. */
     thomas_121(nc - 1, r, u, cp, dp);
     if (boundary == ORACLE_PERIODIC) {
-        long double sum = 0.0L;
-        for (int32_t j = 0; j < nc; ++j) sum = sum + u[j];
-        long double pm = sum / (long double)nc;
+        xreal pm = sum_compensated_ld(u, nc) / (xreal)nc;
         for (int32_t j = 0; j < nc; ++j) phi[j] = (double)(u[j] - pm);
         phi[nc] = phi[0];
     } else {

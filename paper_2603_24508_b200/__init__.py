@@ -21,7 +21,8 @@ EXPORTS = [
     "pic_create", "pic_species_at", "pic_push", "pic_arrange", "pic_wall_flux", "pic_set_field", "pic_n_slots",
     "pic_active_buffer", "pic_cell_counts", "pic_step_count", "pic_arrange_info", "pic_workspace_bytes",
     "pic_set_option", "pic_launch_count", "pic_sync", "pic_destroy", "pic_strerror", "pic_last_error",
-    "pic_run_host", "pic_kernel_time", "pic_fused_info", "pic_deposit",
+    "pic_run_host", "pic_kernel_time", "pic_fused_info", "pic_deposit", "pic_n_live", "pic_set_field_device",
+    "pic_solve_field", "pic_get_field",
 ]
 
 
@@ -79,6 +80,10 @@ def lib():
         L.pic_wall_flux.argtypes = [vp, C.POINTER(pic_wall_flux_t)]
         L.pic_set_field.argtypes = [vp, C.POINTER(C.c_double)]
         L.pic_n_slots.argtypes = [vp, i64p]
+        L.pic_n_live.argtypes = [vp, i64p]
+        L.pic_set_field_device.argtypes = [vp, vp]
+        L.pic_solve_field.argtypes = [vp, vp, C.c_int, vp]
+        L.pic_get_field.argtypes = [vp, C.POINTER(C.c_double)]
         L.pic_active_buffer.argtypes = [vp, C.POINTER(C.c_int)]
         L.pic_cell_counts.argtypes = [vp, i32p, i32p]
         L.pic_step_count.argtypes = [vp, i64p]
@@ -233,6 +238,44 @@ def pic_set_field(sim, E_nodes):
     _check(lib().pic_set_field(sim.handle, _dptr(E)), "pic_set_field")
 
 
+def pic_set_field_device(sim, E_dev):
+    """pic_set_field_device: E (torch float64 device tensor, nc+1) copied on the sim's stream; no host round trip."""
+    import torch
+    assert E_dev.dtype == torch.float64 and E_dev.numel() == sim.nc + 1 and E_dev.is_contiguous() and E_dev.is_cuda
+    sim.stream.wait_stream(torch.cuda.current_stream())  # E_dev was produced on torch's current stream
+    _check(lib().pic_set_field_device(sim.handle, C.c_void_p(E_dev.data_ptr())), "pic_set_field_device")
+    torch.cuda.current_stream().wait_stream(sim.stream)  # the caller may overwrite E_dev afterwards
+
+
+def pic_solve_field(sim, rho, smooth_passes=0, phi=None, want_phi=False):
+    """pic_solve_field: smooth -> Poisson -> E on the device; E replaces the sim's field.  rho: torch float64 device
+    tensor (nc+1), as pic_deposit returns it.  Returns phi (device tensor) if want_phi or phi is given, else None."""
+    import torch
+    assert rho.dtype == torch.float64 and rho.numel() == sim.nc + 1 and rho.is_contiguous() and rho.is_cuda
+    if phi is None and want_phi:
+        phi = torch.empty(sim.nc + 1, dtype=torch.float64, device=rho.device)
+    if phi is not None:
+        assert phi.dtype == torch.float64 and phi.numel() == sim.nc + 1 and phi.is_contiguous()
+    sim.stream.wait_stream(torch.cuda.current_stream())
+    _check(lib().pic_solve_field(sim.handle, C.c_void_p(rho.data_ptr()), int(smooth_passes),
+                                 C.c_void_p(phi.data_ptr()) if phi is not None else None), "pic_solve_field")
+    torch.cuda.current_stream().wait_stream(sim.stream)
+    return phi
+
+
+def pic_get_field(sim):
+    """pic_get_field -> numpy array of the nc+1 node values of E in force."""
+    E = np.empty(sim.nc + 1, dtype=np.float64)
+    _check(lib().pic_get_field(sim.handle, _dptr(E)), "pic_get_field")
+    return E
+
+
+def pic_n_live(sp):
+    n = C.c_int64()
+    _check(lib().pic_n_live(sp.handle, C.byref(n)), "pic_n_live")
+    return n.value
+
+
 def pic_n_slots(sp):
     n = C.c_int64()
     _check(lib().pic_n_slots(sp.handle, C.byref(n)), "pic_n_slots")
@@ -325,6 +368,19 @@ def pic_run_host(*, nc, dx, dt, boundary, E_nodes, B, species, nsteps, stream=No
     hs = (pic_host_species * len(species))()
     for h, s in zip(hs, species):
         a = s["arrays"]
+        if len(a) != 5:
+            raise ValueError("arrays must be [x, vx, vy, vz, cell]")
+        for k, t in enumerate(a):  # the C side reads and overwrites n elements of each: check before handing pointers over
+            want = "int32" if k == 4 else "float64"
+            if hasattr(t, "data_ptr"):
+                ok = str(t.dtype).endswith(want) and t.is_contiguous() and not t.is_cuda and t.dim() == 1
+            else:
+                ok = isinstance(t, np.ndarray) and t.dtype == np.dtype(want) and t.flags.c_contiguous and t.ndim == 1 \
+                    and t.flags.writeable
+            if not ok:
+                raise ValueError(f"arrays[{k}] must be a contiguous, writable, 1-D host {want} array")
+            if len(t) != len(a[0]):
+                raise ValueError("the five arrays of a species must have equal lengths")
         ptrs = [t.data_ptr() if hasattr(t, "data_ptr") else t.ctypes.data for t in a]
         h.qm, h.n = float(s["qm"]), len(a[0])
         h.x, h.vx, h.vy, h.vz, h.cell = ptrs

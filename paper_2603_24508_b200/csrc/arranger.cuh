@@ -77,6 +77,7 @@ struct ScatterArgs {
     DevState *st;
     const int *only_if; // if not NULL: the kernel returns at once unless *only_if != 0
     int nc, periodic, w_limit;
+    int general_follows; // the host has enqueued the general path behind this kernel (else declining is an error)
 };
 
 constexpr int SCATTER_THREADS = 256;
@@ -106,7 +107,11 @@ __global__ void __launch_bounds__(SCATTER_THREADS) scatter_fast_kernel(ScatterAr
     if (a.only_if && !*a.only_if) return;
     const int W = a.st->w_acc;
     if (W > a.w_limit) {
-        if (blockIdx.x == 0 && threadIdx.x == 0) a.st->need_general = 1;
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            a.st->need_general = 1;
+            // the host's displacement bound said this could not happen and nothing runs behind: never silent
+            if (!a.general_follows) atomicOr(&a.st->status, ERR_ARRANGE_SKIPPED);
+        }
         return;
     }
     const int lane = threadIdx.x & 31;

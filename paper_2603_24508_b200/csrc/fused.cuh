@@ -37,7 +37,6 @@ constexpr int FUSED_MIN_NC = 16;
 constexpr int FUSED_CPC_DEFAULT = 32;  // cells per chunk (per CTA) on grids of many waves (measured optimum at config 4)
 constexpr int FUSED_CPC_SEARCH = 64;   // largest chunk the per-launch search considers on smaller grids
 constexpr int FUSED_CPC_MAX = 256;
-constexpr int FUSED_STAGES_DEFAULT = 1;    // stages of the shared-memory ring (1: more CTAs per SM; measured faster than 2)
 constexpr int FUSED_KMAX = 31;         // cells per tile (one lane per cell border)
 constexpr int FUSED_DEF = 32;          // deferred right-movers of a tile's last cell
 constexpr int FUSED_XCAP = 256;        // edge kernel: leavers per edge cell
@@ -82,7 +81,7 @@ __host__ __device__ inline FusedLayout fused_layout(int CAP, int CPC, int NST)
     o = (o + 15) & ~15;
     L.off_cell = o; o += 8 * (FUSED_KMAX + 1); // {first slot, count} of the tile's cells
     L.off_row = o;  o += 16 * 16;              // per row: the three class ballots and the running counts before it
-    L.off_base = o; o += 8 * 3 * 32;           // per (class, cell): {slot base, destination cell}
+    L.off_base = o; o += 8 * 4 * 32;           // per (class, cell): {slot base, destination cell}; class 3 = nothing to store
     L.off_q = o;    o += FUSED_DEF * 40;
     L.off_mbar = o; o += 32;
     L.total = o;
@@ -142,6 +141,9 @@ __global__ void __launch_bounds__(128) fused_edge_kernel(FusedArgs a)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const unsigned lt = (1u << lane) - 1u;
     const int nc = a.k.nc;
+    // programmatic dependent launch: the streaming kernel behind may start now; it waits (griddepcontrol.wait) for
+    // this grid to complete before it reads anything written here or writes anything at all
+    asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
     if (threadIdx.x == 0) s_bad = 0;
     __syncthreads();
     if (st->fused_disabled) {
@@ -172,10 +174,14 @@ __global__ void __launch_bounds__(128) fused_edge_kernel(FusedArgs a)
         const unsigned mR = __ballot_sync(FULL, g == 2), mX = __ballot_sync(FULL, g == 3);
         if (g == 3) {
             const int r = nX + __popc(mX & lt);
-            if (r < FUSED_XCAP && (warp == 0 || warp == 3)) {
-                qx[ql][r] = o.x; qvx[ql][r] = o.vx; qvy[ql][r] = o.vy; qvz[ql][r] = o.vz;
+            if (warp == 0 || warp == 3) {
+                if (r < FUSED_XCAP) {
+                    qx[ql][r] = o.x; qvx[ql][r] = o.vx; qvy[ql][r] = o.vy; qvz[ql][r] = o.vz;
+                } else {
+                    bad |= 2; // more leavers than the list holds
+                }
             } else {
-                bad = 2;
+                bad |= 1; // class X out of cell 1 or nc-2: the particle moved two cells
             }
         }
         nL += __popc(mL); nS += __popc(mS); nR += __popc(mR); nX += __popc(mX);
@@ -306,26 +312,29 @@ __device__ __forceinline__ void fused_issue(const FusedArgs &a, const FusedCtx &
 // outside the tile (the alignment pad, the tail of the last row, rows behind it inside the group)
 // push whatever the stage holds there (every row lies inside the stage; no address depends on it)
 // and are masked out.
-// EDGE = the tile holds cell 0 or cell nc-1: only there can a particle wrap / be absorbed (class X), can
-// floor(x/dx) need the clamp of reading S8, or can x leave the gather range legitimately.  Elsewhere any
-// of that marks the particle bad (it moved more than one cell, or the grouping is broken).
+// TMA: the tile's x, vx, vy, vz were staged in shared memory by bulk copies (p0..p3 point into the stage, E nodes
+// in the shared window pE); otherwise they are read straight from global memory (p0..p3 = the arrays at the tile's
+// first slot, read-only path; slot index clamped to imax so that no load leaves the arrays; pE = the E array).
+// EDGE = the tile holds cell 0, nc-2 or nc-1: only there can a particle wrap / be absorbed (class X), can
+// floor(x/dx) need the clamp of reading S8, or can x leave the gather range legitimately.  Elsewhere a new cell
+// more than one away from the source cell marks the particle bad (it moved more than one cell, left the grid,
+// or the grouping is broken) and no clamp is needed: the source cells are 1 .. nc-3.
 // cellinfo[cl] = {first slot, count} of the tile's cells from off_old: a slot outside its cell's range
-// means the grouping is broken.  W_[r] = class | local cell << 2 | bad << 8.
-template <bool PERIODIC, bool EDGE, bool BZ0, int RMAX, int R0, int CNT>
-__device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *px, const double *sEs, const int2 *cellinfo, int lane,
+// means the grouping is broken.  W_[r] = class << 5 | local cell | bad << 8 (class 3: nothing to store).
+template <bool PERIODIC, bool EDGE, bool BZ0, bool TMA, int RMAX, int R0, int CNT>
+__device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *pE, const int2 *cellinfo, int lane,
                                               int pad, int n, int cA, int ncell, double (&X_)[RMAX], double (&VX_)[RMAX],
                                               double (&VY_)[RMAX], double (&VZ_)[RMAX], int (&W_)[RMAX])
 {
-    constexpr int CAP = RMAX * 32;
     const int nc = k.nc;
 #pragma unroll
     for (int r = R0; r < R0 + CNT; ++r) {
         const int i = (r << 5) + lane;
         const bool valid = (unsigned)(i - pad) < (unsigned)n;
-        const double x = px[i], vx = px[CAP + i], vy = px[2 * CAP + i], vz = px[3 * CAP + i];
+        const double x = X_[r], vx = VX_[r], vy = VY_[r], vz = VZ_[r]; // loaded by fused_load_rows
         const double xs = __dmul_rn(x, k.inv_dx);
-        double jf = floor(xs);
         int jc = __double2int_rd(xs);
+        double jf = (double)jc; // = floor(xs) whenever the particle is inside the grid (anything else is declined)
         bool inr = true;
         if (EDGE) {
             inr = xs >= 0.0 && jc <= nc;
@@ -334,9 +343,12 @@ __device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *
         const int cl = jc - cA;
         inr = inr && (unsigned)cl < (unsigned)ncell;
         const int j = inr ? jc : cA;
+        if (!inr) jf = (double)cA;
         const int2 sc = cellinfo[j - cA];
         const bool inside = (unsigned)(i - sc.x) < (unsigned)sc.y;
-        const double E0 = sEs[j], E1 = sEs[j + 1];
+        double E0, E1;
+        if (TMA) { E0 = pE[j]; E1 = pE[j + 1]; }
+        else { E0 = __ldg(pE + j); E1 = __ldg(pE + j + 1); }
         const double w = __dsub_rn(xs, jf);
         const double dE = __dsub_rn(E1, E0);
         const double Ep = __dadd_rn(E0, __dmul_rn(w, dE));
@@ -363,47 +375,75 @@ __device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *
         const double nvx = __dadd_rn(wx, hE);
         const double xn = __dadd_rn(x, __dmul_rn(nvx, k.dt));
         double xw = xn;
-        bool out = false, legit = false;
-        int wall = 0;
+        int g;
+        bool good;
         if (EDGE) {
+            bool legit = false;
+            int wall = 0;
             if (PERIODIC) {
                 const double xm = __dsub_rn(xn, k.L), xp = __dadd_rn(xn, k.L);
                 xw = xn >= k.L ? xm : (xn < 0.0 ? (xp >= k.L ? 0.0 : xp) : xn);
             } else {
                 wall = xn < 0.0 ? 1 : (xn >= k.L ? 2 : 0);
             }
-        } else {
-            out = xn < 0.0 || xn >= k.L;
-        }
-        const int cn = min(__double2int_rd(__dmul_rn(xw, k.inv_dx)), nc - 1);
-        const int d = cn - j;
-        int g = (unsigned)(d + 1) <= 2u ? d + 1 : 3;
-        if (EDGE) { // class X: out of cell 0 downwards / out of cell nc-1 upwards only
+            const int cn = min(__double2int_rd(__dmul_rn(xw, k.inv_dx)), nc - 1);
+            const int d = cn - j;
+            g = (unsigned)(d + 1) <= 2u ? d + 1 : 3;
+            // class X: out of cell 0 downwards / out of cell nc-1 upwards only
             if (PERIODIC) {
                 legit = (j == nc - 1 && cn == 0) || (j == 0 && cn == nc - 1);
             } else {
                 if (wall) g = 3;
                 legit = (wall == 1 && j == 0) || (wall == 2 && j == nc - 1);
             }
-        } else if (out) {
-            g = 3;
+            good = valid && inr && inside && (g < 3 || legit);
+        } else {
+            const int d = __double2int_rd(__dmul_rn(xn, k.inv_dx)) - j;
+            g = (unsigned)(d + 1) <= 2u ? d + 1 : 3;
+            good = valid && inr && inside && g < 3;
         }
-        const bool good = valid && inr && inside && (g < 3 || legit);
         if (!good) g = 3;
-        W_[r] = g | ((j - cA) << 2) | ((valid && !good) ? 256 : 0);
+        W_[r] = (g << 5) | (j - cA) | ((valid && !good) ? 256 : 0);
         X_[r] = xw; VX_[r] = nvx; VY_[r] = wy; VZ_[r] = wz;
     }
 }
 
 // Row groups of sweep 1a: four rows at a time while at least four remain likely, then two, then single rows,
 // so that a tile of nrows rows pushes at most one surplus row.
-template <bool PERIODIC, bool EDGE, bool BZ0, int RMAX>
-__device__ __forceinline__ void fused_sweep1a_all(const PushConst &k, const double *px, const double *sEs, const int2 *cellinfo, int lane,
+// The tile's x, vx, vy, vz from the stage (or, without TMA, from global memory) into the register tile, by the same
+// row groups as the sweeps.  Done for the whole tile BEFORE the arithmetic, so that the stage is free again at once
+// and the next tile's bulk copies are in flight during all of this tile's work.
+template <bool TMA, int RMAX>
+__device__ __forceinline__ void fused_load_rows(const double *p0, const double *p1, const double *p2, const double *p3, int imax,
+                                                int lane, int nrows, double (&X_)[RMAX], double (&VX_)[RMAX],
+                                                double (&VY_)[RMAX], double (&VZ_)[RMAX])
+{
+#pragma unroll
+    for (int gi = 0; gi < RMAX / 4 + 2; ++gi) {
+        const int g0 = gi < RMAX / 4 - 1 ? 4 * gi : 4 * (RMAX / 4 - 1) + (gi == RMAX / 4 - 1 ? 0 : (gi == RMAX / 4 ? 2 : 3));
+        const int gn = gi < RMAX / 4 - 1 ? 4 : (gi == RMAX / 4 - 1 ? 2 : 1);
+        if (g0 < nrows) {
+#pragma unroll
+            for (int r = g0; r < g0 + gn; ++r) {
+                const int i = (r << 5) + lane;
+                if (TMA) {
+                    X_[r] = p0[i]; VX_[r] = p1[i]; VY_[r] = p2[i]; VZ_[r] = p3[i];
+                } else {
+                    const int il = min(i, imax);
+                    X_[r] = __ldg(p0 + il); VX_[r] = __ldg(p1 + il); VY_[r] = __ldg(p2 + il); VZ_[r] = __ldg(p3 + il);
+                }
+            }
+        }
+    }
+}
+
+template <bool PERIODIC, bool EDGE, bool BZ0, bool TMA, int RMAX>
+__device__ __forceinline__ void fused_sweep1a_all(const PushConst &k, const double *pE, const int2 *cellinfo, int lane,
                                                   int pad, int n, int nrows, int cA, int ncell, double (&X_)[RMAX], double (&VX_)[RMAX],
                                                   double (&VY_)[RMAX], double (&VZ_)[RMAX], int (&W_)[RMAX])
 {
 #define FUSED_ROWS(R0, CNT) \
-    if (R0 < nrows) fused_sweep1a<PERIODIC, EDGE, BZ0, RMAX, R0, CNT>(k, px, sEs, cellinfo, lane, pad, n, cA, ncell, X_, VX_, VY_, VZ_, W_);
+    if (R0 < nrows) fused_sweep1a<PERIODIC, EDGE, BZ0, TMA, RMAX, R0, CNT>(k, pE, cellinfo, lane, pad, n, cA, ncell, X_, VX_, VY_, VZ_, W_);
     FUSED_ROWS(0, 4)
     if (RMAX == 8) {
         FUSED_ROWS(4, 2) FUSED_ROWS(6, 1) FUSED_ROWS(7, 1)
@@ -425,7 +465,10 @@ __host__ __device__ constexpr int fused_group_start(int rmax, int gi)
 }
 __host__ __device__ constexpr int fused_group_count(int rmax, int gi) { return gi < rmax / 4 - 1 ? 4 : (gi == rmax / 4 - 1 ? 2 : 1); }
 
-template <int RMAX, bool PERIODIC, bool BZ0>
+// TMA = true: particles and the chunk's E window are staged in shared memory by bulk copies (cp.async.bulk + mbarrier).
+// TMA = false (option "fused_tma" = 0, the A/B variant of profiles/): plain read-only global loads into the same
+// registers, E through the read-only path; no stage, no mbarrier.
+template <int RMAX, bool PERIODIC, bool BZ0, bool TMA>
 __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fused_kernel(FusedArgs a)
 {
     static_assert(RMAX == 8 || RMAX == 12 || RMAX == 16, "row groups of sweep 1a are written for these sizes");
@@ -448,7 +491,7 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
     int bad = 0;  // FA_* bits
     int mc = 0;   // largest new per-cell count seen by this lane
 
-    if (!*(volatile int *)&st->abort) {
+    {
         FusedCtx X;
         X.C0 = blockIdx.x * a.CPC;
         X.C1 = min(X.C0 + a.CPC, nc);
@@ -458,11 +501,14 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
         X.STR = CAP;
         X.offs = offs;
         const int Cm = X.Cm, Cp = min(X.C1 + 1, nc);
+        // Prologue: reads only what was complete before the edge kernel of this step started (off_old, E, the source
+        // particles), writes nothing outside shared memory -- under programmatic dependent launch it overlaps that
+        // kernel.
         for (int idx = lane; idx <= Cp - Cm; idx += 32) offs[idx] = a.off_old[Cm + idx];
         const int ea = Cm & ~1;
         const double *sEs = sE - ea; // E node j of the chunk's window sits at sEs[j]
         const unsigned cap32 = (unsigned)a.capacity;
-        if (lane == 0) {
+        if (TMA && lane == 0) {
             asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(mb0) : "memory");
             asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(mb1) : "memory");
             asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(mbE) : "memory");
@@ -473,16 +519,29 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
             bulk_g2s(sE, a.E + ea, eb, mbE);
         }
         __syncwarp();
-        const int OL = st->f_OL, AR = st->f_AR, shift = AR - OL;
         int phase = 0, cur = 0;
         FusedItem I0 = fused_next_item(X, phase, cur, lane, bad);
         FusedItem I1 = fused_next_item(X, phase, cur, lane, bad);
         const bool two = a.NST == 2;
         double *stage0 = reinterpret_cast<double *>(fused_smem), *stage1 = reinterpret_cast<double *>(fused_smem + L.stage_bytes);
-        if (lane == 0) {
+        if (TMA && lane == 0) {
             fused_issue(a, X, I0, stage0, mb0);
             if (two) fused_issue(a, X, I1, stage1, mb1);
         }
+        // From here on the edge kernel's results are needed (abort flag, OL, AR) and global memory is written: wait for
+        // it (a no-op without programmatic dependent launch: stream order has done it).
+        asm volatile("griddepcontrol.wait;\n" ::: "memory");
+        if (TMA) mbar_wait(mbE, 0);
+        if (*(volatile int *)&st->abort) {
+            // a fused step declined earlier: this launch must not touch anything.  Let the bulk copies already under
+            // way land before the CTA gives its shared memory back.
+            if (TMA) {
+                if (I0.kind <= FK_HALO && offs[I0.cB - Cm] > offs[I0.cA - Cm]) mbar_wait(mb0, 0);
+                if (two && I1.kind <= FK_HALO && offs[I1.cB - Cm] > offs[I1.cA - Cm]) mbar_wait(mb1, 0);
+            }
+            I0.kind = FK_NONE;
+        }
+        const int OL = st->f_OL, AR = st->f_AR, shift = AR - OL;
         // carry across tiles: class counts of the previous tile's last cell
         int pvL = 0, pvS = 0, pvR = 0;
         int pvRR = 0;    // R of the cell before the carried one
@@ -490,7 +549,6 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
         int pv_real = 0; // the carried cell belongs to this chunk (finalize it)
         int ndef = 0;    // deferred right-movers of the carried cell
         unsigned ph0 = 0, ph1 = 0;
-        mbar_wait(mbE, 0);
 
         for (int it = 0; I0.kind != FK_NONE; ++it) {
             const FusedItem I2 = fused_next_item(X, phase, cur, lane, bad);
@@ -508,39 +566,54 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
             __syncwarp();
             const bool odd = two && (it & 1);
             double *px = odd ? stage1 : stage0;
-            if (n > 0) {
+            if (TMA && n > 0) {
                 if (odd) { mbar_wait(mb1, ph1); ph1 ^= 1u; }
                 else     { mbar_wait(mb0, ph0); ph0 ^= 1u; }
             }
 
             // ---- sweep 1a: push into registers and classify (fused_sweep1a) ----------------------------------
             double X_[RMAX], VX_[RMAX], VY_[RMAX], VZ_[RMAX];
-            int W_[RMAX]; // 1a: class | cell << 2 | bad << 8;  1b: -1, or class prefix count << 8 | class*32 + cell
-            if (cA == 0 || cB == nc) fused_sweep1a_all<PERIODIC, true, BZ0, RMAX>(a.k, px, sEs, cellinfo, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_);
-            else fused_sweep1a_all<PERIODIC, false, BZ0, RMAX>(a.k, px, sEs, cellinfo, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_);
+            int W_[RMAX]; // 1a: class << 5 | cell | bad << 8;  1b: class prefix count << 8 | class*32 + cell
+            {
+                const double *p0 = TMA ? px : a.sx + gbase, *p1 = TMA ? px + CAP : a.svx + gbase;
+                const double *p2 = TMA ? px + 2 * CAP : a.svy + gbase, *p3 = TMA ? px + 3 * CAP : a.svz + gbase;
+                const int imax = TMA ? CAP - 1 : (int)min((long long)(CAP - 1), a.capacity - 1 - gbase);
+                fused_load_rows<TMA, RMAX>(p0, p1, p2, p3, imax, lane, nrows, X_, VX_, VY_, VZ_);
+            }
             __syncwarp();
-            // the stage has been read: refill it with the next item to load
-            if (lane == 0) fused_issue(a, X, two ? I2 : I1, px, odd ? mb1 : mb0);
+            // the stage has been read into registers: refill it with the next item to load
+            if (TMA && lane == 0) fused_issue(a, X, two ? I2 : I1, px, odd ? mb1 : mb0);
+            {
+                const double *pE = TMA ? sEs : a.E;
+                if (cA == 0 || cB >= nc - 1)
+                    fused_sweep1a_all<PERIODIC, true, BZ0, TMA, RMAX>(a.k, pE, cellinfo, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_);
+                else
+                    fused_sweep1a_all<PERIODIC, false, BZ0, TMA, RMAX>(a.k, pE, cellinfo, lane, pad, n, nrows, cA, ncell, X_, VX_, VY_, VZ_, W_);
+            }
+            __syncwarp();
 
             // ---- sweep 1b: prefix counts per class (ballot/popc); the row's ballots are kept for the cell borders ---
-            unsigned run = 0; // running class counts of the tile: L | S << 10 | R << 20
+            int runL = 0, runS = 0, runR = 0; // running class counts of the tile (warp-uniform)
+            int wor = 0;
 #pragma unroll
             for (int gi = 0; gi < fused_ngroups(RMAX); ++gi) {
                 if (fused_group_start(RMAX, gi) < nrows) {
 #pragma unroll
                     for (int r = fused_group_start(RMAX, gi); r < fused_group_start(RMAX, gi) + fused_group_count(RMAX, gi); ++r) {
                         const int w = W_[r];
-                        const int g = w & 3;
-                        if (w & 256) bad |= FA_BAD_PARTICLE;
-                        const unsigned mL = __ballot_sync(FULL, g == 0), mS = __ballot_sync(FULL, g == 1), mR = __ballot_sync(FULL, g == 2);
-                        if (lane == 0) rowinfo[r] = make_int4((int)mL, (int)mS, (int)mR, (int)run);
-                        const unsigned mo = g == 0 ? mL : (g == 1 ? mS : mR);
-                        const int mine = (int)((run >> (10 * g)) & 1023u) + __popc(mo & lt);
-                        W_[r] = g < 3 ? (mine << 8) | (g * 32 + ((w >> 2) & 31)) : -1;
-                        run += (unsigned)__popc(mL) | ((unsigned)__popc(mS) << 10) | ((unsigned)__popc(mR) << 20);
+                        wor |= w;
+                        const bool isL = (w & 96) == 0, isS = (w & 96) == 32;
+                        const unsigned mL = __ballot_sync(FULL, isL), mS = __ballot_sync(FULL, isS), mR = __ballot_sync(FULL, (w & 96) == 64);
+                        if (lane == 0) rowinfo[r] = make_int4((int)mL, (int)mS, (int)mR, runL | (runS << 10) | (runR << 20));
+                        const unsigned mo = isL ? mL : (isS ? mS : mR);
+                        const int rn = isL ? runL : (isS ? runS : runR);
+                        W_[r] = ((rn + __popc(mo & lt)) << 8) | (w & 127); // class 3 keeps a key >= 96: nothing is stored for it
+                        runL += __popc(mL); runS += __popc(mS); runR += __popc(mR);
                     }
                 }
             }
+            if (wor & 256) bad |= FA_BAD_PARTICLE;
+            const unsigned run = (unsigned)(runL | (runS << 10) | (runR << 20));
             __syncwarp();
 
             // ---- per-cell phase (lane q = local cell q; lane ncell = the end of the tile) ---------------------
@@ -612,37 +685,35 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
             if (tile_oob) bad |= FA_BAD_PARTICLE;
             if (kind == FK_REAL && !tile_oob) {
                 const int kdef = 64 + ncell - 1;                                 // class R of the tile's last cell
-                const int rdef = __shfl_sync(FULL, st_q, max(ncell - 1, 0)) >> 5; // first row that can hold it
+                const int lastq = max(ncell - 1, 0);
+                const int rdef = __shfl_sync(FULL, st_q, lastq) >> 5;            // first row that can hold it
+                const int psRlast = __shfl_sync(FULL, psR, lastq);               // R particles of the tile before that cell
+                const int nRlast = __shfl_sync(FULL, Rc, lastq);                 // its right-movers: deferred to the next tile
+                if (nRlast > FUSED_DEF) bad |= FA_DEFER_OVERFLOW;
 #pragma unroll
                 for (int gi = 0; gi < fused_ngroups(RMAX); ++gi) {
                     if (fused_group_start(RMAX, gi) < nrows) {
 #pragma unroll
                         for (int r = fused_group_start(RMAX, gi); r < fused_group_start(RMAX, gi) + fused_group_count(RMAX, gi); ++r) {
                             const int pk = W_[r];
-                            const bool has = pk >= 0;
-                            const int2 bd = basd[pk & 127];
+                            const int key = pk & 127;
+                            const int2 bd = basd[key];
                             const int p = bd.x + (pk >> 8);
-                            const bool defer = has && (pk & 127) == kdef;
-                            if (has && !defer) {
+                            if (key < 96 && key != kdef) {
                                 a.dx[p] = X_[r]; a.dvx[p] = VX_[r]; a.dvy[p] = VY_[r]; a.dvz[p] = VZ_[r];
                                 a.dcell[p] = bd.y;
                             }
-                            if (r >= rdef) {
-                                const unsigned md = __ballot_sync(FULL, defer);
-                                if (md) {
-                                    if (defer) {
-                                        const int q = ndef + __popc(md & lt);
-                                        if (q < FUSED_DEF) {
-                                            qx[q] = X_[r]; qvx[q] = VX_[r]; qvy[q] = VY_[r]; qvz[q] = VZ_[r];
-                                            qpos[q] = p;
-                                        } else bad |= FA_DEFER_OVERFLOW;
-                                    }
-                                    ndef = min(ndef + __popc(md), FUSED_DEF);
+                            if (r >= rdef && key == kdef) { // its rank inside the class is its place in the queue
+                                const int q = (pk >> 8) - psRlast;
+                                if (q < FUSED_DEF) {
+                                    qx[q] = X_[r]; qvx[q] = VX_[r]; qvy[q] = VY_[r]; qvz[q] = VZ_[r];
+                                    qpos[q] = p;
                                 }
                             }
                         }
                     }
                 }
+                ndef = min(nRlast, FUSED_DEF);
             }
             // carry: this tile's last cell
             if (kind != FK_VIRTUAL) {
@@ -681,6 +752,7 @@ __global__ void fused_commit_kernel(DevState *st, int step_id)
         st->n = st->n_next;
         st->wall[0] += st->wall_pend[0];
         st->wall[1] += st->wall_pend[1];
+        st->wall_arr = st->wall[0] + st->wall[1];
         st->vmax2 = 0x7f800000u; // speed bound unknown after a fused step (+inf): the split path, should it
                                  // take over, enqueues its general arranger until its mover has measured one
         st->maxcount = st->maxcount_next;

@@ -71,7 +71,9 @@ __global__ void __launch_bounds__(MOVER_THREADS) mover_kernel(MoverArgs a)
                 nleft += (o.wall == 1); nright += (o.wall == 2);
             } else {
                 bad = 1;
-                cn[q] = READ_CELL ? c[q] : 0;
+                // left untouched as the oracle does; without a stored cell index to keep, flag it dead so that the
+                // arrange behind this step stays self-consistent (it is dropped) while ERR_OUT_OF_DOMAIN is reported
+                cn[q] = READ_CELL ? c[q] : -1;
                 live = false;
             }
         }

@@ -2,6 +2,7 @@
 // constants, kernel launches on the caller's stream).  No torch types; no CPU compute path.
 #include "../../include/pic.h"
 
+#include <chrono>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -16,6 +17,7 @@
 #include "general.cuh"
 #include "tilesort.cuh"
 #include "deposit.cuh"
+#include "field.cuh"
 #include "fused.cuh"
 
 using namespace pic;
@@ -33,8 +35,8 @@ static int cuda_fail(cudaError_t e, const char *what)
         if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
     } while (0)
 
-enum { K_MOVER = 0, K_HIST, K_SCAN, K_SCATTER, K_GENERAL, K_FUSED, K_DEPOSIT, K_COUNT };
-static const char *const K_NAMES[K_COUNT] = {"mover", "hist", "scan", "scatter", "general", "fused", "deposit"};
+enum { K_MOVER = 0, K_HIST, K_SCAN, K_SCATTER, K_GENERAL, K_FUSED, K_DEPOSIT, K_FIELD, K_COUNT };
+static const char *const K_NAMES[K_COUNT] = {"mover", "hist", "scan", "scatter", "general", "fused", "deposit", "field"};
 
 struct pic_species {
     pic_sim *sim = nullptr;
@@ -68,8 +70,10 @@ struct pic_species {
     int unv_cur0 = 0, unv_off0 = 0;
     // host-side conservative bound on cell displacement since the last arrange (decides whether the
     // general-path kernels need to be enqueued at all)
-    double vkick = 0;                  // 2*|h|*max|E|
+    double vkick = 0;                  // 2*|h|*max|E| of the field in force now
     double h_vmax = 0;                 // speed bound at the last sync
+    double h_kick_acc = 0;             // sum of the per-step kicks of the steps enqueued since the last sync (the field
+                                       // may change between steps: each step is bounded with the field it ran under)
     long long h_steps_since_sync = 0;
     long long h_wsum = 0;              // sum of per-step displacement bounds since the last arrange
     bool h_grouped = false;
@@ -89,9 +93,14 @@ struct pic_sim {
     double dx = 0, dt = 0;
     double B[3]{};
     double Emax = 0; // max |E_node|
+    bool emax_known = true; // false after the field was replaced on the device until the next sync reads its max |E|
+    // field solve (field.cuh): library-owned scratch, allocated at the first pic_solve_field / pic_set_field_device
+    double *d_f[2]{}, *d_phi = nullptr, *d_tile = nullptr, *d_scal = nullptr;
+    unsigned long long *d_emax = nullptr;
+    int device = 0;
     std::vector<pic_species *> sp;
     unsigned long long launches = 0;
-    int opt_fused = 1, opt_timing = 0, opt_tile_scatter = 1;
+    int opt_fused = 1, opt_timing = 0, opt_tile_scatter = 1, opt_fused_tma = 1, opt_fused_pdl = 1;
     int opt_fused_cpc = 0, opt_fused_rows = 0, opt_fused_slots = 0, opt_fused_stages = 0; // tuning knobs of the fused step (0 = automatic)
     int sm_count = 148;
     // per-kernel device timing (option "kernel_timing"): event pairs recorded around launches
@@ -171,6 +180,8 @@ extern "C" void pic_destroy(pic_sim *sim)
     for (auto &sp : sim->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
     for (cudaEvent_t e : sim->free_events) cudaEventDestroy(e);
     cudaFree(sim->d_E);
+    cudaFree(sim->d_f[0]); cudaFree(sim->d_f[1]); cudaFree(sim->d_phi); cudaFree(sim->d_tile); cudaFree(sim->d_scal);
+    cudaFree(sim->d_emax);
     delete sim;
 }
 
@@ -205,6 +216,7 @@ static int status_to_rc(int status)
 {
     if (status & ERR_BAD_INITIAL) return PIC_ESTATE;
     if (status & ERR_OUT_OF_DOMAIN) return PIC_ESTATE;
+    if (status & ERR_ARRANGE_SKIPPED) return PIC_ESTATE;
     if (status & ERR_NEED_WORKSPACE) return PIC_ECAPACITY;
     return PIC_OK;
 }
@@ -248,16 +260,46 @@ static bool fused_possible(const pic_species *s)
 // Host-side bound (cells) on what one more mover step can displace any particle.
 static long long host_step_bound(pic_species *s)
 {
-    const double v = s->h_vmax * (1.0 + 1e-6) + (double)(s->h_steps_since_sync + 1) * s->vkick;
+    if (!s->sim->emax_known) return 1LL << 40; // the field was replaced on the device: no bound until the next sync
+    const double v = s->h_vmax * (1.0 + 1e-6) + s->h_kick_acc + s->vkick;
     const double reach = v * s->k.dt * s->k.inv_dx;
     if (!(reach < 1e9)) return 1LL << 40;
     return (long long)std::ceil(reach + 1e-9) + 1;
 }
 
+// The instance of fused_kernel for a launch geometry.
+static void (*fused_pick(int rows, bool periodic, bool bz0, bool tma))(FusedArgs)
+{
+#define PIC_FK(R) (periodic ? (bz0 ? (tma ? fused_kernel<R, true, true, true> : fused_kernel<R, true, true, false>)      \
+                                   : (tma ? fused_kernel<R, true, false, true> : fused_kernel<R, true, false, false>))   \
+                            : (bz0 ? (tma ? fused_kernel<R, false, true, true> : fused_kernel<R, false, true, false>)    \
+                                   : (tma ? fused_kernel<R, false, false, true> : fused_kernel<R, false, false, false>)))
+    return rows == 8 ? PIC_FK(8) : rows == 12 ? PIC_FK(12) : PIC_FK(16);
+#undef PIC_FK
+}
+
+// The fused kernels need more dynamic shared memory than the default limit: raise it once per DEVICE (the attribute
+// is per device and per function; a process may create sims on several devices).
+static int fused_set_attributes(int device)
+{
+    static bool done[64] = {};
+    if (device >= 0 && device < 64 && done[device]) return PIC_OK;
+    std::vector<void (*)(FusedArgs)> kerns;
+    for (int rows : {8, 12, 16})
+        for (int per = 0; per < 2; ++per)
+            for (int bz0 = 0; bz0 < 2; ++bz0)
+                for (int tma = 0; tma < 2; ++tma) kerns.push_back(fused_pick(rows, per != 0, bz0 != 0, tma != 0));
+    for (auto kfn : kerns) CU(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    if (device >= 0 && device < 64) done[device] = true;
+    return PIC_OK;
+}
+
 // ------------------------------------------------------------------------------------------
 // create
 // ------------------------------------------------------------------------------------------
-static int create_species(pic_sim *sim, const pic_species_desc &d, pic_species **out)
+// Host-side half of creating a species: argument checks and every allocation, no wait on the stream (so that it
+// overlaps whatever the caller has in flight on it, e.g. the uploads of pic_run_host).
+static int alloc_species(pic_sim *sim, const pic_species_desc &d, pic_species **out)
 {
     if (!std::isfinite(d.qm) || d.n < 0 || d.capacity < 0 || d.arrange_every < 0) return PIC_EINVAL;
     if (d.n > d.capacity) return PIC_ECAPACITY;
@@ -304,7 +346,13 @@ static int create_species(pic_sim *sim, const pic_species_desc &d, pic_species *
     CU(cudaMalloc(&s->d_scan, s->scan_words * sizeof(unsigned long long)));
     CU(cudaMallocHost(&s->h_tel, sizeof(DevState)));
     CU(cudaEventCreateWithFlags(&s->tel_ev, cudaEventDisableTiming));
+    return PIC_OK;
+}
 
+// Stream-side half: validate the initial state on the device, build its per-cell count / offset.  Syncs.
+static int init_species(pic_sim *sim, pic_species *s, const pic_species_desc &d)
+{
+    const int nc = sim->nc;
     DevState h{};
     h.n = (int)d.n;
     CU(cudaMemcpyAsync(s->d_st, &h, sizeof h, cudaMemcpyHostToDevice, sim->stream));
@@ -348,17 +396,7 @@ static int create_species(pic_sim *sim, const pic_species_desc &d, pic_species *
     s->counts_fresh = grouped;
     s->all_live = true;
     s->reset_w = false;
-    {
-        static bool attr_set = false;
-        if (!attr_set) {
-            void (*kerns[])(FusedArgs) = {fused_kernel<8, true, true>,   fused_kernel<12, true, true>,   fused_kernel<16, true, true>,
-                                          fused_kernel<8, false, true>,  fused_kernel<12, false, true>,  fused_kernel<16, false, true>,
-                                          fused_kernel<8, true, false>,  fused_kernel<12, true, false>,  fused_kernel<16, true, false>,
-                                          fused_kernel<8, false, false>, fused_kernel<12, false, false>, fused_kernel<16, false, false>};
-            for (auto kfn : kerns) CU(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
-            attr_set = true;
-        }
-    }
+    if (int rc = fused_set_attributes(sim->device)) return rc;
     return PIC_OK;
 }
 
@@ -382,6 +420,7 @@ extern "C" int pic_create(const pic_grid_desc *g, const pic_species_desc *specie
     pic_sim *sim = new (std::nothrow) pic_sim;
     if (!sim) return PIC_ENOMEM;
     sim->stream = static_cast<cudaStream_t>(g->stream);
+    sim->device = dev;
     sim->nc = g->nc;
     sim->periodic = g->boundary == PIC_PERIODIC;
     sim->dx = g->dx;
@@ -395,17 +434,19 @@ extern "C" int pic_create(const pic_grid_desc *g, const pic_species_desc *specie
         // E padded to an even number of nodes (+2) so that 16-byte bulk copies of any window stay inside
         e = cudaMalloc(&sim->d_E, sizeof(double) * ((size_t)g->nc + 8));
         if (e != cudaSuccess) { rc = e == cudaErrorMemoryAllocation ? PIC_ENOMEM : cuda_fail(e, "cudaMalloc E"); break; }
+        for (int i = 0; i < nspecies && rc == PIC_OK; ++i) { // all allocations first: nothing here waits on the stream
+            pic_species *s = nullptr;
+            rc = alloc_species(sim, species[i], &s);
+            if (s) sim->sp.push_back(s);
+        }
+        if (rc != PIC_OK) break;
         e = cudaMemsetAsync(sim->d_E, 0, sizeof(double) * ((size_t)g->nc + 8), sim->stream);
         if (e != cudaSuccess) { rc = cuda_fail(e, "cudaMemsetAsync E"); break; }
         e = cudaMemcpyAsync(sim->d_E, g->E_nodes, sizeof(double) * ((size_t)g->nc + 1), cudaMemcpyHostToDevice, sim->stream);
         if (e != cudaSuccess) { rc = cuda_fail(e, "cudaMemcpyAsync E"); break; }
         e = cudaStreamSynchronize(sim->stream);
         if (e != cudaSuccess) { rc = cuda_fail(e, "cudaStreamSynchronize"); break; }
-        for (int i = 0; i < nspecies && rc == PIC_OK; ++i) {
-            pic_species *s = nullptr;
-            rc = create_species(sim, species[i], &s);
-            if (s) sim->sp.push_back(s);
-        }
+        for (int i = 0; i < nspecies && rc == PIC_OK; ++i) rc = init_species(sim, sim->sp[i], species[i]);
     } while (0);
     if (rc != PIC_OK) {
         pic_destroy(sim);
@@ -432,9 +473,98 @@ extern "C" int pic_set_field(pic_sim *sim, const double *E)
         emax = std::max(emax, std::fabs(E[j]));
     }
     sim->Emax = emax;
+    sim->emax_known = true;
     for (pic_species *s : sim->sp) s->vkick = 2.0 * std::fabs(s->k.h) * emax;
     CU(cudaMemcpyAsync(sim->d_E, E, sizeof(double) * ((size_t)sim->nc + 1), cudaMemcpyHostToDevice, sim->stream));
     CU(cudaStreamSynchronize(sim->stream)); // E is a caller buffer that may be pageable
+    return PIC_OK;
+}
+
+// scratch of the field solve, allocated on first use
+static int field_alloc(pic_sim *sim)
+{
+    if (sim->d_emax) return PIC_OK;
+    const size_t nb = sizeof(double) * ((size_t)sim->nc + 8);
+    const size_t nt = (size_t)fld_ntiles(sim->nc);
+    cudaError_t e = cudaMalloc(&sim->d_f[0], nb);
+    if (e == cudaSuccess) e = cudaMalloc(&sim->d_f[1], nb);
+    if (e == cudaSuccess) e = cudaMalloc(&sim->d_phi, nb);
+    if (e == cudaSuccess) e = cudaMalloc(&sim->d_tile, sizeof(double) * 4 * nt);
+    if (e == cudaSuccess) e = cudaMalloc(&sim->d_scal, sizeof(double) * 4);
+    if (e == cudaSuccess) e = cudaMalloc(&sim->d_emax, sizeof(unsigned long long));
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? PIC_ENOMEM : cuda_fail(e, "cudaMalloc field scratch");
+    return PIC_OK;
+}
+
+// steps already enqueued must have run (or be redone by the split kernels) with the field they were issued under
+static int field_barrier(pic_sim *sim)
+{
+    for (pic_species *s : sim->sp)
+        if (int rc = verify_fused(s)) return rc;
+    return PIC_OK;
+}
+
+extern "C" int pic_set_field_device(pic_sim *sim, const double *E_dev)
+{
+    if (!sim || !E_dev) return PIC_EINVAL;
+    if (int rc = field_barrier(sim)) return rc;
+    if (int rc = field_alloc(sim)) return rc;
+    const int nc = sim->nc;
+    CU(cudaMemcpyAsync(sim->d_E, E_dev, sizeof(double) * ((size_t)nc + 1), cudaMemcpyDeviceToDevice, sim->stream));
+    CU(cudaMemsetAsync(sim->d_emax, 0, sizeof(unsigned long long), sim->stream));
+    KernelSpan span(sim, K_FIELD);
+    field_emax_kernel<<<(nc + 1 + FLD_THREADS - 1) / FLD_THREADS, FLD_THREADS, 0, sim->stream>>>(sim->d_E, nc, sim->d_emax);
+    if (int rc = launch_check(sim, "field_emax_kernel")) return rc;
+    sim->emax_known = false;
+    return PIC_OK;
+}
+
+extern "C" int pic_solve_field(pic_sim *sim, const double *rho_dev, int smooth_passes, double *phi_dev)
+{
+    if (!sim || !rho_dev || smooth_passes < 0 || smooth_passes > 1024) return PIC_EINVAL;
+    if (sim->nc < 2) return PIC_EINVAL;
+    if (int rc = field_barrier(sim)) return rc;
+    if (int rc = field_alloc(sim)) return rc;
+    const int nc = sim->nc;
+    const int nblk = (nc + 1 + FLD_THREADS - 1) / FLD_THREADS;
+    KernelSpan span(sim, K_FIELD);
+    const double *rho = rho_dev;
+    for (int p = 0; p < smooth_passes; ++p) {
+        double *out = sim->d_f[p & 1];
+        field_smooth_kernel<<<nblk, FLD_THREADS, 0, sim->stream>>>(rho, out, nc, sim->periodic);
+        if (int rc = launch_check(sim, "field_smooth_kernel")) return rc;
+        rho = out;
+    }
+    FieldArgs a{};
+    a.rho = rho; a.phi = sim->d_phi; a.E = sim->d_E; a.phi_out = phi_dev;
+    a.ntiles = fld_ntiles(nc);
+    a.tile_s = sim->d_tile; a.tile_t = sim->d_tile + a.ntiles; a.tile_sum = sim->d_tile + 2 * (size_t)a.ntiles;
+    a.tile_lo = sim->d_tile + 3 * (size_t)a.ntiles;
+    a.scal = sim->d_scal; a.emax_bits = sim->d_emax;
+    a.nc = nc; a.periodic = sim->periodic;
+    { volatile double d2 = sim->dx * sim->dx; a.dx2 = d2; volatile double inv = 1.0 / sim->dx; a.inv_dx = inv; }
+    CU(cudaMemsetAsync(sim->d_emax, 0, sizeof(unsigned long long), sim->stream));
+    if (sim->periodic) {
+        field_sum_kernel<<<a.ntiles, FLD_THREADS, 0, sim->stream>>>(a);
+        if (int rc = launch_check(sim, "field_sum_kernel")) return rc;
+    }
+    field_tile_kernel<<<a.ntiles, FLD_THREADS, 0, sim->stream>>>(a);
+    if (int rc = launch_check(sim, "field_tile_kernel")) return rc;
+    field_chain_kernel<<<1, FLD_THREADS, 0, sim->stream>>>(a);
+    if (int rc = launch_check(sim, "field_chain_kernel")) return rc;
+    field_phi_kernel<<<a.ntiles, FLD_THREADS, 0, sim->stream>>>(a);
+    if (int rc = launch_check(sim, "field_phi_kernel")) return rc;
+    field_e_kernel<<<nblk, FLD_THREADS, 0, sim->stream>>>(a);
+    if (int rc = launch_check(sim, "field_e_kernel")) return rc;
+    sim->emax_known = false;
+    return PIC_OK;
+}
+
+extern "C" int pic_get_field(pic_sim *sim, double *E_host)
+{
+    if (!sim || !E_host) return PIC_EINVAL;
+    CU(cudaMemcpyAsync(E_host, sim->d_E, sizeof(double) * ((size_t)sim->nc + 1), cudaMemcpyDeviceToHost, sim->stream));
+    CU(cudaStreamSynchronize(sim->stream));
     return PIC_OK;
 }
 
@@ -445,6 +575,8 @@ extern "C" int pic_set_option(pic_sim *sim, const char *key, int value)
     if (!strcmp(key, "tile_scatter") && flag) sim->opt_tile_scatter = value;
     else if (!strcmp(key, "kernel_timing") && flag) sim->opt_timing = value;
     else if (!strcmp(key, "fused") && flag) sim->opt_fused = value;
+    else if (!strcmp(key, "fused_tma") && flag) sim->opt_fused_tma = value;
+    else if (!strcmp(key, "fused_pdl") && flag) sim->opt_fused_pdl = value;
     else if (!strcmp(key, "fused_cells_per_cta") && value >= 0 && value <= FUSED_CPC_MAX) sim->opt_fused_cpc = value;
     else if (!strcmp(key, "fused_stage_slots") && value >= 0 && value <= 512 && value % 2 == 0) sim->opt_fused_slots = value;
     else if (!strcmp(key, "fused_stages") && value >= 0 && value <= 2) sim->opt_fused_stages = value;
@@ -515,6 +647,9 @@ static int arrange_split(pic_species *s, bool hist_ready, bool after_mover)
     a.off_old = s->d_off[oo]; a.count_new = s->d_count[on]; a.off_new = s->d_off[on];
     a.st = s->d_st; a.nc = nc; a.periodic = sim->periodic;
     a.w_limit = FAST_W_LIMIT;
+    // general path: enqueued only if the host-side displacement bound cannot rule it out
+    const bool general_follows = !(s->h_grouped && s->h_wsum <= FAST_W_LIMIT);
+    a.general_follows = general_follows ? 1 : 0;
     {
         KernelSpan span(sim, K_SCATTER);
         // tile-ranked stable scatter (tilesort.cuh) when the caller gave a workspace; the destination-driven
@@ -526,6 +661,7 @@ static int arrange_split(pic_species *s, bool hist_ready, bool after_mover)
             t.dx = a.dx; t.dvx = a.dvx; t.dvy = a.dvy; t.dvz = a.dvz; t.dcell = a.dcell;
             t.off_old = a.off_old; t.off_new = a.off_new; t.st = s->d_st;
             t.nc = nc; t.periodic = sim->periodic; t.w_limit = FAST_W_LIMIT;
+            t.general_follows = a.general_follows;
             const int nt = (int)ts_ntiles(s->n_ub);
             t.tinfo = reinterpret_cast<int2 *>(s->ws);
             t.thist = reinterpret_cast<int *>(static_cast<char *>(s->ws) + (((size_t)(nt + 1) * sizeof(int2) + 255) & ~(size_t)255));
@@ -542,9 +678,9 @@ static int arrange_split(pic_species *s, bool hist_ready, bool after_mover)
         scatter_fast_kernel<<<blocks, SCATTER_THREADS, 0, sim->stream>>>(a);
         if (int rc = launch_check(sim, "scatter_fast_kernel")) return rc;
     }
-    // general path: enqueued only if the host-side displacement bound cannot rule it out; every
-    // kernel of it returns at once unless scatter_fast_kernel declined on the device
-    if (!(s->h_grouped && s->h_wsum <= FAST_W_LIMIT)) {
+    // every kernel of the general path returns at once unless scatter_fast_kernel declined on the device; if it is not
+    // enqueued and the device declines after all (the host bound was wrong), ERR_ARRANGE_SKIPPED is raised
+    if (general_follows) {
         GeneralArgs ga{};
         ga.sx = a.sx; ga.svx = a.svx; ga.svy = a.svy; ga.svz = a.svz; ga.scell = a.scell;
         ga.dx = a.dx; ga.dvx = a.dvx; ga.dvy = a.dvy; ga.dvz = a.dvz; ga.dcell = a.dcell;
@@ -604,6 +740,7 @@ static int push_split(pic_species *s, bool will_arrange)
     }
     s->h_wsum = std::min<long long>(s->h_wsum + host_step_bound(s), 1LL << 40);
     s->h_steps_since_sync++;
+    s->h_kick_acc += s->vkick;
     if (!sim->periodic) s->all_live = false;
     s->counts_fresh = false;
     if (!will_arrange) {
@@ -663,7 +800,9 @@ static FusedGeom fused_geom(const pic_species *s)
     g.rows = sim->opt_fused_rows;
     if (g.rows == 0) g.rows = need <= 8 * 32 ? 8 : need <= 12 * 32 ? 12 : need <= 16 * 32 ? 16 : 0;
     if (g.rows == 0) return g;
-    g.stages = sim->opt_fused_stages ? sim->opt_fused_stages : FUSED_STAGES_DEFAULT;
+    // two stages under the 8-row tiles (11 CTAs of 19.7 KB per SM: measured 3-7 % faster than one stage at 16 CTAs);
+    // the wider tiles keep one stage (a second one would halve their CTAs per SM: measured slower)
+    g.stages = !sim->opt_fused_tma ? 0 : (sim->opt_fused_stages ? sim->opt_fused_stages : (g.rows == 8 ? 2 : 1));
     g.cpc = fused_cells_per_cta(s, g.rows, g.stages);
     g.slots = sim->opt_fused_slots ? std::min(sim->opt_fused_slots, g.rows * 32) : g.rows * 32;
     g.smem = (size_t)fused_layout(g.rows * 32, g.cpc, g.stages).total;
@@ -725,12 +864,24 @@ static int push_fused(pic_species *s)
         fused_edge_kernel<<<1, 128, 0, sim->stream>>>(a);
         if (int rc = launch_check(sim, "fused_edge_kernel")) return rc;
         const bool bz0 = s->k.tz == 0.0 && s->k.sz == 0.0; // B in the x-y plane: the kernel drops the exact-zero products
-        void (*kern)(FusedArgs);
-#define PIC_FUSED_PICK(P, Z) (rows == 8 ? fused_kernel<8, P, Z> : rows == 12 ? fused_kernel<12, P, Z> : fused_kernel<16, P, Z>)
-        if (sim->periodic) kern = bz0 ? PIC_FUSED_PICK(true, true) : PIC_FUSED_PICK(true, false);
-        else kern = bz0 ? PIC_FUSED_PICK(false, true) : PIC_FUSED_PICK(false, false);
-#undef PIC_FUSED_PICK
-        kern<<<grid, 32, smem, sim->stream>>>(a);
+        void (*kern)(FusedArgs) = fused_pick(rows, sim->periodic != 0, bz0, sim->opt_fused_tma != 0);
+        if (sim->opt_fused_pdl) {
+            // programmatic dependent launch: the CTAs start while fused_edge_kernel is still running and do their
+            // prologue (offsets, E window, first bulk copies); griddepcontrol.wait holds them before anything else
+            cudaLaunchConfig_t cfg{};
+            cfg.gridDim = dim3((unsigned)grid);
+            cfg.blockDim = dim3(32);
+            cfg.dynamicSmemBytes = smem;
+            cfg.stream = sim->stream;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            attr[0].val.programmaticStreamSerializationAllowed = 1;
+            cfg.attrs = attr;
+            cfg.numAttrs = 1;
+            CU(cudaLaunchKernelEx(&cfg, kern, a));
+        } else {
+            kern<<<grid, 32, smem, sim->stream>>>(a);
+        }
         if (int rc = launch_check(sim, "fused_kernel")) return rc;
         fused_commit_kernel<<<1, 1, 0, sim->stream>>>(s->d_st, a.step_id);
         if (int rc = launch_check(sim, "fused_commit_kernel")) return rc;
@@ -743,6 +894,7 @@ static int push_fused(pic_species *s)
     }
     s->unv_steps++;
     s->h_steps_since_sync++;
+    s->h_kick_acc += s->vkick;
     s->cur = dst;
     s->cur_off = on;
     s->counts_fresh = true;
@@ -782,6 +934,7 @@ static int verify_fused(pic_species *s)
     s->h_grouped = true;
     s->h_vmax = std::sqrt((double)bits_to_float(h.vmax2));
     s->h_steps_since_sync = 0;
+    s->h_kick_acc = 0;
     s->h_maxcount = h.maxcount;
     for (long long left = run - k; left > 0;) {
         const int chunk = (int)std::min<long long>(left, 1 << 20);
@@ -822,6 +975,18 @@ static int read_state(pic_species *s, DevState &h)
     if (h.n >= 0 && h.n <= s->n_ub) s->n_ub = h.n;
     s->h_vmax = std::sqrt((double)bits_to_float(h.vmax2));
     s->h_steps_since_sync = 0;
+    s->h_kick_acc = 0;
+    if (!s->sim->emax_known) { // the field was replaced on the device: fetch its max |E| for the displacement bound
+        pic_sim *sim = s->sim;
+        unsigned long long bits = 0;
+        CU(cudaMemcpyAsync(&bits, sim->d_emax, sizeof bits, cudaMemcpyDeviceToHost, sim->stream));
+        CU(cudaStreamSynchronize(sim->stream));
+        double em;
+        memcpy(&em, &bits, sizeof em);
+        sim->Emax = em;
+        sim->emax_known = true;
+        for (pic_species *o : sim->sp) o->vkick = 2.0 * std::fabs(o->k.h) * em;
+    }
     if (h.fused_disabled) s->fused_off = true;
     s->h_maxcount = h.maxcount;
     s->h_abort_reason = h.abort_reason;
@@ -860,6 +1025,16 @@ extern "C" int pic_n_slots(pic_species *s, int64_t *n)
     DevState h;
     if (int rc = read_state(s, h)) return rc;
     *n = h.n;
+    return status_to_rc(h.status);
+}
+
+extern "C" int pic_n_live(pic_species *s, int64_t *n)
+{
+    if (!s || !n) return PIC_EINVAL;
+    DevState h;
+    if (int rc = read_state(s, h)) return rc;
+    // slots in use minus the particles absorbed (flagged, still in place) since the last arrange
+    *n = (int64_t)h.n - (int64_t)((h.wall[0] + h.wall[1]) - h.wall_arr);
     return status_to_rc(h.status);
 }
 
@@ -965,54 +1140,75 @@ extern "C" int pic_run_host(const pic_grid_desc *g, pic_host_species *hs, int ns
 {
     if (!g || !hs || nspecies < 1 || nsteps < 0) return PIC_EINVAL;
     cudaStream_t stream = static_cast<cudaStream_t>(g->stream);
+    // optional wall-clock trace of the phases (stderr), switched on by the environment variable PIC_TRACE
+    const bool trace = getenv("PIC_TRACE") != nullptr;
+    const auto t_begin = std::chrono::steady_clock::now();
+    auto mark = [&](const char *what) {
+        if (!trace) return;
+        cudaStreamSynchronize(stream);
+        const double ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count();
+        fprintf(stderr, "[pic_run_host] %-28s %9.3f ms\n", what, ms);
+    };
     std::vector<pic_species_desc> descs(nspecies);
-    std::vector<void *> allocs;
     int rc = PIC_OK;
     pic_sim *sim = nullptr;
-    auto dmalloc = [&](size_t bytes) -> void * {
-        void *p = nullptr;
-        if (cudaMalloc(&p, bytes ? bytes : 16) != cudaSuccess) { cudaGetLastError(); return nullptr; }
-        allocs.push_back(p);
-        return p;
-    };
+    char *arena = nullptr;
+    cudaStream_t copy_stream = nullptr;
+    auto align256 = [](size_t b) { return (b + 255) & ~(size_t)255; };
     do {
-        for (int i = 0; i < nspecies && rc == PIC_OK; ++i) {
-            pic_host_species &h = hs[i];
+        // one device allocation for everything: two buffer sets and the workspace of every species
+        size_t total = 0;
+        for (int i = 0; i < nspecies; ++i) {
+            const pic_host_species &h = hs[i];
             if (h.n < 0 || (h.n > 0 && (!h.x || !h.vx || !h.vy || !h.vz || !h.cell))) { rc = PIC_EINVAL; break; }
+            const size_t nb = align256(sizeof(double) * (size_t)h.n + 16), ni = align256(sizeof(int32_t) * (size_t)h.n + 16);
+            total += 2 * (4 * nb + ni) + align256(pic_workspace_bytes(g->nc, h.n) + 16);
+        }
+        if (rc) break;
+        cudaError_t e = cudaMalloc(&arena, total ? total : 256);
+        if (e != cudaSuccess) { cudaGetLastError(); arena = nullptr; rc = PIC_ENOMEM; break; }
+        mark("device arena allocated");
+        size_t off = 0;
+        auto carve = [&](size_t bytes) { void *p = arena + off; off += bytes; return p; };
+        for (int i = 0; i < nspecies; ++i) {
+            pic_host_species &h = hs[i];
             pic_species_desc &d = descs[i];
             memset(&d, 0, sizeof d);
             d.qm = h.qm; d.n = h.n; d.capacity = h.n; d.arrange_every = h.arrange_every;
-            const size_t nb = sizeof(double) * (size_t)h.n, ni = sizeof(int32_t) * (size_t)h.n;
+            const size_t nb = align256(sizeof(double) * (size_t)h.n + 16), ni = align256(sizeof(int32_t) * (size_t)h.n + 16);
             for (int b = 0; b < 2; ++b) {
-                d.x[b] = (double *)dmalloc(nb); d.vx[b] = (double *)dmalloc(nb);
-                d.vy[b] = (double *)dmalloc(nb); d.vz[b] = (double *)dmalloc(nb);
-                d.cell[b] = (int32_t *)dmalloc(ni);
-                if (!d.x[b] || !d.vx[b] || !d.vy[b] || !d.vz[b] || !d.cell[b]) { rc = PIC_ENOMEM; break; }
+                d.x[b] = (double *)carve(nb); d.vx[b] = (double *)carve(nb);
+                d.vy[b] = (double *)carve(nb); d.vz[b] = (double *)carve(nb);
+                d.cell[b] = (int32_t *)carve(ni);
             }
-            if (rc) break;
             d.workspace_bytes = pic_workspace_bytes(g->nc, h.n);
-            d.workspace = dmalloc(d.workspace_bytes);
-            if (!d.workspace) { rc = PIC_ENOMEM; break; }
-            cudaError_t e = cudaSuccess;
+            d.workspace = carve(align256(d.workspace_bytes + 16));
+            const size_t cb = sizeof(double) * (size_t)h.n, ci = sizeof(int32_t) * (size_t)h.n;
             if (h.n > 0) {
-                e = cudaMemcpyAsync(d.x[0], h.x, nb, cudaMemcpyHostToDevice, stream);
-                if (e == cudaSuccess) e = cudaMemcpyAsync(d.vx[0], h.vx, nb, cudaMemcpyHostToDevice, stream);
-                if (e == cudaSuccess) e = cudaMemcpyAsync(d.vy[0], h.vy, nb, cudaMemcpyHostToDevice, stream);
-                if (e == cudaSuccess) e = cudaMemcpyAsync(d.vz[0], h.vz, nb, cudaMemcpyHostToDevice, stream);
-                if (e == cudaSuccess) e = cudaMemcpyAsync(d.cell[0], h.cell, ni, cudaMemcpyHostToDevice, stream);
+                e = cudaMemcpyAsync(d.x[0], h.x, cb, cudaMemcpyHostToDevice, stream);
+                if (e == cudaSuccess) e = cudaMemcpyAsync(d.cell[0], h.cell, ci, cudaMemcpyHostToDevice, stream);
+                if (e == cudaSuccess) e = cudaMemcpyAsync(d.vx[0], h.vx, cb, cudaMemcpyHostToDevice, stream);
+                if (e == cudaSuccess) e = cudaMemcpyAsync(d.vy[0], h.vy, cb, cudaMemcpyHostToDevice, stream);
+                if (e == cudaSuccess) e = cudaMemcpyAsync(d.vz[0], h.vz, cb, cudaMemcpyHostToDevice, stream);
             }
             if (e != cudaSuccess) { rc = cuda_fail(e, "cudaMemcpyAsync H2D"); break; }
         }
         if (rc) break;
+        mark("H2D done");
         rc = pic_create(g, descs.data(), nspecies, &sim);
         if (rc) break;
+        mark("pic_create done");
         for (int i = 0; i < nspecies && rc == PIC_OK; ++i) rc = pic_push(sim->sp[i], nsteps);
         if (rc) break;
+        mark("steps done");
+        // the copies back: each array on a second stream as soon as its species has been read out, so that they
+        // queue behind one another without host round trips
+        if (cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking) != cudaSuccess) { rc = cuda_fail(cudaGetLastError(), "copy stream"); break; }
         for (int i = 0; i < nspecies && rc == PIC_OK; ++i) {
             pic_species *s = sim->sp[i];
             pic_host_species &h = hs[i];
             pic_wall_flux_t wf;
-            rc = pic_wall_flux(s, &wf);
+            rc = pic_wall_flux(s, &wf); // syncs: the species' state is final
             if (rc) break;
             int64_t n = 0;
             rc = pic_n_slots(s, &n);
@@ -1020,20 +1216,27 @@ extern "C" int pic_run_host(const pic_grid_desc *g, pic_host_species *hs, int ns
             h.n_out = n; h.wall_left = wf.left_total; h.wall_right = wf.right_total;
             const size_t nb = sizeof(double) * (size_t)n, ni = sizeof(int32_t) * (size_t)n;
             const int b = s->cur;
-            cudaError_t e = cudaSuccess;
+            e = cudaSuccess;
             if (n > 0) {
-                e = cudaMemcpyAsync(h.x, s->x[b], nb, cudaMemcpyDeviceToHost, stream);
-                if (e == cudaSuccess) e = cudaMemcpyAsync(h.vx, s->vx[b], nb, cudaMemcpyDeviceToHost, stream);
-                if (e == cudaSuccess) e = cudaMemcpyAsync(h.vy, s->vy[b], nb, cudaMemcpyDeviceToHost, stream);
-                if (e == cudaSuccess) e = cudaMemcpyAsync(h.vz, s->vz[b], nb, cudaMemcpyDeviceToHost, stream);
-                if (e == cudaSuccess) e = cudaMemcpyAsync(h.cell, s->cell[b], ni, cudaMemcpyDeviceToHost, stream);
+                e = cudaMemcpyAsync(h.x, s->x[b], nb, cudaMemcpyDeviceToHost, copy_stream);
+                if (e == cudaSuccess) e = cudaMemcpyAsync(h.vx, s->vx[b], nb, cudaMemcpyDeviceToHost, copy_stream);
+                if (e == cudaSuccess) e = cudaMemcpyAsync(h.vy, s->vy[b], nb, cudaMemcpyDeviceToHost, copy_stream);
+                if (e == cudaSuccess) e = cudaMemcpyAsync(h.vz, s->vz[b], nb, cudaMemcpyDeviceToHost, copy_stream);
+                if (e == cudaSuccess) e = cudaMemcpyAsync(h.cell, s->cell[b], ni, cudaMemcpyDeviceToHost, copy_stream);
             }
-            if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
             if (e != cudaSuccess) { rc = cuda_fail(e, "cudaMemcpyAsync D2H"); break; }
         }
+        if (rc == PIC_OK) {
+            e = cudaStreamSynchronize(copy_stream);
+            if (e != cudaSuccess) rc = cuda_fail(e, "cudaStreamSynchronize D2H");
+        }
+        mark("D2H done");
     } while (0);
+    if (copy_stream) { cudaStreamSynchronize(copy_stream); cudaStreamDestroy(copy_stream); }
     if (sim) pic_destroy(sim);
     else cudaStreamSynchronize(stream);
-    for (void *p : allocs) cudaFree(p);
+    mark("sim destroyed");
+    if (arena) cudaFree(arena);
+    mark("arena released");
     return rc;
 }

@@ -16,6 +16,7 @@ constexpr int ERR_NEED_WORKSPACE = 2; // general arranger needed but no / too sm
 constexpr int ERR_BAD_INITIAL = 4;    // initial state violates cell == floor(x/dx), live, in range
 constexpr int ERR_NOT_GROUPED = 8;    // (info) initial state is not grouped by cell
 constexpr int ERR_FUSED_OVERFLOW = 16; // (info) fused step fell back to the split path
+constexpr int ERR_ARRANGE_SKIPPED = 32; // the fast arranger declined on the device but the general path was not enqueued
 
 constexpr int W_UNKNOWN = 1 << 29; // displacement bound of a state that is not grouped by cell
 
@@ -30,6 +31,7 @@ struct DevState {
     int fused_disabled; // sticky: a fused step has declined (fail_step says which); later fused launches exit at once
     unsigned long long wall[2];      // cumulative absorbed at x<0 / x>=L
     unsigned long long wall_pend[2]; // fused step in flight: absorbed, not yet committed
+    unsigned long long wall_arr;     // wall[0] + wall[1] at the last arrange (n - absorbed since = live particles)
     unsigned vmax2, vmax2_next;      // float bits (rounded up) of max |v|^2: current state / step in flight
     int n_next;                      // fused step in flight: particle count after it
     int abort;                       // fused step in flight: some CTA declined

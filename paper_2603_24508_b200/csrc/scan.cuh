@@ -140,7 +140,10 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_exclusive_kernel(const int 
     if (tile == ntiles - 1 && threadIdx.x == 0) {
         int grand = s_prefix + total;
         out[m] = grand;
-        if (fold.st && fold.set_n) fold.st->n = grand;
+        if (fold.st && fold.set_n) {
+            fold.st->n = grand;
+            fold.st->wall_arr = fold.st->wall[0] + fold.st->wall[1]; // the mover of this step has finished: stream order
+        }
     }
 }
 

@@ -43,6 +43,7 @@ struct TileArgs {
     int *thist;         // per tile TS_WIN entries: counts, then first slots
     DevState *st;
     int nc, periodic, w_limit;
+    int general_follows; // the host has enqueued the general path behind (else declining is an error)
 };
 
 // bin of cell c in a window starting at cell cmin (circular on a periodic grid)
@@ -140,7 +141,10 @@ __global__ void __launch_bounds__(256) tile_base_kernel(TileArgs a)
     if (*(volatile int *)&st->tile_declined) return;
     const int W = st->w_acc;
     if (W > a.w_limit) { // the displacement bound is too large for a window: the general path must run
-        if (c == 0) st->need_general = 1;
+        if (c == 0) {
+            st->need_general = 1;
+            if (!a.general_follows) atomicOr(&st->status, ERR_ARRANGE_SKIPPED);
+        }
         return;
     }
     const int nc = a.nc;

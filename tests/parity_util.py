@@ -15,8 +15,8 @@ import paper_2603_24508_b200 as pic
 RTOL, ATOL = 1e-12, 1e-14
 
 
-def close(a, b):
-    return np.all(np.abs(a - b) <= np.maximum(ATOL, RTOL * np.abs(b)))
+def close(a, b, rtol=RTOL, atol=ATOL):
+    return np.all(np.abs(a - b) <= np.maximum(atol, rtol * np.abs(b)))
 
 
 def make_pair(inp, *, arrange_every=None, capacity_pad=0, workspace=True, options=None, stream=None):
@@ -36,7 +36,7 @@ def make_pair(inp, *, arrange_every=None, capacity_pad=0, workspace=True, option
     return sim, states
 
 
-def compare(sp, st, *, where="", bitwise=True, counts=False, nc=None):
+def compare(sp, st, *, where="", bitwise=True, counts=False, nc=None, rtol=RTOL, atol=ATOL):
     """Compare the GPU species `sp` with the oracle state `st` over the slots in use."""
     n_gpu = pic.pic_n_slots(sp)
     assert n_gpu == st.n, f"{where}: slots in use {n_gpu} != oracle {st.n}"
@@ -45,7 +45,7 @@ def compare(sp, st, *, where="", bitwise=True, counts=False, nc=None):
     names = ("x", "vx", "vy", "vz", "cell")
     assert np.array_equal(g[4], o[4]), f"{where}: cell / dead flags differ at {np.flatnonzero(g[4] != o[4])[:8]}"
     for k in range(4):
-        assert close(g[k], o[k]), f"{where}: {names[k]} outside tolerance, max abs diff {np.max(np.abs(g[k] - o[k]))}"
+        assert close(g[k], o[k], rtol, atol), f"{where}: {names[k]} outside tolerance, max abs diff {np.max(np.abs(g[k] - o[k]))}"
         if bitwise:
             assert np.array_equal(g[k], o[k]), (f"{where}: {names[k]} not bitwise equal at "
                                                 f"{np.flatnonzero(g[k] != o[k])[:8]}")

@@ -1,0 +1,224 @@
+"""GPU parity of the field solve (pic_solve_field: 1-2-1 smoother -> 1D Poisson -> E)
+and of the device-resident field (pic_set_field_device), pic_n_live, and the closed PIC loop
+push -> arrange -> deposit -> smooth -> solve -> push against the same loop of the oracle.
+
+Tolerance: the kernels sum in a fixed tree, the oracle eliminates sequentially (in long
+double), so phi agrees to rounding, not bitwise:  |phi_gpu - phi_oracle| <= 1e-12 * max|phi|   (north_star's
+floating-point bar, relative to the largest potential: an absolute error in phi is what a prefix sum produces).
+E is a difference of two potentials over dx, so it inherits  1e-12 * max|phi| / dx  (and never less than
+1e-12 * max|E|).  The filter is the same two rounded additions on both sides: bitwise.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2603_24508_b200 as pic
+from paper_2603_24508_b200 import workloads
+from parity_util import compare
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-12
+
+
+def _tiny_sim(nc, boundary, dx=1.0, n=0):
+    """A sim that exists only to own a grid (one particle in cell 0)."""
+    x = np.array([0.5 * dx])
+    z = np.zeros(1)
+    sp = pic.make_species(x, z, z, z, np.zeros(1, dtype=np.int32), qm=-1.0, arrange_every=1)
+    return pic.pic_create(nc=nc, dx=dx, dt=0.1, boundary=boundary, E_nodes=np.zeros(nc + 1), B=[0.0, 0.0, 0.0], species=[sp])
+
+
+def _rho_cases(nc, boundary, rng):
+    j = np.arange(nc + 1, dtype=np.float64)
+    cases = {
+        "noise": rng.normal(size=nc + 1),
+        "uniform": np.full(nc + 1, 0.37),
+        "sine+net": np.sin(2 * np.pi * 3 * j / nc) + 0.2,
+        "quasi-neutral": 1e-3 * rng.normal(size=nc + 1) * (1.0 + np.cos(2 * np.pi * j / nc)),
+        "point": np.where(j == nc // 3, 5.0, 0.0),
+    }
+    if boundary == workloads.PERIODIC:
+        for v in cases.values():
+            v[nc] = v[0]
+    return cases
+
+
+def _check_fields(sim, rho, nc, dx, boundary, passes, where):
+    rho_t = torch.from_numpy(rho).cuda()
+    phi_t = pic.pic_solve_field(sim, rho_t, smooth_passes=passes, want_phi=True)
+    E = pic.pic_get_field(sim)
+    phi = phi_t.cpu().numpy()
+    rs, phi_o, E_o = oracle.field_solve(rho, nc, dx, boundary, passes)
+    # scale of the potential: max|phi|, and never less than the rounding floor of the right-hand side dx^2*rho (a
+    # filtered-then-neutralised rho can vanish identically, e.g. the Nyquist mode on a ring: phi is then pure rounding)
+    pmax = max(np.max(np.abs(phi_o)), dx * dx * np.max(np.abs(rho)))
+    assert np.max(np.abs(phi - phi_o)) <= TOL * pmax, f"{where}: phi differs by {np.max(np.abs(phi - phi_o)) / pmax:.3e} of max|phi|"
+    etol = TOL * max(np.max(np.abs(E_o)), pmax / dx)
+    assert np.max(np.abs(E - E_o)) <= etol, f"{where}: E differs by {np.max(np.abs(E - E_o)):.3e} (bound {etol:.3e})"
+    if boundary == workloads.PERIODIC:
+        assert E[nc] == E[0] and phi[nc] == phi[0]
+    else:
+        assert phi[0] == 0.0 and phi[nc] == 0.0
+    return phi, E
+
+
+@pytest.mark.parametrize("boundary", [workloads.PERIODIC, workloads.ABSORBING])
+@pytest.mark.parametrize("nc", [2, 3, 17, 2047, 2048, 2049, 5000, 65536, 100000])
+def test_solve_field_matches_oracle(nc, boundary):
+    rng = np.random.default_rng(1000 + nc)
+    dx = [1.0, 0.5, 0.3][nc % 3]
+    sim = _tiny_sim(nc, boundary, dx)
+    for name, rho in _rho_cases(nc, boundary, rng).items():
+        for passes in (0, 1, 3):
+            _check_fields(sim, rho, nc, dx, boundary, passes, f"nc={nc} boundary={boundary} {name} passes={passes}")
+    pic.pic_destroy(sim)
+
+
+@pytest.mark.parametrize("boundary", [workloads.PERIODIC, workloads.ABSORBING])
+def test_solve_field_at_config4_size_and_repeatable(boundary):
+    nc, dx = 1_000_000, 1.0
+    rng = np.random.default_rng(7)
+    sim = _tiny_sim(nc, boundary, dx)
+    rho = _rho_cases(nc, boundary, rng)["noise"] * 0.05 + 0.01
+    phi1, E1 = _check_fields(sim, rho, nc, dx, boundary, 2, "config-4 size")
+    phi2, E2 = _check_fields(sim, rho, nc, dx, boundary, 2, "config-4 size, again")
+    assert np.array_equal(phi1, phi2) and np.array_equal(E1, E2), "the solve must be bitwise reproducible"
+    pic.pic_destroy(sim)
+
+
+@pytest.mark.parametrize("boundary", [workloads.PERIODIC, workloads.ABSORBING])
+def test_filter_alone_is_bitwise(boundary):
+    """E of a solve with k passes == E of a solve without passes fed the oracle's filtered rho: bit for bit, which
+    holds only if the device filter produced exactly the oracle's filtered values."""
+    nc, dx = 5000, 1.0
+    rng = np.random.default_rng(11)
+    sim = _tiny_sim(nc, boundary, dx)
+    rho = rng.normal(size=nc + 1)
+    if boundary == workloads.PERIODIC:
+        rho[nc] = rho[0]
+    for passes in (1, 2, 5):
+        pic.pic_solve_field(sim, torch.from_numpy(rho).cuda(), smooth_passes=passes)
+        Ea = pic.pic_get_field(sim)
+        pic.pic_solve_field(sim, torch.from_numpy(oracle.smooth(rho, nc, boundary, passes)).cuda(), smooth_passes=0)
+        Eb = pic.pic_get_field(sim)
+        assert np.array_equal(Ea, Eb)
+    pic.pic_destroy(sim)
+
+
+def test_solve_field_argument_errors():
+    sim = _tiny_sim(16, workloads.PERIODIC)
+    L = pic.lib()
+    rho = torch.zeros(17, dtype=torch.float64, device="cuda")
+    assert L.pic_solve_field(sim.handle, None, 0, None) == pic.PIC_EINVAL
+    assert L.pic_solve_field(sim.handle, rho.data_ptr(), -1, None) == pic.PIC_EINVAL
+    assert L.pic_set_field_device(sim.handle, None) == pic.PIC_EINVAL
+    assert L.pic_get_field(sim.handle, None) == pic.PIC_EINVAL
+    assert L.pic_n_live(None, None) == pic.PIC_EINVAL
+    pic.pic_destroy(sim)
+
+
+@pytest.mark.parametrize("config,kw", [(1, dict(nc=256, ppc=32)), (5, dict(nc=2048))])
+def test_set_field_device_equals_set_field(config, kw):
+    """The same run with the field replaced from a host array and from a device array: identical states, and both
+    identical to the oracle given the new field (fused and split paths; config 5 arranges every 10th step, so the
+    host-side displacement bound, unknown after a device-side field change, is exercised)."""
+    inp = workloads.make(config, **kw)
+    rng = np.random.default_rng(3)
+    E2 = inp["E"] + 0.02 * rng.normal(size=inp["nc"] + 1)
+    if inp["boundary"] == workloads.PERIODIC:
+        E2[-1] = E2[0]
+    s = inp["species"][0]
+    sims = []
+    for mode in ("host", "device"):
+        sp = pic.make_species(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], qm=s["qm"], arrange_every=inp["arrange_every"])
+        sim = pic.pic_create(nc=inp["nc"], dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E_nodes=inp["E"],
+                             B=inp["B"], species=[sp])
+        pic.pic_push(sim.species[0], 7)
+        if mode == "host":
+            pic.pic_set_field(sim, E2)
+        else:
+            pic.pic_set_field_device(sim, torch.from_numpy(E2).cuda())
+        pic.pic_push(sim.species[0], 23)
+        assert np.array_equal(pic.pic_get_field(sim), E2)
+        sims.append(sim)
+    st = oracle.State(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], nc=inp["nc"], dx=inp["dx"], dt=inp["dt"],
+                      boundary=inp["boundary"], E=inp["E"].copy(), qm=s["qm"], B=inp["B"],
+                      arrange_every=inp["arrange_every"])
+    st.push(7)
+    st.E[:] = E2
+    st.push(23)
+    for sim in sims:
+        compare(sim.species[0], st, where=f"config {config}")
+        assert pic.pic_arrange_info(sim.species[0])[1] == 0
+        pic.pic_destroy(sim)
+
+
+def test_n_live_between_arranges():
+    inp = workloads.make(5, nc=1024)
+    s = inp["species"][0]
+    sp_d = pic.make_species(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], qm=s["qm"], arrange_every=10)
+    sim = pic.pic_create(nc=inp["nc"], dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E_nodes=inp["E"], B=inp["B"],
+                         species=[sp_d])
+    sp = sim.species[0]
+    st = oracle.State(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], nc=inp["nc"], dx=inp["dx"], dt=inp["dt"],
+                      boundary=inp["boundary"], E=inp["E"], qm=s["qm"], B=inp["B"], arrange_every=10)
+    saw_gap = False
+    for step in range(1, 41):
+        pic.pic_push(sp, 1)
+        st.push(1)
+        live = int(np.count_nonzero(st.cell[:st.n] >= 0))
+        assert pic.pic_n_live(sp) == live, f"step {step}"
+        assert pic.pic_n_slots(sp) == st.n
+        saw_gap |= live != st.n
+        if step % 10 == 0:
+            assert pic.pic_n_live(sp) == pic.pic_n_slots(sp)
+    assert saw_gap, "the case must absorb particles between arranges"
+    pic.pic_arrange(sp)
+    st.arrange()
+    assert pic.pic_n_live(sp) == pic.pic_n_slots(sp) == st.n
+    pic.pic_destroy(sim)
+
+
+@pytest.mark.parametrize("boundary_cfg", [3, 1])
+def test_closed_pic_loop_against_the_oracle_loop(boundary_cfg):
+    """push -> arrange -> deposit (all species) -> smooth -> solve -> push ..., 20 steps, field kept on the device
+    (reduced config 3: e- + D+, absorbing walls; reduced config 1 with a neutralising background: periodic)."""
+    if boundary_cfg == 3:
+        inp = workloads.make(3, nc=1500)
+    else:
+        inp = workloads.make(1, nc=1024, ppc=64)
+    nc, dx, boundary = inp["nc"], inp["dx"], inp["boundary"]
+    ppc = len(inp["species"][0]["x"]) / nc
+    w = 0.25 / ppc  # density 0.25: omega_p dt = 0.05, Debye length 2 cells
+    weights = [-w if s["qm"] < 0 else w for s in inp["species"]]
+    passes = 2
+    descs, states = [], []
+    for s in inp["species"]:
+        descs.append(pic.make_species(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], qm=s["qm"], arrange_every=1))
+        states.append(oracle.State(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], nc=nc, dx=dx, dt=inp["dt"],
+                                   boundary=boundary, E=inp["E"].copy(), qm=s["qm"], B=inp["B"], arrange_every=1))
+    sim = pic.pic_create(nc=nc, dx=dx, dt=inp["dt"], boundary=boundary, E_nodes=inp["E"], B=inp["B"], species=descs)
+    for step in range(1, 21):
+        rho_t = None
+        for si, sp in enumerate(sim.species):
+            pic.pic_push(sp, 1)
+            rho_t = pic.pic_deposit(sp, weights[si], rho=rho_t, accumulate=si > 0)
+        pic.pic_solve_field(sim, rho_t, smooth_passes=passes)
+        rho_o = np.zeros(nc + 1)
+        for si, st in enumerate(states):
+            st.push(1)
+            rho_o = rho_o + st.deposit(weights[si])
+        _, phi_o, E_o = oracle.field_solve(rho_o, nc, dx, boundary, passes)
+        for st in states:
+            st.E[:] = E_o
+        E = pic.pic_get_field(sim)
+        pmax = np.max(np.abs(phi_o))
+        assert np.max(np.abs(E - E_o)) <= 1e-11 * max(np.max(np.abs(E_o)), pmax / dx), f"step {step}: E drifted"
+        for si, (sp, st) in enumerate(zip(sim.species, states)):
+            # the fields agree to rounding (1e-12 of max|phi|/dx), not bitwise, so from the second step on neither do
+            # the particles: each step adds a kick difference h*dE to v; cells, counts, order and walls stay exact
+            compare(sp, st, where=f"closed loop step {step} species {si}", bitwise=False, counts=True, nc=nc,
+                    rtol=1e-10, atol=1e-11)
+    assert np.max(np.abs(E_o)) > 0
+    pic.pic_destroy(sim)

@@ -17,6 +17,7 @@ VARIANTS = [
     pytest.param({"fused": 0, "tile_scatter": 0}, id="split-destscatter"),
     pytest.param({"fused": 1}, id="fused"),
     pytest.param({"fused": 1, "fused_stages": 2}, id="fused-2stage"),
+    pytest.param({"fused": 1, "fused_tma": 0}, id="fused-plainloads"),
 ]
 
 
@@ -529,3 +530,42 @@ def test_fused_path_comes_back_after_the_cause_is_gone():
                 seen_back = True
     assert seen_off and seen_back, "fused path should have declined and then come back"
     assert pic.pic_fused_info(sp)["decline_reasons"] & 1
+
+
+def test_bench_guard_fires_when_a_fused_step_declines_in_the_timed_region():
+    """bench.py must not be able to time skipped work: a particle that jumps two cells a few steps into the timed
+    region makes a fused step decline; the redo by the split kernels has to fall inside the timed region
+    (pic_sync before the closing event), the line must say so ("invalid", fused_path) and the exit code is 3."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    inp = workloads.make(1)
+    s = inp["species"][0]
+    p, vz = 7777, 26.0
+    probe = oracle.State(s["x"][p:p + 1], np.zeros(1), np.zeros(1), np.full(1, vz), s["cell"][p:p + 1], nc=inp["nc"],
+                         dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E=inp["E"], qm=s["qm"], B=inp["B"], arrange_every=0)
+    first = None
+    for k in range(1, 24):
+        c0 = int(probe.cell[0])
+        probe.push(1)
+        d = abs(int(probe.cell[0]) - c0)
+        if min(d, inp["nc"] - d) >= 2:
+            first = k
+            break
+    assert first is not None and 3 < first <= 23, f"the jump must fall inside the timed region (step {first})"
+    cmd = [sys.executable, os.path.join(root, "bench.py"), "--config", "1", "--steps", "20", "--warmup", "3", "--no-e2e",
+           "--no-cpu", "--no-deposit", "--debug-fast-particle", str(vz)]
+    r = subprocess.run(cmd, capture_output=True, text=True, cwd=root, timeout=600)
+    assert r.returncode == 3, (r.returncode, r.stderr[-2000:])
+    line = json.loads(r.stdout.strip().splitlines()[-1])
+    assert line["invalid"] is True and "declined" in line["invalid_reason"]
+    fp = line["fused_path"]
+    assert fp["expected"] and fp["split_mover_steps"] > 0 and fp["decline_reasons"][0] & 1 and fp["active_after"] == [0]
+    # and the clean run carries the same keys with nothing declined
+    r = subprocess.run(cmd[:-2], capture_output=True, text=True, cwd=root, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    line = json.loads(r.stdout.strip().splitlines()[-1])
+    fp = line["fused_path"]
+    assert "invalid" not in line and fp["split_mover_steps"] == 0 and fp["fused_steps"] == 20 and fp["decline_reasons"] == [0]
