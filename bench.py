@@ -241,6 +241,34 @@ def workload_config(config, inp):
     return out
 
 
+def compact(line):
+    r = line.get("roofline") or {}
+    return {"value": line["value"], "ms_per_step": line["ms_per_step"], "kernel": r.get("kernel"), "frac": r.get("frac"),
+            "step_frac": r.get("step_frac"), "kernel_ms_per_step": r.get("kernel_ms_per_step"),
+            "particles": line["config"].get("particles"), "sm_mhz": (line.get("clocks") or {}).get("sm_mhz"),
+            "reasons": (line.get("clocks") or {}).get("reasons"), "fused_path": line.get("fused_path"),
+            "deposit_frac": (line.get("deposit") or {}).get("frac"), "invalid": line.get("invalid", False)}
+
+
+def per_config_block(args, own_line):
+    """The five configs in one place: this run's own, and the other four measured by this script in subprocesses
+    (device-resident leg only: no e2e, no CPU baseline), 30 timed steps after 3 warm-up steps each."""
+    import subprocess
+    out = {str(args.config): compact(own_line)}
+    for c in (1, 2, 3, 4, 5):
+        if c == args.config:
+            continue
+        cmd = [sys.executable, os.path.abspath(__file__), "--config", str(c), "--steps", "30", "--warmup", "3", "--no-e2e",
+               "--no-cpu", "--no-field"] + [a for o in args.option for a in ("--option", o)]
+        r = subprocess.run(cmd, capture_output=True, text=True, cwd=ROOT)
+        try:
+            out[str(c)] = compact(json.loads(r.stdout.strip().splitlines()[-1]))
+            out[str(c)]["exit_code"] = r.returncode
+        except Exception as e:
+            out[str(c)] = {"error": repr(e), "exit_code": r.returncode, "stderr": r.stderr[-500:]}
+    return out
+
+
 # ----------------------------------------------------------------------------------------------
 # main arm
 # ----------------------------------------------------------------------------------------------
@@ -254,6 +282,9 @@ def main():
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the CPU-oracle baseline leg")
     ap.add_argument("--no-deposit", action="store_true", help="skip the separate timing of pic_deposit")
+    ap.add_argument("--no-field", action="store_true", help="skip the separate timing of pic_solve_field and of the closed cycle")
+    ap.add_argument("--all-configs", action="store_true",
+                    help="append a compact per_config block: the other four configs, each run by this script in a subprocess")
     ap.add_argument("--option", action="append", default=[], help="pic_set_option key=value (e.g. fused=0)")
     ap.add_argument("--scale", type=float, default=1.0, help="scale nc (debug only; the line is then not a bench value)")
     ap.add_argument("--debug-fast-particle", type=float, default=None, metavar="VZ",
@@ -395,6 +426,37 @@ def main():
             deposit = {"ms_per_call": d_ms, "calls": int(dn), "algorithmic_bytes_per_particle": DEPOSIT_BYTES,
                        "achieved": d_gbs, "unit": "GB/s", "frac": d_gbs / peak, "particles_per_call": n_per_launch,
                        "total_charge_check": float(rho[:-1].sum().item() if all_live else rho.sum().item())}
+    # the row after that: the field solve on the device (two filter passes, Poisson,
+    # E), and one whole PIC cycle with the field kept on the device: push + arrange, deposit (all species), solve
+    field = None
+    cycle = None
+    if deposit is not None and not args.no_field:
+        pic.pic_kernel_time(sim, "field")
+        for _ in range(20):
+            pic.pic_solve_field(sim, rho, smooth_passes=2)
+        fms, fn = pic.pic_kernel_time(sim, "field")
+        if fn:
+            field = {"ms_per_call": fms / fn, "calls": int(fn), "nodes": inp["nc"] + 1, "smooth_passes": 2,
+                     "note": "launch-latency bound: 8-24 MB of node data, 7 small kernels"}
+        pic.pic_set_field(sim, inp["E"])  # the workload's own field again
+        wts = [(-1.0 if s["qm"] < 0 else 1.0) * 1e-4 / max(1.0, n_per_launch / inp["nc"]) for s in inp["species"]]
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ncyc = 10
+        torch.cuda.synchronize()
+        c0.record(stream)
+        for _ in range(ncyc):
+            r = None
+            for si, sp in enumerate(sim.species):
+                pic.pic_push(sp, 1)
+                r = pic.pic_deposit(sp, wts[si], rho=r, accumulate=si > 0)
+            pic.pic_solve_field(sim, r, smooth_passes=2)
+        pic.pic_sync(sim)
+        c1.record(stream)
+        torch.cuda.synchronize()
+        cms = c0.elapsed_time(c1) / ncyc
+        cycle = {"ms_per_cycle": cms, "cycles": ncyc, "pushes_per_s": n_per_launch * len(sim.species) / (cms * 1e-3),
+                 "what": "pic_push(1) + pic_deposit per species, pic_solve_field(2 passes); E never leaves the device",
+                 "fused_declines": [pic.pic_fused_info(sp)["decline_reasons"] for sp in sim.species]}
     pic.pic_destroy(sim)
     del descs, sim
     torch.cuda.empty_cache()
@@ -440,7 +502,7 @@ def main():
                 "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic", "config": workload_config(args.config, inp),
                 "clocks": sampler.result(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-                "cpu_baseline": cpu, "deposit": deposit, "fused_path": fused_path,
+                "cpu_baseline": cpu, "deposit": deposit, "field_solve": field, "pic_cycle": cycle, "fused_path": fused_path,
                 "path": {"arranger": ["general" if g else "fast" for (_, g) in info],
                          "options": args.option, "numpy": np.__version__}}
         if args.scale != 1.0:
@@ -448,6 +510,8 @@ def main():
             line["config"]["workload"] += f" SCALED x{args.scale} (debug, not a bench value)"
         if args.debug_fast_particle is not None:
             line["config"]["workload"] += " with an injected fast particle (debug, not a bench value)"
+        if args.all_configs and world == 1:
+            line["per_config"] = per_config_block(args, line)
         if invalid:
             line["invalid"] = True
             line["invalid_reason"] = invalid

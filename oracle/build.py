@@ -22,10 +22,23 @@ SRC_FIELD = os.path.join(HERE, "oracle_field.c")
 LIB_FIELD = os.path.join(HERE, "liboracle_field.so")
 
 
+# ORACLE_SANITIZE=1: build and load AddressSanitizer + UndefinedBehaviorSanitizer variants (separate files) instead;
+# run the oracle's own test-suite under them with
+#   LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 ORACLE_SANITIZE=1 \
+#       python -m pytest tests/test_oracle_mover.py tests/test_oracle_arranger.py tests/test_oracle_deposit.py \
+#       tests/test_oracle_omp.py tests/test_oracle_field.py -q
+SANITIZE = os.environ.get("ORACLE_SANITIZE", "") not in ("", "0")
+SAN_FLAGS = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
+
+
 def _compile(src, lib, extra, force):
+    flags = list(FLAGS)
+    if SANITIZE:
+        lib = lib[:-3] + "_san.so"
+        flags = [f for f in flags if f != "-O2"] + SAN_FLAGS
     if not force and os.path.exists(lib) and os.path.getmtime(lib) >= os.path.getmtime(src):
         return lib
-    subprocess.run(["gcc", *FLAGS, *extra, "-o", lib, src, "-lm"], check=True)
+    subprocess.run(["gcc", *flags, *extra, "-o", lib, src, "-lm"], check=True)
     return lib
 
 

@@ -67,6 +67,7 @@ struct FieldArgs {
     double *tile_lo;   // per tile: low word of the double-double sum of rho
     double *scal;      // [0] mean of rho, [1] F, [2] mean of phi, [3] low word of the mean of rho
     unsigned long long *emax_bits; // max |E| as the bits of a non-negative double
+    unsigned *ticket;  // two arrival counters (zero between launches): the last block of a reduction finishes it
     int nc, periodic, ntiles;
     double dx2, inv_dx;
 };
@@ -152,6 +153,19 @@ __global__ void __launch_bounds__(FLD_THREADS) field_sum_kernel(FieldArgs a)
         for (int w = 0; w < FLD_THREADS / 32; ++w) r = fld_dd_add(r, s_w[w]);
         a.tile_sum[blockIdx.x] = r.hi;
         a.tile_lo[blockIdx.x] = r.lo;
+        __threadfence();
+        if (atomicAdd(a.ticket, 1u) == gridDim.x - 1) { // the last tile to arrive adds the tile sums, in tile order
+            __threadfence();
+            FieldDD sum{0.0, 0.0};
+            for (int t = 0; t < a.ntiles; ++t)
+                sum = fld_dd_add(sum, FieldDD{((volatile double *)a.tile_sum)[t], ((volatile double *)a.tile_lo)[t]});
+            const double n = (double)a.nc;
+            const double q = sum.hi / n;
+            const double rem = __fma_rn(-q, n, sum.hi); // exact remainder of the division
+            a.scal[0] = q;
+            a.scal[3] = __dadd_rn(rem, sum.lo) / n;
+            *a.ticket = 0u;
+        }
     }
 }
 
@@ -159,18 +173,6 @@ __global__ void __launch_bounds__(FLD_THREADS) field_sum_kernel(FieldArgs a)
 __device__ __forceinline__ double fld_r(const FieldArgs &a, int j, double mhi, double mlo)
 {
     return (j >= 1 && j <= a.nc - 1) ? a.dx2 * __dsub_rn(__dsub_rn(a.rho[j], mhi), mlo) : 0.0;
-}
-
-// mean of rho from the tile sums as a double-double (every block adds them in the same order)
-__device__ __forceinline__ FieldDD fld_mean(const FieldArgs &a)
-{
-    if (!a.periodic) return FieldDD{0.0, 0.0};
-    FieldDD sum{0.0, 0.0};
-    for (int t = 0; t < a.ntiles; ++t) sum = fld_dd_add(sum, FieldDD{a.tile_sum[t], a.tile_lo[t]});
-    const double n = (double)a.nc;
-    const double q = sum.hi / n;
-    const double rem = __fma_rn(-q, n, sum.hi); // exact remainder of the division
-    return FieldDD{q, __dadd_rn(rem, sum.lo) / n};
 }
 
 // The in-tile scan: thread-local over FLD_ITEMS nodes, then an ordered scan of the thread aggregates.
@@ -209,10 +211,7 @@ __device__ __forceinline__ FieldSeg fld_tile_scan(const double (&r)[FLD_ITEMS], 
 __global__ void __launch_bounds__(FLD_THREADS) field_tile_kernel(FieldArgs a)
 {
     __shared__ FieldSeg s_w[FLD_THREADS / 32];
-    __shared__ FieldDD s_mean;
-    if (threadIdx.x == 0) s_mean = fld_mean(a);
-    __syncthreads();
-    const FieldDD mean = s_mean;
+    const FieldDD mean{a.scal[0], a.scal[3]}; // zero on a bounded grid; written by field_sum_kernel on a periodic one
     const int base = blockIdx.x * FLD_TILE + threadIdx.x * FLD_ITEMS;
     double r[FLD_ITEMS];
 #pragma unroll
@@ -222,7 +221,6 @@ __global__ void __launch_bounds__(FLD_THREADS) field_tile_kernel(FieldArgs a)
     if (threadIdx.x == 0) {
         a.tile_s[blockIdx.x] = total.s;
         a.tile_t[blockIdx.x] = total.t;
-        if (blockIdx.x == 0) { a.scal[0] = mean.hi; a.scal[3] = mean.lo; }
     }
 }
 
@@ -302,27 +300,27 @@ __global__ void __launch_bounds__(FLD_THREADS) field_phi_kernel(FieldArgs a)
         T += S;
     }
     psum = fld_block_sum(psum, s_sum);
-    if (threadIdx.x == 0) a.tile_sum[blockIdx.x] = psum;
+    if (threadIdx.x == 0) {
+        a.tile_sum[blockIdx.x] = psum;
+        __threadfence();
+        if (atomicAdd(a.ticket + 1, 1u) == gridDim.x - 1) { // last tile: the mean of phi (the gauge of a periodic grid)
+            __threadfence();
+            double sum = 0.0;
+            if (a.periodic)
+                for (int t = 0; t < a.ntiles; ++t) sum += ((volatile double *)a.tile_sum)[t];
+            a.scal[2] = sum / (double)a.nc;
+            a.ticket[1] = 0u;
+        }
+    }
 }
 
 // E from phi (S26), gauge shift on a periodic grid (S25), max |E|, optional copy of phi
 __global__ void __launch_bounds__(FLD_THREADS) field_e_kernel(FieldArgs a)
 {
-    __shared__ double s_pm;
     __shared__ unsigned long long s_max;
-    if (threadIdx.x == 0) {
-        double pm = 0.0;
-        if (a.periodic) {
-            double sum = 0.0;
-            for (int t = 0; t < a.ntiles; ++t) sum += a.tile_sum[t];
-            pm = sum / (double)a.nc;
-        }
-        s_pm = pm;
-        s_max = 0ull;
-        if (blockIdx.x == 0) a.scal[2] = pm;
-    }
+    if (threadIdx.x == 0) s_max = 0ull;
     __syncthreads();
-    const double pm = s_pm;
+    const double pm = a.scal[2]; // zero on a bounded grid
     const int nc = a.nc;
     const int j = blockIdx.x * FLD_THREADS + threadIdx.x;
     double e = 0.0;

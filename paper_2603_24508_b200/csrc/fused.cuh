@@ -63,6 +63,7 @@ struct FusedArgs {
     int SCAP; // largest tile, in slots (<= RMAX*32, even)
     int NST;  // stages of the ring: 1 or 2
     int step_id; // low 31 bits of the species' step counter before this step
+    int COLS, RUN; // chunk of CTA b = (b % COLS) * RUN + b / COLS: COLS = CTAs resident at once, RUN = ceil(chunks / COLS)
 };
 
 // Dynamic shared memory of one fused_kernel CTA (one warp): NST stages of CAP = RMAX*32 slots.
@@ -491,9 +492,13 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
     int bad = 0;  // FA_* bits
     int mc = 0;   // largest new per-cell count seen by this lane
 
-    {
+    // CTAs are dispatched in blockIdx order and a new one starts when an old one ends, so slot (b % COLS) of the
+    // machine works through chunks RUN*slot, RUN*slot + 1, ... one after the other: the halo cell a chunk shares with
+    // its neighbour is read by the two CTAs back to back (option "fused_columns"; COLS = number of chunks: chunk = b).
+    const int chunk = ((int)blockIdx.x % a.COLS) * a.RUN + (int)blockIdx.x / a.COLS;
+    if ((long long)chunk * a.CPC < nc) { // else: a spare CTA of the last columns
         FusedCtx X;
-        X.C0 = blockIdx.x * a.CPC;
+        X.C0 = chunk * a.CPC;
         X.C1 = min(X.C0 + a.CPC, nc);
         X.Cm = max(X.C0 - 1, 0);
         X.nc = nc;

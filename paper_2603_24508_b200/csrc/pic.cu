@@ -100,7 +100,7 @@ struct pic_sim {
     int device = 0;
     std::vector<pic_species *> sp;
     unsigned long long launches = 0;
-    int opt_fused = 1, opt_timing = 0, opt_tile_scatter = 1, opt_fused_tma = 1, opt_fused_pdl = 1;
+    int opt_fused = 1, opt_timing = 0, opt_tile_scatter = 1, opt_fused_tma = 1, opt_fused_pdl = 1, opt_fused_cols = 0;
     int opt_fused_cpc = 0, opt_fused_rows = 0, opt_fused_slots = 0, opt_fused_stages = 0; // tuning knobs of the fused step (0 = automatic)
     int sm_count = 148;
     // per-kernel device timing (option "kernel_timing"): event pairs recorded around launches
@@ -491,7 +491,9 @@ static int field_alloc(pic_sim *sim)
     if (e == cudaSuccess) e = cudaMalloc(&sim->d_phi, nb);
     if (e == cudaSuccess) e = cudaMalloc(&sim->d_tile, sizeof(double) * 4 * nt);
     if (e == cudaSuccess) e = cudaMalloc(&sim->d_scal, sizeof(double) * 4);
-    if (e == cudaSuccess) e = cudaMalloc(&sim->d_emax, sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(&sim->d_emax, 2 * sizeof(unsigned long long)); // max |E| bits, two tickets
+    if (e == cudaSuccess) e = cudaMemsetAsync(sim->d_emax, 0, 2 * sizeof(unsigned long long), sim->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(sim->d_scal, 0, sizeof(double) * 4, sim->stream);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? PIC_ENOMEM : cuda_fail(e, "cudaMalloc field scratch");
     return PIC_OK;
 }
@@ -541,6 +543,7 @@ extern "C" int pic_solve_field(pic_sim *sim, const double *rho_dev, int smooth_p
     a.tile_s = sim->d_tile; a.tile_t = sim->d_tile + a.ntiles; a.tile_sum = sim->d_tile + 2 * (size_t)a.ntiles;
     a.tile_lo = sim->d_tile + 3 * (size_t)a.ntiles;
     a.scal = sim->d_scal; a.emax_bits = sim->d_emax;
+    a.ticket = reinterpret_cast<unsigned *>(sim->d_emax + 1);
     a.nc = nc; a.periodic = sim->periodic;
     { volatile double d2 = sim->dx * sim->dx; a.dx2 = d2; volatile double inv = 1.0 / sim->dx; a.inv_dx = inv; }
     CU(cudaMemsetAsync(sim->d_emax, 0, sizeof(unsigned long long), sim->stream));
@@ -577,6 +580,7 @@ extern "C" int pic_set_option(pic_sim *sim, const char *key, int value)
     else if (!strcmp(key, "fused") && flag) sim->opt_fused = value;
     else if (!strcmp(key, "fused_tma") && flag) sim->opt_fused_tma = value;
     else if (!strcmp(key, "fused_pdl") && flag) sim->opt_fused_pdl = value;
+    else if (!strcmp(key, "fused_columns") && flag) sim->opt_fused_cols = value;
     else if (!strcmp(key, "fused_cells_per_cta") && value >= 0 && value <= FUSED_CPC_MAX) sim->opt_fused_cpc = value;
     else if (!strcmp(key, "fused_stage_slots") && value >= 0 && value <= 512 && value % 2 == 0) sim->opt_fused_slots = value;
     else if (!strcmp(key, "fused_stages") && value >= 0 && value <= 2) sim->opt_fused_stages = value;
@@ -852,7 +856,10 @@ static int push_fused(pic_species *s)
     a.NST = geo.stages;
     a.step_id = (int)(s->steps & 0x7fffffff);
     const int rows = geo.rows;
-    const int grid = (sim->nc + a.CPC - 1) / a.CPC;
+    const int nchunks = (sim->nc + a.CPC - 1) / a.CPC;
+    a.COLS = sim->opt_fused_cols ? std::max(1, std::min(nchunks, sim->sm_count * geo.ctas_per_sm)) : nchunks;
+    a.RUN = (nchunks + a.COLS - 1) / a.COLS;
+    const int grid = a.COLS * a.RUN;
     const size_t smem = geo.smem;
     if (s->unv_steps == 0) {
         s->unv_steps0 = s->steps;

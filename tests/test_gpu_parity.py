@@ -569,3 +569,38 @@ def test_bench_guard_fires_when_a_fused_step_declines_in_the_timed_region():
     line = json.loads(r.stdout.strip().splitlines()[-1])
     fp = line["fused_path"]
     assert "invalid" not in line and fp["split_mover_steps"] == 0 and fp["fused_steps"] == 20 and fp["decline_reasons"] == [0]
+
+
+@pytest.mark.parametrize("options", VARIANTS)
+@pytest.mark.parametrize("config,kw,steps", [(2, dict(nc=1024), 30), (5, dict(nc=2048), 30), (4, dict(nc=1531), 20)])
+def test_no_write_beyond_the_initial_slot_count(options, config, kw, steps):
+    """compute-sanitizer is closed on this pool (profiles/r02_sanitizers.md), so the bound is checked by hand: the
+    buffers are allocated with 333 spare slots filled with a sentinel; the particle count never grows, so no kernel
+    of any path (fused, split, tile-ranked, destination-driven) may ever write a slot >= n0 of either buffer set."""
+    import torch
+    inp = workloads.make(config, **kw)
+    pad = 333
+    sim, states = make_pair(inp, capacity_pad=pad, options=options)
+    sent_f, sent_i = -1.2345678e300, -77777
+    n0s = []
+    for sp, s in zip(sim.species, inp["species"]):
+        n0 = len(s["x"])
+        n0s.append(n0)
+        for b in range(2):
+            for t in sp.bufs[b][:4]:
+                t[n0:].fill_(sent_f)
+            sp.bufs[b][4][n0:].fill_(sent_i)
+    torch.cuda.synchronize()
+    for sp, st in zip(sim.species, states):
+        pic.pic_push(sp, steps)
+        st.push(steps)
+        pic.pic_arrange(sp)
+        st.arrange()
+        compare(sp, st, where=f"config {config} with spare capacity", counts=True, nc=inp["nc"])
+    pic.pic_sync(sim)
+    for sp, n0 in zip(sim.species, n0s):
+        for b in range(2):
+            for t in sp.bufs[b][:4]:
+                assert bool((t[n0:] == sent_f).all()), "a kernel wrote beyond the initial slot count"
+            assert bool((sp.bufs[b][4][n0:] == sent_i).all()), "a kernel wrote beyond the initial slot count (cell)"
+    pic.pic_destroy(sim)
