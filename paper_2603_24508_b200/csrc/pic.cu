@@ -290,6 +290,7 @@ static int fused_set_attributes(int device)
             for (int bz0 = 0; bz0 < 2; ++bz0)
                 for (int tma = 0; tma < 2; ++tma) kerns.push_back(fused_pick(rows, per != 0, bz0 != 0, tma != 0));
     for (auto kfn : kerns) CU(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    CU(cudaFuncSetAttribute(tile_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TS_SMEM_BYTES));
     if (device >= 0 && device < 64) done[device] = true;
     return PIC_OK;
 }
@@ -673,7 +674,7 @@ static int arrange_split(pic_species *s, bool hist_ready, bool after_mover)
             if (int rc = launch_check(sim, "tile_hist_kernel")) return rc;
             tile_base_kernel<<<(nc + 255) / 256, 256, 0, sim->stream>>>(t);
             if (int rc = launch_check(sim, "tile_base_kernel")) return rc;
-            tile_scatter_kernel<<<nt, TS_THREADS, (TS_WARPS + 1) * TS_WIN * sizeof(int), sim->stream>>>(t);
+            tile_scatter_kernel<<<nt, TS_THREADS, TS_SMEM_BYTES, sim->stream>>>(t);
             if (int rc = launch_check(sim, "tile_scatter_kernel")) return rc;
             a.only_if = &s->d_st->tile_declined;
         }

@@ -23,7 +23,7 @@ constexpr int TS_THREADS = 256;
 constexpr int TS_WARPS = TS_THREADS / 32;
 constexpr int TS_ROWS = 8;                           // rows of 32 slots per warp segment
 constexpr int TS_TILE = TS_THREADS * TS_ROWS;        // 2048 source slots per tile
-constexpr int TS_WIN = 1024;                         // destination cells per tile window
+constexpr int TS_WIN = 512;                          // destination cells per tile window
 
 static inline long long ts_ntiles(long long n) { return (n + TS_TILE - 1) / TS_TILE; }
 static inline size_t ts_workspace_bytes(long long capacity)
@@ -170,25 +170,55 @@ __global__ void __launch_bounds__(256) tile_base_kernel(TileArgs a)
         const int s0 = pass ? rb0 : ra0, s1 = pass ? rb1 : ra1;
         if (s1 <= s0) continue;
         const int t0 = max(s0 / TS_TILE, tnext), t1 = (s1 - 1) / TS_TILE;
-        for (int t = t0; t <= t1; ++t) {
-            const int2 info = a.tinfo[t];
-            if (info.y <= 0) continue;
-            const int u = ts_bin(c, info.x, nc, a.periodic);
-            if ((unsigned)u < (unsigned)info.y) {
-                int *h = a.thist + (size_t)t * TS_WIN + u;
-                const int cnt = *h;
-                *h = run;
-                run += cnt;
+        // four tiles at a time: their window descriptors, then their counts, are loaded independently of one another
+        // (the walk is a latency chain otherwise: up to ~20 tiles per cell in the dense part of config 5)
+        for (int tq = t0; tq <= t1; tq += 4) {
+            int2 info[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) info[q] = tq + q <= t1 ? __ldg(a.tinfo + tq + q) : make_int2(0, 0);
+            int *h[4];
+            int cnt[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int u = info[q].y > 0 ? ts_bin(c, info[q].x, nc, a.periodic) : -1;
+                h[q] = (unsigned)u < (unsigned)info[q].y ? a.thist + (size_t)(tq + q) * TS_WIN + u : nullptr;
+                cnt[q] = h[q] ? *h[q] : 0;
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                if (h[q]) *h[q] = run;
+                run += cnt[q];
             }
         }
         tnext = max(tnext, t1 + 1);
     }
 }
 
+// Dynamic shared memory of tile_scatter_kernel: per-warp counters (16-bit: a warp segment has 256 slots, a tile 2048),
+// the tile's first slot and first staging place per window cell, and the staging area in which the tile is put into
+// DESTINATION order before it is written.  39 KB: five blocks per SM.
+constexpr size_t TS_SMEM_WC = (size_t)TS_WARPS * TS_WIN * sizeof(unsigned short);
+constexpr size_t TS_SMEM_TB = (size_t)TS_WIN * sizeof(int);
+constexpr size_t TS_SMEM_LBASE = ((size_t)(TS_WIN + 1) * sizeof(unsigned short) + 15) & ~(size_t)15;
+constexpr size_t TS_SMEM_BYTES = TS_SMEM_WC + TS_SMEM_TB + TS_SMEM_LBASE + (size_t)TS_TILE * (sizeof(int) + sizeof(unsigned short) + sizeof(double));
+
 // One block per tile; warp w owns the slots [w*256, w*256+256) of the tile, row by row.
+// Every particle gets its rank k among the tile's particles bound for the same cell (earlier warps' counts + rank in
+// slot order inside the warp), hence its final slot d = (tile's first slot of the cell) + k and its place in the
+// tile's own destination order lpos = (particles of the tile bound for lower cells) + k.  Field by field the tile is
+// then staged in shared memory in that order and written out with consecutive threads on consecutive slots of a run:
+// a tile that spreads over W cells writes W contiguous runs instead of 2048 scattered 8-byte stores (14.4 -> 8.2
+// sectors per request at config 5).
 __global__ void __launch_bounds__(TS_THREADS) tile_scatter_kernel(TileArgs a)
 {
-    extern __shared__ int ts_smem[]; // [TS_WARPS + 1][win]: per-warp counters, then the tile's first slots
+    extern __shared__ __align__(16) unsigned char ts_raw[];
+    unsigned short *wc_all = reinterpret_cast<unsigned short *>(ts_raw);                              // [TS_WARPS][win]
+    int *tb = reinterpret_cast<int *>(ts_raw + TS_SMEM_WC);                                           // [win] tile's first slot
+    unsigned short *lbase = reinterpret_cast<unsigned short *>(ts_raw + TS_SMEM_WC + TS_SMEM_TB);     // [win + 1]
+    double *stage = reinterpret_cast<double *>(ts_raw + TS_SMEM_WC + TS_SMEM_TB + TS_SMEM_LBASE);     // [TS_TILE] one field
+    int *sdest = reinterpret_cast<int *>(stage + TS_TILE);                                            // [TS_TILE] final slot
+    unsigned short *sbin = reinterpret_cast<unsigned short *>(sdest + TS_TILE);                       // [TS_TILE] window cell
+    __shared__ int s_scan[TS_WARPS];
     DevState *st = a.st;
     if (*(volatile int *)&st->tile_declined || *(volatile int *)&st->need_general) return;
     const int n = a.off_old[a.nc];
@@ -198,9 +228,8 @@ __global__ void __launch_bounds__(TS_THREADS) tile_scatter_kernel(TileArgs a)
     if (win <= 0) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const unsigned lt = (1u << lane) - 1u;
-    int *wc = ts_smem + warp * win;
-    int *tb = ts_smem + TS_WARPS * win;
-    for (int b = threadIdx.x; b < TS_WARPS * win; b += TS_THREADS) ts_smem[b] = 0;
+    unsigned short *wc = wc_all + warp * win;
+    for (int b = threadIdx.x; b < TS_WARPS * win; b += TS_THREADS) wc_all[b] = 0;
     {
         const int *h = a.thist + (size_t)t * TS_WIN;
         for (int b = threadIdx.x; b < win; b += TS_THREADS) tb[b] = h[b];
@@ -217,51 +246,95 @@ __global__ void __launch_bounds__(TS_THREADS) tile_scatter_kernel(TileArgs a)
         const unsigned live = __ballot_sync(FULL, bin[r] >= 0);
         if (bin[r] >= 0) {
             const unsigned m = __match_any_sync(live, bin[r]);
-            if ((m & lt) == 0) wc[bin[r]] += __popc(m);
+            if ((m & lt) == 0) wc[bin[r]] = (unsigned short)(wc[bin[r]] + __popc(m));
         }
         __syncwarp();
     }
     __syncthreads();
-    // first slot of every (warp, cell) group: the tile's first slot of the cell + the earlier warps' counts
-    for (int b = threadIdx.x; b < win; b += TS_THREADS) {
-        int run = tb[b];
+    // per window cell: the warps' counts become their first ranks (exclusive over the warps), and the tile's count,
+    // by a block-wide exclusive scan over the cells, the cell's first place in the staging order
+    {
+        constexpr int PER = TS_WIN / TS_THREADS; // window cells per thread, consecutive
+        int cnt[PER], tsum = 0;
 #pragma unroll
-        for (int w = 0; w < TS_WARPS; ++w) {
-            const int cnt = ts_smem[w * win + b];
-            ts_smem[w * win + b] = run;
-            run += cnt;
+        for (int q = 0; q < PER; ++q) {
+            const int b = threadIdx.x * PER + q;
+            int run = 0;
+            if (b < win) {
+#pragma unroll
+                for (int w = 0; w < TS_WARPS; ++w) {
+                    const int k = wc_all[w * win + b];
+                    wc_all[w * win + b] = (unsigned short)run;
+                    run += k;
+                }
+            }
+            cnt[q] = run;
+            tsum += run;
         }
+        int incl = tsum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int u = __shfl_up_sync(FULL, incl, o);
+            if (lane >= o) incl += u;
+        }
+        if (lane == 31) s_scan[warp] = incl;
+        __syncthreads();
+        int pre = incl - tsum;
+        for (int w = 0; w < warp; ++w) pre += s_scan[w];
+#pragma unroll
+        for (int q = 0; q < PER; ++q) {
+            const int b = threadIdx.x * PER + q;
+            if (b <= win) lbase[b] = (unsigned short)pre;
+            pre += cnt[q];
+        }
+        if (threadIdx.x == TS_THREADS - 1) lbase[TS_WIN] = (unsigned short)pre; // a full window ends behind the last thread's cells
     }
     __syncthreads();
-    // sweep B: rank inside the group in slot order, copy.  The source fields of four rows are loaded ahead of
-    // the ranking so that their latency overlaps it.
+    const int nlive = lbase[win];
+    // sweep B: rank inside the (tile, cell) group in slot order -> final slot and staging place of every particle
+    int lpos[TS_ROWS];
 #pragma unroll
-    for (int r0 = 0; r0 < TS_ROWS; r0 += 4) {
-        double x[4], vx[4], vy[4], vz[4];
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const long long i = base + (r0 + q) * 32 + lane;
-            if (bin[r0 + q] >= 0) { x[q] = a.sx[i]; vx[q] = a.svx[i]; vy[q] = a.svy[i]; vz[q] = a.svz[i]; }
-            else { x[q] = vx[q] = vy[q] = vz[q] = 0.0; }
+    for (int r = 0; r < TS_ROWS; ++r) {
+        const int bq = bin[r];
+        const unsigned live = __ballot_sync(FULL, bq >= 0);
+        lpos[r] = -1;
+        if (bq >= 0) {
+            const unsigned m = __match_any_sync(live, bq);
+            const int k = wc[bq] + __popc(m & lt);
+            __syncwarp(live);
+            if ((m & lt) == 0) wc[bq] = (unsigned short)(wc[bq] + __popc(m));
+            const int lp = lbase[bq] + k;
+            lpos[r] = lp;
+            sdest[lp] = tb[bq] + k;
+            sbin[lp] = (unsigned short)bq;
         }
+        __syncwarp();
+    }
+    // the four fp64 fields, one after the other through the staging area; the cell index rides with the first
+    const double *src[4] = {a.sx, a.svx, a.svy, a.svz};
+    double *dst[4] = {a.dx, a.dvx, a.dvy, a.dvz};
+    double v[TS_ROWS];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const int bq = bin[r0 + q];
-            const unsigned live = __ballot_sync(FULL, bq >= 0);
-            if (bq >= 0) {
-                const unsigned m = __match_any_sync(live, bq);
-                const int d = wc[bq] + __popc(m & lt);
-                __syncwarp(live);
-                if ((m & lt) == 0) wc[bq] += __popc(m);
-                int c = cmin + bq;
+    for (int r = 0; r < TS_ROWS; ++r) v[r] = lpos[r] >= 0 ? src[0][base + r * 32 + lane] : 0.0;
+#pragma unroll
+    for (int f = 0; f < 4; ++f) {
+        __syncthreads(); // sdest / sbin complete (f = 0); the previous field has left the staging area (f > 0)
+#pragma unroll
+        for (int r = 0; r < TS_ROWS; ++r)
+            if (lpos[r] >= 0) stage[lpos[r]] = v[r];
+        if (f < 3) { // the next field's loads fly while this one is written out
+#pragma unroll
+            for (int r = 0; r < TS_ROWS; ++r) v[r] = lpos[r] >= 0 ? src[f + 1][base + r * 32 + lane] : 0.0;
+        }
+        __syncthreads();
+        for (int i = threadIdx.x; i < nlive; i += TS_THREADS) {
+            const int g = sdest[i];
+            dst[f][g] = stage[i];
+            if (f == 0) {
+                int c = cmin + (int)sbin[i];
                 if (c >= a.nc) c -= a.nc;
-                a.dx[d] = x[q];
-                a.dvx[d] = vx[q];
-                a.dvy[d] = vy[q];
-                a.dvz[d] = vz[q];
-                a.dcell[d] = c;
+                a.dcell[g] = c;
             }
-            __syncwarp();
         }
     }
 }
