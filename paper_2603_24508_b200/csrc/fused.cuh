@@ -38,7 +38,8 @@ constexpr int FUSED_CPC_DEFAULT = 32;  // cells per chunk (per CTA) on grids of 
 constexpr int FUSED_CPC_SEARCH = 64;   // largest chunk the per-launch search considers on smaller grids
 constexpr int FUSED_CPC_MAX = 256;
 constexpr int FUSED_KMAX = 31;         // cells per tile (one lane per cell border)
-constexpr int FUSED_DEF = 32;          // deferred right-movers of a tile's last cell
+constexpr int FUSED_DEF = 32;          // deferred right-movers of a tile's last cell: the usual queue ...
+constexpr int FUSED_DEF_BIG = 128;     // ... and the one taken after a step has overflowed it (strongly drifting flows)
 constexpr int FUSED_XCAP = 256;        // edge kernel: leavers per edge cell
 constexpr int FUSED_TELEMETRY_STEPS = 4; // fused steps between two asynchronous copies of DevState to the host
 constexpr int FUSED_RETRY_STEPS = 16;  // split steps after a decline before the fused path is tried again
@@ -72,7 +73,7 @@ struct FusedLayout {
     int off_E, off_offs, off_cell, off_row, off_base, off_q, off_mbar, total;
 };
 
-__host__ __device__ inline FusedLayout fused_layout(int CAP, int CPC, int NST)
+__host__ __device__ inline FusedLayout fused_layout(int CAP, int CPC, int NST, int DEF = FUSED_DEF)
 {
     FusedLayout L;
     L.stage_bytes = 32 * CAP;
@@ -83,7 +84,7 @@ __host__ __device__ inline FusedLayout fused_layout(int CAP, int CPC, int NST)
     L.off_cell = o; o += 8 * (FUSED_KMAX + 1); // {first slot, count} of the tile's cells
     L.off_row = o;  o += 16 * 16;              // per row: the three class ballots and the running counts before it
     L.off_base = o; o += 8 * 4 * 32;           // per (class, cell): {slot base, destination cell}; class 3 = nothing to store
-    L.off_q = o;    o += FUSED_DEF * 40;
+    L.off_q = o;    o += DEF * 40;
     L.off_mbar = o; o += 32;
     L.total = o;
     return L;
@@ -469,21 +470,21 @@ __host__ __device__ constexpr int fused_group_count(int rmax, int gi) { return g
 // TMA = true: particles and the chunk's E window are staged in shared memory by bulk copies (cp.async.bulk + mbarrier).
 // TMA = false (option "fused_tma" = 0, the A/B variant of profiles/): plain read-only global loads into the same
 // registers, E through the read-only path; no stage, no mbarrier.
-template <int RMAX, bool PERIODIC, bool BZ0, bool TMA>
+// DEF = capacity of the queue of right-movers deferred to the next tile (FUSED_DEF, or FUSED_DEF_BIG after an overflow).
+template <int RMAX, bool PERIODIC, bool BZ0, bool TMA, int DEF>
 __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fused_kernel(FusedArgs a)
 {
     static_assert(RMAX == 8 || RMAX == 12 || RMAX == 16, "row groups of sweep 1a are written for these sizes");
     extern __shared__ __align__(128) unsigned char fused_smem[];
     constexpr int CAP = RMAX * 32;
-    const FusedLayout L = fused_layout(CAP, a.CPC, a.NST);
+    const FusedLayout L = fused_layout(CAP, a.CPC, a.NST, DEF);
     double *sE = reinterpret_cast<double *>(fused_smem + L.off_E);
     int *offs = reinterpret_cast<int *>(fused_smem + L.off_offs);
     int2 *cellinfo = reinterpret_cast<int2 *>(fused_smem + L.off_cell); // {first slot, count} of the tile's cells
     int4 *rowinfo = reinterpret_cast<int4 *>(fused_smem + L.off_row);   // per row: ballots L, S, R; running counts before it
     int2 *basd = reinterpret_cast<int2 *>(fused_smem + L.off_base);     // [class*32 + cell]: {slot base, destination cell}
-    double *qx = reinterpret_cast<double *>(fused_smem + L.off_q), *qvx = qx + FUSED_DEF, *qvy = qx + 2 * FUSED_DEF,
-           *qvz = qx + 3 * FUSED_DEF;
-    int *qpos = reinterpret_cast<int *>(qx + 4 * FUSED_DEF);
+    double *qx = reinterpret_cast<double *>(fused_smem + L.off_q), *qvx = qx + DEF, *qvy = qx + 2 * DEF, *qvz = qx + 3 * DEF;
+    int *qpos = reinterpret_cast<int *>(qx + 4 * DEF);
     const unsigned mb0 = smem_u32(fused_smem + L.off_mbar), mb1 = mb0 + 8, mbE = mb0 + 16;
     const int lane = threadIdx.x;
     const unsigned lt = (1u << lane) - 1u;
@@ -673,13 +674,18 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
                 mc = max(mc, cn);
             }
             if (ndef) { // right-movers of the previous tile's last cell: their cell is cA, its L count is known now
-                if (lane < ndef) {
-                    const int p = qpos[lane] + Lc0;
-                    if ((unsigned)p >= cap32) bad |= FA_BAD_PARTICLE;
-                    else {
-                        a.dx[p] = qx[lane]; a.dvx[p] = qvx[lane]; a.dvy[p] = qvy[lane]; a.dvz[p] = qvz[lane];
-                        a.dcell[p] = cA;
+#pragma unroll
+                for (int q0 = 0; q0 < DEF; q0 += 32) {
+                    const int q = q0 + lane;
+                    if (q < ndef) {
+                        const int p = qpos[q] + Lc0;
+                        if ((unsigned)p >= cap32) bad |= FA_BAD_PARTICLE;
+                        else {
+                            a.dx[p] = qx[q]; a.dvx[p] = qvx[q]; a.dvy[p] = qvy[q]; a.dvz[p] = qvz[q];
+                            a.dcell[p] = cA;
+                        }
                     }
+                    if (DEF > 32 && q0 + 32 >= ndef) break;
                 }
                 ndef = 0;
             }
@@ -694,7 +700,10 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
                 const int rdef = __shfl_sync(FULL, st_q, lastq) >> 5;            // first row that can hold it
                 const int psRlast = __shfl_sync(FULL, psR, lastq);               // R particles of the tile before that cell
                 const int nRlast = __shfl_sync(FULL, Rc, lastq);                 // its right-movers: deferred to the next tile
-                if (nRlast > FUSED_DEF) bad |= FA_DEFER_OVERFLOW;
+                if (nRlast > DEF) { // the host learns how many there were and takes the larger queue when it comes back
+                    bad |= FA_DEFER_OVERFLOW;
+                    if (lane == 0) atomicMax(&st->maxdef, nRlast);
+                }
 #pragma unroll
                 for (int gi = 0; gi < fused_ngroups(RMAX); ++gi) {
                     if (fused_group_start(RMAX, gi) < nrows) {
@@ -710,7 +719,7 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
                             }
                             if (r >= rdef && key == kdef) { // its rank inside the class is its place in the queue
                                 const int q = (pk >> 8) - psRlast;
-                                if (q < FUSED_DEF) {
+                                if (q < DEF) {
                                     qx[q] = X_[r]; qvx[q] = VX_[r]; qvy[q] = VY_[r]; qvz[q] = VZ_[r];
                                     qpos[q] = p;
                                 }
@@ -718,7 +727,7 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
                         }
                     }
                 }
-                ndef = min(nRlast, FUSED_DEF);
+                ndef = min(nRlast, DEF);
             }
             // carry: this tile's last cell
             if (kind != FK_VIRTUAL) {

@@ -55,6 +55,7 @@ struct pic_species {
     // fused push+arrange step (fused.cuh)
     double2 *d_cs = nullptr;           // deposition: per-cell partial sums (allocated at the first pic_deposit)
     int h_maxcount = 0;                // bound of the largest per-cell count last seen by the host (sizes the fused tiles)
+    int h_maxdef = 0;                  // most right-movers of one cell deferred to the next tile, last seen (sizes their queue)
     // asynchronous telemetry of the fused path: every few fused steps the device state is copied to pinned host
     // memory without waiting; push_fused reads the latest copy that has landed (the largest per-cell count drifts
     // over a long pic_push without any synchronising call, and a cell that outgrows the tile declines the step)
@@ -268,14 +269,25 @@ static long long host_step_bound(pic_species *s)
 }
 
 // The instance of fused_kernel for a launch geometry.
-static void (*fused_pick(int rows, bool periodic, bool bz0, bool tma))(FusedArgs)
+template <int R, int D>
+static void (*fused_pick_rd(bool periodic, bool bz0, bool tma))(FusedArgs)
 {
-#define PIC_FK(R) (periodic ? (bz0 ? (tma ? fused_kernel<R, true, true, true> : fused_kernel<R, true, true, false>)      \
-                                   : (tma ? fused_kernel<R, true, false, true> : fused_kernel<R, true, false, false>))   \
-                            : (bz0 ? (tma ? fused_kernel<R, false, true, true> : fused_kernel<R, false, true, false>)    \
-                                   : (tma ? fused_kernel<R, false, false, true> : fused_kernel<R, false, false, false>)))
-    return rows == 8 ? PIC_FK(8) : rows == 12 ? PIC_FK(12) : PIC_FK(16);
-#undef PIC_FK
+    if (D != FUSED_DEF) // the large queue exists for the TMA kernels only
+        return periodic ? (bz0 ? fused_kernel<R, true, true, true, D> : fused_kernel<R, true, false, true, D>)
+                        : (bz0 ? fused_kernel<R, false, true, true, D> : fused_kernel<R, false, false, true, D>);
+    return periodic ? (bz0 ? (tma ? fused_kernel<R, true, true, true, FUSED_DEF> : fused_kernel<R, true, true, false, FUSED_DEF>)
+                           : (tma ? fused_kernel<R, true, false, true, FUSED_DEF> : fused_kernel<R, true, false, false, FUSED_DEF>))
+                    : (bz0 ? (tma ? fused_kernel<R, false, true, true, FUSED_DEF> : fused_kernel<R, false, true, false, FUSED_DEF>)
+                           : (tma ? fused_kernel<R, false, false, true, FUSED_DEF> : fused_kernel<R, false, false, false, FUSED_DEF>));
+}
+
+static void (*fused_pick(int rows, bool periodic, bool bz0, bool tma, int def))(FusedArgs)
+{
+    if (def != FUSED_DEF)
+        return rows == 8 ? fused_pick_rd<8, FUSED_DEF_BIG>(periodic, bz0, tma)
+             : rows == 12 ? fused_pick_rd<12, FUSED_DEF_BIG>(periodic, bz0, tma) : fused_pick_rd<16, FUSED_DEF_BIG>(periodic, bz0, tma);
+    return rows == 8 ? fused_pick_rd<8, FUSED_DEF>(periodic, bz0, tma)
+         : rows == 12 ? fused_pick_rd<12, FUSED_DEF>(periodic, bz0, tma) : fused_pick_rd<16, FUSED_DEF>(periodic, bz0, tma);
 }
 
 // The fused kernels need more dynamic shared memory than the default limit: raise it once per DEVICE (the attribute
@@ -288,7 +300,9 @@ static int fused_set_attributes(int device)
     for (int rows : {8, 12, 16})
         for (int per = 0; per < 2; ++per)
             for (int bz0 = 0; bz0 < 2; ++bz0)
-                for (int tma = 0; tma < 2; ++tma) kerns.push_back(fused_pick(rows, per != 0, bz0 != 0, tma != 0));
+                for (int tma = 0; tma < 2; ++tma)
+                    for (int def : {FUSED_DEF, FUSED_DEF_BIG})
+                        if (tma || def == FUSED_DEF) kerns.push_back(fused_pick(rows, per != 0, bz0 != 0, tma != 0, def));
     for (auto kfn : kerns) CU(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
     CU(cudaFuncSetAttribute(tile_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TS_SMEM_BYTES));
     if (device >= 0 && device < 64) done[device] = true;
@@ -756,30 +770,30 @@ static int push_split(pic_species *s, bool will_arrange)
     return PIC_OK;
 }
 
-struct FusedGeom { int rows, slots, stages, cpc, ctas_per_sm; size_t smem; };
+struct FusedGeom { int rows, slots, stages, cpc, ctas_per_sm, def; size_t smem; };
 
 // CTAs of fused_kernel<rows> an SM holds: registers (launch bounds of the instance) or shared memory.
-static int fused_ctas_per_sm(int rows, int cpc, int stages)
+static int fused_ctas_per_sm(int rows, int cpc, int stages, int def)
 {
     const int by_regs = rows == 8 ? 16 : rows == 12 ? 12 : 8;
-    const int by_smem = FUSED_SMEM_SM / (fused_layout(rows * 32, cpc, stages).total + 1024);
+    const int by_smem = FUSED_SMEM_SM / (fused_layout(rows * 32, cpc, stages, def).total + 1024);
     return std::max(1, std::min(32, std::min(by_regs, by_smem)));
 }
 
 // Cells per CTA.  Every chunk pushes two halo cells on top of its own, and the grid runs in waves of
 // sm_count * ctas_per_sm CTAs: pick the chunk size that wastes least to halo work and a ragged last wave.
-static int fused_cells_per_cta(const pic_species *s, int rows, int stages)
+static int fused_cells_per_cta(const pic_species *s, int rows, int stages, int def)
 {
     const pic_sim *sim = s->sim;
     if (sim->opt_fused_cpc > 0) return sim->opt_fused_cpc;
     int best = FUSED_CPC_DEFAULT;
     {   // many waves: the ragged last wave is noise, keep the measured optimum
-        const double resident = (double)sim->sm_count * fused_ctas_per_sm(rows, best, stages);
+        const double resident = (double)sim->sm_count * fused_ctas_per_sm(rows, best, stages, def);
         if ((double)((sim->nc + best - 1) / best) >= 4.0 * resident) return best;
     }
     double best_score = -1.0;
     for (int cpc = 2; cpc <= FUSED_CPC_SEARCH; ++cpc) {
-        const double resident = (double)sim->sm_count * fused_ctas_per_sm(rows, cpc, stages);
+        const double resident = (double)sim->sm_count * fused_ctas_per_sm(rows, cpc, stages, def);
         const double chunks = (double)((sim->nc + cpc - 1) / cpc);
         const double score = chunks / (std::ceil(chunks / resident) * resident) * cpc / (cpc + 2.0);
         if (score > best_score * 1.0001) { best_score = score; best = cpc; }
@@ -808,10 +822,13 @@ static FusedGeom fused_geom(const pic_species *s)
     // two stages under the 8-row tiles (11 CTAs of 19.7 KB per SM: measured 3-7 % faster than one stage at 16 CTAs);
     // the wider tiles keep one stage (a second one would halve their CTAs per SM: measured slower)
     g.stages = !sim->opt_fused_tma ? 0 : (sim->opt_fused_stages ? sim->opt_fused_stages : (g.rows == 8 ? 2 : 1));
-    g.cpc = fused_cells_per_cta(s, g.rows, g.stages);
+    // queue of the right-movers that wait for the next tile: the usual one until a step has overflowed it
+    g.def = s->h_maxdef > FUSED_DEF ? FUSED_DEF_BIG : FUSED_DEF;
+    if (!sim->opt_fused_tma) g.def = FUSED_DEF; // the plain-load A/B variant exists with the usual queue only
+    g.cpc = fused_cells_per_cta(s, g.rows, g.stages, g.def);
     g.slots = sim->opt_fused_slots ? std::min(sim->opt_fused_slots, g.rows * 32) : g.rows * 32;
-    g.smem = (size_t)fused_layout(g.rows * 32, g.cpc, g.stages).total;
-    g.ctas_per_sm = fused_ctas_per_sm(g.rows, g.cpc, g.stages);
+    g.smem = (size_t)fused_layout(g.rows * 32, g.cpc, g.stages, g.def).total;
+    g.ctas_per_sm = fused_ctas_per_sm(g.rows, g.cpc, g.stages, g.def);
     return g;
 }
 
@@ -855,6 +872,16 @@ static int push_fused(pic_species *s)
     a.CPC = geo.cpc;
     a.SCAP = geo.slots;
     a.NST = geo.stages;
+    {   // PIC_TRACE: report the launch geometry whenever it changes
+        static const bool trace = getenv("PIC_TRACE") != nullptr;
+        static int last[6] = {-1, -1, -1, -1, -1, -1};
+        const int now[6] = {geo.rows, geo.cpc, geo.stages, geo.def, geo.ctas_per_sm, (int)geo.smem};
+        if (trace && memcmp(last, now, sizeof now)) {
+            memcpy(last, now, sizeof now);
+            fprintf(stderr, "[pic fused] step %lld: rows %d, cells/CTA %d, stages %d, queue %d, CTAs/SM %d, smem %d B (maxcount %d, maxdef %d)\n",
+                    s->steps, geo.rows, geo.cpc, geo.stages, geo.def, geo.ctas_per_sm, (int)geo.smem, s->h_maxcount, s->h_maxdef);
+        }
+    }
     a.step_id = (int)(s->steps & 0x7fffffff);
     const int rows = geo.rows;
     const int nchunks = (sim->nc + a.CPC - 1) / a.CPC;
@@ -872,7 +899,7 @@ static int push_fused(pic_species *s)
         fused_edge_kernel<<<1, 128, 0, sim->stream>>>(a);
         if (int rc = launch_check(sim, "fused_edge_kernel")) return rc;
         const bool bz0 = s->k.tz == 0.0 && s->k.sz == 0.0; // B in the x-y plane: the kernel drops the exact-zero products
-        void (*kern)(FusedArgs) = fused_pick(rows, sim->periodic != 0, bz0, sim->opt_fused_tma != 0);
+        void (*kern)(FusedArgs) = fused_pick(rows, sim->periodic != 0, bz0, sim->opt_fused_tma != 0, geo.def);
         if (sim->opt_fused_pdl) {
             // programmatic dependent launch: the CTAs start while fused_edge_kernel is still running and do their
             // prologue (offsets, E window, first bulk copies); griddepcontrol.wait holds them before anything else
@@ -944,6 +971,7 @@ static int verify_fused(pic_species *s)
     s->h_steps_since_sync = 0;
     s->h_kick_acc = 0;
     s->h_maxcount = h.maxcount;
+    s->h_maxdef = std::max(s->h_maxdef, h.maxdef);
     for (long long left = run - k; left > 0;) {
         const int chunk = (int)std::min<long long>(left, 1 << 20);
         if (int rc = pic_push(s, chunk)) return rc;
@@ -997,11 +1025,12 @@ static int read_state(pic_species *s, DevState &h)
     }
     if (h.fused_disabled) s->fused_off = true;
     s->h_maxcount = h.maxcount;
+    s->h_maxdef = std::max(s->h_maxdef, h.maxdef);
     s->h_abort_reason = h.abort_reason;
     // A declined fused path comes back once the cause is gone: the state is arranged, the split mover's last
     // step moved no particle by more than one cell, and some steps have passed since the decline.
     if (s->fused_off && s->arrange_every == 1 && s->counts_fresh && h.w_acc <= 1 && h.status == 0 &&
-        s->steps - s->declined_at >= FUSED_RETRY_STEPS && !(h.abort_reason & (FA_DEFER_OVERFLOW | FA_EDGE_OVERFLOW))) {
+        s->steps - s->declined_at >= FUSED_RETRY_STEPS && !(h.abort_reason & FA_EDGE_OVERFLOW) && s->h_maxdef <= FUSED_DEF_BIG) {
         const int zero = 0;
         CU(cudaMemcpyAsync(&s->d_st->fused_disabled, &zero, sizeof zero, cudaMemcpyHostToDevice, s->sim->stream));
         CU(cudaStreamSynchronize(s->sim->stream));

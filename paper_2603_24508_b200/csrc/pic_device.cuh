@@ -39,6 +39,7 @@ struct DevState {
     int f_OL, f_AR;                  // fused step in flight: leavers of cell 0 downwards / wrapped arrivals in cell 0
     int ntiles, ntiles_next;         // tiles of the current partition (fused.cuh) / of the one being written
     int maxcount, maxcount_next;     // upper bound of the largest per-cell count: current state / step in flight
+    int maxdef;                      // fused step: most right-movers of one cell that overflowed the deferred queue (0: never)
     int fail_step;                   // step id (FusedArgs::step_id) of the first fused step that declined
     int tile_declined;               // tilesort.cuh: a tile's window was too wide; scatter_fast_kernel takes the arrange
 };

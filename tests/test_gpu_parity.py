@@ -604,3 +604,34 @@ def test_no_write_beyond_the_initial_slot_count(options, config, kw, steps):
                 assert bool((t[n0:] == sent_f).all()), "a kernel wrote beyond the initial slot count"
             assert bool((sp.bufs[b][4][n0:] == sent_i).all()), "a kernel wrote beyond the initial slot count (cell)"
     pic.pic_destroy(sim)
+
+
+def test_fused_queue_of_deferred_right_movers_grows_with_the_flow():
+    """A beam drifting at 3 cells per 10 steps on top of v_th = 1: about a third of every cell's particles move right
+    each step, more than the 32 the smallest queue of deferred right-movers holds.  The first fused step declines
+    (reason 4), the split kernels carry on, and once the host has seen the device's count the fused step comes back
+    with a larger queue -- results bit-identical throughout."""
+    inp = workloads.make(2, nc=1024)
+    s = inp["species"][0]
+    s["vx"] = s["vx"] + 3.0
+    inp["B"] = np.array([2.0, 0.0, 0.0])  # B along x: the drift is not rotated away
+    sim, (st,) = make_pair(inp, options={"fused": 1, "kernel_timing": 1})
+    sp = sim.species[0]
+    pic.pic_push(sp, 1)
+    st.push(1)
+    compare(sp, st, where="first step", counts=True, nc=inp["nc"])
+    info = pic.pic_fused_info(sp)
+    assert info["decline_reasons"] & 4 and info["active"] == 0, info
+    for k in range(18):
+        pic.pic_push(sp, 1)
+        st.push(1)
+    compare(sp, st, where="after the split steps", counts=True, nc=inp["nc"])
+    info = pic.pic_fused_info(sp)
+    assert info["active"] == 1, info
+    pic.pic_kernel_time(sim, "fused")
+    pic.pic_kernel_time(sim, "mover")
+    pic.pic_push(sp, 25)
+    st.push(25)
+    compare(sp, st, where="fused again with a larger queue", counts=True, nc=inp["nc"])
+    assert pic.pic_kernel_time(sim, "fused")[1] == 25 and pic.pic_kernel_time(sim, "mover")[1] == 0
+    assert pic.pic_fused_info(sp)["active"] == 1
