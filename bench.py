@@ -478,22 +478,33 @@ def main():
                 h2d += t.numel() * t.element_size()
             host_species.append(dict(qm=s["qm"], arrays=arrs, arrange_every=ae))
         h2d += inp["E"].nbytes
-        torch.cuda.synchronize()
-        if dist is not None:
-            dist.barrier()
-        t0 = time.perf_counter()
-        res = pic.pic_run_host(nc=inp["nc"], dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E_nodes=inp["E"],
-                               B=inp["B"], species=host_species, nsteps=cfg_steps, stream=stream)
-        torch.cuda.synchronize()
-        t_e2e = time.perf_counter() - t0
+        # three calls from the same pinned buffers (refilled outside the timed region: the call overwrites them with
+        # the final state); the median is reported, all three are listed -- the first call of a process also pays the
+        # one-off module load and allocator warm-up, and PCIe rates on a shared host vary from call to call
+        samples = []
+        for rep in range(3):
+            if rep:
+                for hs_, s in zip(host_species, inp["species"]):
+                    for t, k in zip(hs_["arrays"], ("x", "vx", "vy", "vz", "cell")):
+                        t.copy_(torch.from_numpy(s[k]))
+            torch.cuda.synchronize()
+            if dist is not None:
+                dist.barrier()
+            t0 = time.perf_counter()
+            res = pic.pic_run_host(nc=inp["nc"], dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E_nodes=inp["E"],
+                                   B=inp["B"], species=host_species, nsteps=cfg_steps, stream=stream)
+            torch.cuda.synchronize()
+            samples.append(time.perf_counter() - t0)
+        t_e2e = statistics.median(samples)
         n_out = sum(r[0] for r in res)
         d2h = n_out * 36 + 16 * len(res)
         n0_e = sum(len(s["x"]) for s in inp["species"])
         e_pushes = 0.5 * (n0_e + n_out) * cfg_steps
         t_e2e, e_pushes = aggregate_over_ranks(dist, t_e2e, e_pushes, dev)
         e2e = {"value": e_pushes / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d / cfg_steps,
-               "d2h_bytes_per_step": d2h / cfg_steps, "steps": cfg_steps, "seconds": t_e2e,
-               "call": "pic_run_host (pinned host SoA in, cudaMalloc + H2D + pic_create + pic_push(nsteps) + D2H + free inside)"}
+               "d2h_bytes_per_step": d2h / cfg_steps, "steps": cfg_steps, "seconds": t_e2e, "seconds_all_calls": samples,
+               "call": "pic_run_host (pinned host SoA in; one device arena + H2D + pic_create + pic_push(nsteps) + D2H + free "
+                       "inside; median of 3 calls)"}
         del host_species
 
     cpu = None

@@ -148,22 +148,39 @@ __global__ void __launch_bounds__(FLD_THREADS) field_sum_kernel(FieldArgs a)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (lane == 0) s_w[warp] = v;
     __syncthreads();
+    __shared__ int s_last;
     if (threadIdx.x == 0) {
         FieldDD r{0.0, 0.0};
         for (int w = 0; w < FLD_THREADS / 32; ++w) r = fld_dd_add(r, s_w[w]);
         a.tile_sum[blockIdx.x] = r.hi;
         a.tile_lo[blockIdx.x] = r.lo;
         __threadfence();
-        if (atomicAdd(a.ticket, 1u) == gridDim.x - 1) { // the last tile to arrive adds the tile sums, in tile order
-            __threadfence();
-            FieldDD sum{0.0, 0.0};
-            for (int t = 0; t < a.ntiles; ++t)
-                sum = fld_dd_add(sum, FieldDD{((volatile double *)a.tile_sum)[t], ((volatile double *)a.tile_lo)[t]});
+        s_last = atomicAdd(a.ticket, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (s_last) { // the last tile to arrive adds the tile sums: every thread a fixed subset, then a fixed tree
+        __threadfence();
+        FieldDD sum{0.0, 0.0};
+        for (int t = threadIdx.x; t < a.ntiles; t += FLD_THREADS)
+            sum = fld_dd_add(sum, FieldDD{((volatile double *)a.tile_sum)[t], ((volatile double *)a.tile_lo)[t]});
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            FieldDD u;
+            u.hi = __shfl_down_sync(FULL, sum.hi, o);
+            u.lo = __shfl_down_sync(FULL, sum.lo, o);
+            sum = fld_dd_add(sum, u);
+        }
+        __syncthreads();
+        if (lane == 0) s_w[warp] = sum;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            FieldDD tot{0.0, 0.0};
+            for (int w = 0; w < FLD_THREADS / 32; ++w) tot = fld_dd_add(tot, s_w[w]);
             const double n = (double)a.nc;
-            const double q = sum.hi / n;
-            const double rem = __fma_rn(-q, n, sum.hi); // exact remainder of the division
+            const double q = tot.hi / n;
+            const double rem = __fma_rn(-q, n, tot.hi); // exact remainder of the division
             a.scal[0] = q;
-            a.scal[3] = __dadd_rn(rem, sum.lo) / n;
+            a.scal[3] = __dadd_rn(rem, tot.lo) / n;
             *a.ticket = 0u;
         }
     }
@@ -300,14 +317,20 @@ __global__ void __launch_bounds__(FLD_THREADS) field_phi_kernel(FieldArgs a)
         T += S;
     }
     psum = fld_block_sum(psum, s_sum);
+    __shared__ int s_last;
     if (threadIdx.x == 0) {
         a.tile_sum[blockIdx.x] = psum;
         __threadfence();
-        if (atomicAdd(a.ticket + 1, 1u) == gridDim.x - 1) { // last tile: the mean of phi (the gauge of a periodic grid)
-            __threadfence();
-            double sum = 0.0;
-            if (a.periodic)
-                for (int t = 0; t < a.ntiles; ++t) sum += ((volatile double *)a.tile_sum)[t];
+        s_last = atomicAdd(a.ticket + 1, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (s_last) { // last tile: the mean of phi (the gauge of a periodic grid), by a fixed tree over the tile sums
+        __threadfence();
+        double sum = 0.0;
+        if (a.periodic)
+            for (int t = threadIdx.x; t < a.ntiles; t += FLD_THREADS) sum += ((volatile double *)a.tile_sum)[t];
+        sum = fld_block_sum(sum, s_sum);
+        if (threadIdx.x == 0) {
             a.scal[2] = sum / (double)a.nc;
             a.ticket[1] = 0u;
         }
