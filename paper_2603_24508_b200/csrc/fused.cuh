@@ -28,6 +28,10 @@
 // moving two cells, a cell larger than a tile) declines the whole step: the source buffers are
 // untouched, the step's id is recorded, later fused launches exit at once, and the host redoes
 // the declined steps with the split kernels (mover / scan / scatter) at its next synchronising call.
+// A step is three launches: fused_edge_kernel, fused_kernel (programmatic dependent launch: its prologue overlaps
+// the edge kernel, griddepcontrol.wait holds it before it reads OL / AR or writes anything), fused_commit_kernel
+// (one thread: commits n, the wall counters and the bounds, or records the decline; no fence or arrival counter
+// in the streaming kernel).
 #pragma once
 #include "pic_device.cuh"
 
