@@ -229,6 +229,46 @@ def test_run_host_end_to_end():
         assert np.array_equal(a[:n_out], o)
 
 
+@pytest.mark.parametrize("config,kw,steps,pinned", [(3, dict(nc=1500), 25, True), (5, dict(nc=2048), 23, False)])
+def test_run_host_two_species_and_pinned_buffers(config, kw, steps, pinned):
+    """pic_run_host with several species in one call (one device arena, D2H on a second stream), pinned torch
+    buffers or plain numpy arrays; config 5 ends between two arranges, so flagged-dead particles come back in place;
+    and the binding refuses arrays it cannot hand to the C side."""
+    import torch
+    inp = workloads.make(config, **kw)
+    ae = inp["arrange_every"]
+    species, states = [], []
+    for s in inp["species"]:
+        st = oracle.State(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], nc=inp["nc"], dx=inp["dx"], dt=inp["dt"],
+                          boundary=inp["boundary"], E=inp["E"], qm=s["qm"], B=inp["B"], arrange_every=ae)
+        st.push(steps)
+        states.append(st)
+        arrs = [np.array(s[k]) for k in ("x", "vx", "vy", "vz", "cell")]
+        if pinned:
+            arrs = [torch.from_numpy(a).pin_memory() for a in arrs]
+        species.append(dict(qm=s["qm"], arrays=arrs, arrange_every=ae))
+    if config == 5:  # a second species of the same shape, so that both kinds of state come back from one call
+        species.append(dict(qm=species[0]["qm"], arrays=[np.array(inp["species"][0][k]) for k in ("x", "vx", "vy", "vz", "cell")],
+                            arrange_every=ae))
+        states.append(states[0])
+    res = pic.pic_run_host(nc=inp["nc"], dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E_nodes=inp["E"], B=inp["B"],
+                           species=species, nsteps=steps)
+    for (n_out, wl, wr), sp, st in zip(res, species, states):
+        assert n_out == st.n and (wl, wr) == (int(st.wall[0]), int(st.wall[1]))
+        for a, o in zip(sp["arrays"], st.live()):
+            a = a.numpy() if hasattr(a, "numpy") else a
+            assert np.array_equal(a[:n_out], o)
+    bad = [np.array(inp["species"][0][k]) for k in ("x", "vx", "vy", "vz", "cell")]
+    bad[1] = bad[1].astype(np.float32)
+    with pytest.raises(ValueError):
+        pic.pic_run_host(nc=inp["nc"], dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E_nodes=inp["E"], B=inp["B"],
+                         species=[dict(qm=-1.0, arrays=bad, arrange_every=ae)], nsteps=1)
+    bad[1] = bad[1].astype(np.float64)[:-1]
+    with pytest.raises(ValueError):
+        pic.pic_run_host(nc=inp["nc"], dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E_nodes=inp["E"], B=inp["B"],
+                         species=[dict(qm=-1.0, arrays=bad, arrange_every=ae)], nsteps=1)
+
+
 @pytest.mark.parametrize("config,kw,steps", [(1, {}, 40), (2, dict(nc=2048), 40), (3, dict(nc=1000), 30),
                                              (4, dict(nc=4099), 30)])
 def test_fused_step_is_the_one_that_runs(config, kw, steps):
