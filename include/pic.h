@@ -212,13 +212,14 @@ size_t pic_workspace_bytes(int32_t nc, int64_t capacity);
  * scatter kernels (E through the read-only global path); "fused_tma": 1 = the fused step stages particles and E by TMA bulk copies (default),
  * 0 = it reads them with plain read-only global loads (the A/B variant of profiles/); "kernel_timing": 1 = record CUDA events
  * around every kernel launch (see pic_kernel_time).  Knobs of the fused step:
- * "fused_cells_per_cta" (cells per chunk, 1..256; 0 = automatic: 32 on large grids), "fused_rows" (rows
+ * "fused_cells_per_cta" (cells per chunk, 1..256; 0 = automatic), "fused_rows" (rows
  * of 32 slots per tile: 8, 12 or 16; 0 = automatic from the largest per-cell count),
  * "fused_stage_slots" (largest tile in slots, even, <= 32*rows; 0 = 32*rows), "fused_stages"
  * (stages of the TMA ring: 1 or 2; 0 = automatic: 2 under 8-row tiles, else 1), "fused_pdl" (1 = the streaming
  * kernel is launched with programmatic dependent launch and overlaps its prologue with the edge kernel, default;
- * 0 = plain stream order), "fused_columns" (1 = consecutive chunks are handed to the same slot of the machine one after
- * the other so that shared halo cells are read back to back; 0 = chunk = block index, default: measured 0.7 % faster).  Results never depend on any of them.
+ * 0 = plain stream order), "fused_taper" (0..3: how many times the chunk size is halved towards the end of the grid, one
+ * machine-load of CTAs per size, so that the CTAs that run last are short; -1 = automatic, default: 64-cell chunks
+ * tapered three times on grids of four or more waves, no taper on smaller ones).  Results never depend on any of them.
  * PIC_EINVAL for an unknown key or a value out of range. */
 int pic_set_option(pic_sim *sim, const char *key, int value);
 

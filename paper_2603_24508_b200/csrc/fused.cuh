@@ -41,6 +41,8 @@ constexpr int FUSED_MIN_NC = 16;
 constexpr int FUSED_CPC_DEFAULT = 32;  // cells per chunk (per CTA) on grids of many waves (measured optimum at config 4)
 constexpr int FUSED_CPC_SEARCH = 64;   // largest chunk the per-launch search considers on smaller grids
 constexpr int FUSED_CPC_MAX = 256;
+constexpr int FUSED_CPC_TAPER = 64;    // chunk size of the bulk of a many-wave grid under the tapered schedule
+constexpr int FUSED_SEGS = 4;          // segments of the chunk schedule (chunk sizes CPC, CPC/2, CPC/4, CPC/8)
 constexpr int FUSED_KMAX = 31;         // cells per tile (one lane per cell border)
 constexpr int FUSED_DEF = 32;          // deferred right-movers of a tile's last cell: the usual queue ...
 constexpr int FUSED_DEF_BIG = 128;     // ... and the one taken after a step has overflowed it (strongly drifting flows)
@@ -68,7 +70,10 @@ struct FusedArgs {
     int SCAP; // largest tile, in slots (<= RMAX*32, even)
     int NST;  // stages of the ring: 1 or 2
     int step_id; // low 31 bits of the species' step counter before this step
-    int COLS, RUN; // chunk of CTA b = (b % COLS) * RUN + b / COLS: COLS = CTAs resident at once, RUN = ceil(chunks / COLS)
+    // Chunk schedule: CTAs seg_blk[s] .. seg_blk[s+1]-1 own seg_cpc[s] cells each, starting at cell seg_cell[s]
+    // (seg_cell[nseg] = nc, unused seg_blk = INT_MAX).  Large chunks first (little halo work), then ever smaller ones
+    // so that the CTAs that run last are short and every SM runs dry at about the same time (pic.cu: fused_schedule).
+    int seg_blk[FUSED_SEGS], seg_cell[FUSED_SEGS + 1], seg_cpc[FUSED_SEGS];
 };
 
 // Dynamic shared memory of one fused_kernel CTA (one warp): NST stages of CAP = RMAX*32 slots.
@@ -414,8 +419,30 @@ __device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *
     }
 }
 
-// Row groups of sweep 1a: four rows at a time while at least four remain likely, then two, then single rows,
-// so that a tile of nrows rows pushes at most one surplus row.
+// Row groups of the sweeps.  Width 0: rows 4 by 4 while at least four more can follow, then 2, 1, 1 (for RMAX = 8:
+// {0-3} {4,5} {6} {7}; a tile pushes at most one surplus row).  Width W > 0: groups of W rows ({0-3} {4-7}).  A group
+// runs if its first row is inside the tile; rows of it behind the tile are masked out (class X, nothing stored), so
+// that a group is straight-line code whose rows' dependency chains interleave.  The kernel is bound by the latency of
+// these chains, not by issue slots: fewer, wider groups win although they push more surplus rows.
+#ifndef FUSED_W1A
+#define FUSED_W1A 0 // sweep 1a (and the loads)
+#endif
+#ifndef FUSED_W1B
+#define FUSED_W1B 0 // sweep 1b
+#endif
+#ifndef FUSED_W2
+#define FUSED_W2 0  // sweep 2
+#endif
+__host__ __device__ constexpr int fused_ngroups(int rmax, int w) { return w ? (rmax + w - 1) / w : rmax / 4 + 2; }
+__host__ __device__ constexpr int fused_group_start(int rmax, int w, int gi)
+{
+    return w ? w * gi : (gi < rmax / 4 - 1 ? 4 * gi : 4 * (rmax / 4 - 1) + (gi == rmax / 4 - 1 ? 0 : (gi == rmax / 4 ? 2 : 3)));
+}
+__host__ __device__ constexpr int fused_group_count(int rmax, int w, int gi)
+{
+    return w ? (w * gi + w <= rmax ? w : rmax - w * gi) : (gi < rmax / 4 - 1 ? 4 : (gi == rmax / 4 - 1 ? 2 : 1));
+}
+
 // The tile's x, vx, vy, vz from the stage (or, without TMA, from global memory) into the register tile, by the same
 // row groups as the sweeps.  Done for the whole tile BEFORE the arithmetic, so that the stage is free again at once
 // and the next tile's bulk copies are in flight during all of this tile's work.
@@ -425,9 +452,8 @@ __device__ __forceinline__ void fused_load_rows(const double *p0, const double *
                                                 double (&VY_)[RMAX], double (&VZ_)[RMAX])
 {
 #pragma unroll
-    for (int gi = 0; gi < RMAX / 4 + 2; ++gi) {
-        const int g0 = gi < RMAX / 4 - 1 ? 4 * gi : 4 * (RMAX / 4 - 1) + (gi == RMAX / 4 - 1 ? 0 : (gi == RMAX / 4 ? 2 : 3));
-        const int gn = gi < RMAX / 4 - 1 ? 4 : (gi == RMAX / 4 - 1 ? 2 : 1);
+    for (int gi = 0; gi < fused_ngroups(RMAX, FUSED_W1A); ++gi) {
+        const int g0 = fused_group_start(RMAX, FUSED_W1A, gi), gn = fused_group_count(RMAX, FUSED_W1A, gi);
         if (g0 < nrows) {
 #pragma unroll
             for (int r = g0; r < g0 + gn; ++r) {
@@ -448,28 +474,13 @@ __device__ __forceinline__ void fused_sweep1a_all(const PushConst &k, const doub
                                                   int pad, int n, int nrows, int cA, int ncell, double (&X_)[RMAX], double (&VX_)[RMAX],
                                                   double (&VY_)[RMAX], double (&VZ_)[RMAX], int (&W_)[RMAX])
 {
-#define FUSED_ROWS(R0, CNT) \
-    if (R0 < nrows) fused_sweep1a<PERIODIC, EDGE, BZ0, TMA, RMAX, R0, CNT>(k, pE, cellinfo, lane, pad, n, cA, ncell, X_, VX_, VY_, VZ_, W_);
-    FUSED_ROWS(0, 4)
-    if (RMAX == 8) {
-        FUSED_ROWS(4, 2) FUSED_ROWS(6, 1) FUSED_ROWS(7, 1)
-    } else if (RMAX == 12) {
-        FUSED_ROWS(4, 4) FUSED_ROWS(8, 2) FUSED_ROWS(10, 1) FUSED_ROWS(11, 1)
-    } else {
-        FUSED_ROWS(4, 4) FUSED_ROWS(8, 4) FUSED_ROWS(12, 2) FUSED_ROWS(14, 1) FUSED_ROWS(15, 1)
-    }
+#define FUSED_ROWS(GI) \
+    if constexpr (GI < fused_ngroups(RMAX, FUSED_W1A)) if (fused_group_start(RMAX, FUSED_W1A, GI) < nrows) \
+        fused_sweep1a<PERIODIC, EDGE, BZ0, TMA, RMAX, fused_group_start(RMAX, FUSED_W1A, GI), fused_group_count(RMAX, FUSED_W1A, GI)>( \
+            k, pE, cellinfo, lane, pad, n, cA, ncell, X_, VX_, VY_, VZ_, W_);
+    FUSED_ROWS(0) FUSED_ROWS(1) FUSED_ROWS(2) FUSED_ROWS(3) FUSED_ROWS(4) FUSED_ROWS(5)
 #undef FUSED_ROWS
 }
-
-// Row groups shared by the three sweeps: rows 4 by 4 while at least four more can follow, then 2, 1, 1 (for RMAX = 8:
-// {0-3} {4,5} {6} {7}).  A group runs if its first row is inside the tile; rows of it behind the tile are masked
-// out (class X, nothing stored), so that a group is straight-line code whose rows interleave.
-__host__ __device__ constexpr int fused_ngroups(int rmax) { return rmax / 4 + 2; }
-__host__ __device__ constexpr int fused_group_start(int rmax, int gi)
-{
-    return gi < rmax / 4 - 1 ? 4 * gi : 4 * (rmax / 4 - 1) + (gi == rmax / 4 - 1 ? 0 : (gi == rmax / 4 ? 2 : 3));
-}
-__host__ __device__ constexpr int fused_group_count(int rmax, int gi) { return gi < rmax / 4 - 1 ? 4 : (gi == rmax / 4 - 1 ? 2 : 1); }
 
 // TMA = true: particles and the chunk's E window are staged in shared memory by bulk copies (cp.async.bulk + mbarrier).
 // TMA = false (option "fused_tma" = 0, the A/B variant of profiles/): plain read-only global loads into the same
@@ -497,14 +508,15 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
     int bad = 0;  // FA_* bits
     int mc = 0;   // largest new per-cell count seen by this lane
 
-    // CTAs are dispatched in blockIdx order and a new one starts when an old one ends, so slot (b % COLS) of the
-    // machine works through chunks RUN*slot, RUN*slot + 1, ... one after the other: the halo cell a chunk shares with
-    // its neighbour is read by the two CTAs back to back (option "fused_columns"; COLS = number of chunks: chunk = b).
-    const int chunk = ((int)blockIdx.x % a.COLS) * a.RUN + (int)blockIdx.x / a.COLS;
-    if ((long long)chunk * a.CPC < nc) { // else: a spare CTA of the last columns
+    // CTAs are dispatched in blockIdx order: the schedule's large chunks run first, its small ones last.
+    int sg_blk = 0, sg_cell = 0, sg_cpc = a.seg_cpc[0], sg_end = a.seg_cell[1];
+#pragma unroll
+    for (int sg = 1; sg < FUSED_SEGS; ++sg)
+        if ((int)blockIdx.x >= a.seg_blk[sg]) { sg_blk = a.seg_blk[sg]; sg_cell = a.seg_cell[sg]; sg_cpc = a.seg_cpc[sg]; sg_end = a.seg_cell[sg + 1]; }
+    {
         FusedCtx X;
-        X.C0 = chunk * a.CPC;
-        X.C1 = min(X.C0 + a.CPC, nc);
+        X.C0 = sg_cell + ((int)blockIdx.x - sg_blk) * sg_cpc;
+        X.C1 = min(X.C0 + sg_cpc, sg_end);
         X.Cm = max(X.C0 - 1, 0);
         X.nc = nc;
         X.CAP = a.SCAP;
@@ -606,10 +618,10 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
             int runL = 0, runS = 0, runR = 0; // running class counts of the tile (warp-uniform)
             int wor = 0;
 #pragma unroll
-            for (int gi = 0; gi < fused_ngroups(RMAX); ++gi) {
-                if (fused_group_start(RMAX, gi) < nrows) {
+            for (int gi = 0; gi < fused_ngroups(RMAX, FUSED_W1B); ++gi) {
+                if (fused_group_start(RMAX, FUSED_W1B, gi) < nrows) {
 #pragma unroll
-                    for (int r = fused_group_start(RMAX, gi); r < fused_group_start(RMAX, gi) + fused_group_count(RMAX, gi); ++r) {
+                    for (int r = fused_group_start(RMAX, FUSED_W1B, gi); r < fused_group_start(RMAX, FUSED_W1B, gi) + fused_group_count(RMAX, FUSED_W1B, gi); ++r) {
                         const int w = W_[r];
                         wor |= w;
                         const bool isL = (w & 96) == 0, isS = (w & 96) == 32;
@@ -709,10 +721,10 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
                     if (lane == 0) atomicMax(&st->maxdef, nRlast);
                 }
 #pragma unroll
-                for (int gi = 0; gi < fused_ngroups(RMAX); ++gi) {
-                    if (fused_group_start(RMAX, gi) < nrows) {
+                for (int gi = 0; gi < fused_ngroups(RMAX, FUSED_W2); ++gi) {
+                    if (fused_group_start(RMAX, FUSED_W2, gi) < nrows) {
 #pragma unroll
-                        for (int r = fused_group_start(RMAX, gi); r < fused_group_start(RMAX, gi) + fused_group_count(RMAX, gi); ++r) {
+                        for (int r = fused_group_start(RMAX, FUSED_W2, gi); r < fused_group_start(RMAX, FUSED_W2, gi) + fused_group_count(RMAX, FUSED_W2, gi); ++r) {
                             const int pk = W_[r];
                             const int key = pk & 127;
                             const int2 bd = basd[key];

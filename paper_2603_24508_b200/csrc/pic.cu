@@ -3,6 +3,7 @@
 #include "../../include/pic.h"
 
 #include <chrono>
+#include <climits>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -101,7 +102,7 @@ struct pic_sim {
     int device = 0;
     std::vector<pic_species *> sp;
     unsigned long long launches = 0;
-    int opt_fused = 1, opt_timing = 0, opt_tile_scatter = 1, opt_fused_tma = 1, opt_fused_pdl = 1, opt_fused_cols = 0;
+    int opt_fused = 1, opt_timing = 0, opt_tile_scatter = 1, opt_fused_tma = 1, opt_fused_pdl = 1, opt_fused_taper = -1;
     int opt_fused_cpc = 0, opt_fused_rows = 0, opt_fused_slots = 0, opt_fused_stages = 0; // tuning knobs of the fused step (0 = automatic)
     int sm_count = 148;
     // per-kernel device timing (option "kernel_timing"): event pairs recorded around launches
@@ -595,7 +596,7 @@ extern "C" int pic_set_option(pic_sim *sim, const char *key, int value)
     else if (!strcmp(key, "fused") && flag) sim->opt_fused = value;
     else if (!strcmp(key, "fused_tma") && flag) sim->opt_fused_tma = value;
     else if (!strcmp(key, "fused_pdl") && flag) sim->opt_fused_pdl = value;
-    else if (!strcmp(key, "fused_columns") && flag) sim->opt_fused_cols = value;
+    else if (!strcmp(key, "fused_taper") && value >= -1 && value < FUSED_SEGS) sim->opt_fused_taper = value;
     else if (!strcmp(key, "fused_cells_per_cta") && value >= 0 && value <= FUSED_CPC_MAX) sim->opt_fused_cpc = value;
     else if (!strcmp(key, "fused_stage_slots") && value >= 0 && value <= 512 && value % 2 == 0) sim->opt_fused_slots = value;
     else if (!strcmp(key, "fused_stages") && value >= 0 && value <= 2) sim->opt_fused_stages = value;
@@ -770,7 +771,7 @@ static int push_split(pic_species *s, bool will_arrange)
     return PIC_OK;
 }
 
-struct FusedGeom { int rows, slots, stages, cpc, ctas_per_sm, def; size_t smem; };
+struct FusedGeom { int rows, slots, stages, cpc, ctas_per_sm, def, taper; size_t smem; };
 
 // CTAs of fused_kernel<rows> an SM holds: registers (launch bounds of the instance) or shared memory.
 static int fused_ctas_per_sm(int rows, int cpc, int stages, int def)
@@ -782,14 +783,18 @@ static int fused_ctas_per_sm(int rows, int cpc, int stages, int def)
 
 // Cells per CTA.  Every chunk pushes two halo cells on top of its own, and the grid runs in waves of
 // sm_count * ctas_per_sm CTAs: pick the chunk size that wastes least to halo work and a ragged last wave.
-static int fused_cells_per_cta(const pic_species *s, int rows, int stages, int def)
+static int fused_cells_per_cta(const pic_species *s, int rows, int stages, int def, int *taper)
 {
     const pic_sim *sim = s->sim;
+    *taper = std::max(sim->opt_fused_taper, 0);
     if (sim->opt_fused_cpc > 0) return sim->opt_fused_cpc;
     int best = FUSED_CPC_DEFAULT;
-    {   // many waves: the ragged last wave is noise, keep the measured optimum
+    {   // many waves: large chunks (little halo work), the last waves tapered (fused_schedule)
         const double resident = (double)sim->sm_count * fused_ctas_per_sm(rows, best, stages, def);
-        if ((double)((sim->nc + best - 1) / best) >= 4.0 * resident) return best;
+        if ((double)((sim->nc + best - 1) / best) >= 4.0 * resident) {
+            if (sim->opt_fused_taper < 0) { *taper = FUSED_SEGS - 1; return FUSED_CPC_TAPER; }
+            return best;
+        }
     }
     double best_score = -1.0;
     for (int cpc = 2; cpc <= FUSED_CPC_SEARCH; ++cpc) {
@@ -825,7 +830,7 @@ static FusedGeom fused_geom(const pic_species *s)
     // queue of the right-movers that wait for the next tile: the usual one until a step has overflowed it
     g.def = s->h_maxdef > FUSED_DEF ? FUSED_DEF_BIG : FUSED_DEF;
     if (!sim->opt_fused_tma) g.def = FUSED_DEF; // the plain-load A/B variant exists with the usual queue only
-    g.cpc = fused_cells_per_cta(s, g.rows, g.stages, g.def);
+    g.cpc = fused_cells_per_cta(s, g.rows, g.stages, g.def, &g.taper);
     g.slots = sim->opt_fused_slots ? std::min(sim->opt_fused_slots, g.rows * 32) : g.rows * 32;
     g.smem = (size_t)fused_layout(g.rows * 32, g.cpc, g.stages, g.def).total;
     g.ctas_per_sm = fused_ctas_per_sm(g.rows, g.cpc, g.stages, g.def);
@@ -837,6 +842,40 @@ static int fused_rows(const pic_species *s, int *ctas_per_sm)
     const FusedGeom g = fused_geom(s);
     if (g.rows && ctas_per_sm) *ctas_per_sm = g.ctas_per_sm;
     return g.rows;
+}
+
+// Chunk schedule of one fused launch (FusedArgs::seg_*): the bulk of the grid in chunks of cpc cells, then -- `taper`
+// times -- one machine-load (sm_count * ctas_per_sm CTAs) of chunks half as large as the ones before, the smallest
+// last.  CTAs start in blockIdx order, so the CTAs still running when the grid drains are the short ones: the tail in
+// which SMs idle shrinks with the chunk size while the bulk pays the halo cells of large chunks only.  Returns the grid.
+static int fused_schedule(FusedArgs &a, int nc, int cpc, int taper, int resident)
+{
+    int sizes[FUSED_SEGS], cells[FUSED_SEGS];
+    int nseg = 1, left = nc;
+    sizes[0] = cpc;
+    for (int t = 1; t <= taper && nseg < FUSED_SEGS; ++t) {
+        const int sz = cpc >> t;
+        if (sz < 2) break;
+        sizes[nseg++] = sz;
+    }
+    for (int sg = nseg - 1; sg >= 1; --sg) { // the tail segments take their cells from the end of the grid
+        const long long want = (long long)resident * sizes[sg];
+        cells[sg] = (int)std::min<long long>(want, std::max(0, left - cpc)); // the bulk keeps at least one chunk
+        left -= cells[sg];
+    }
+    cells[0] = left;
+    int blk = 0, cell = 0;
+    for (int sg = 0; sg < FUSED_SEGS; ++sg) {
+        if (sg < nseg && cells[sg] > 0) {
+            a.seg_blk[sg] = blk; a.seg_cell[sg] = cell; a.seg_cpc[sg] = sizes[sg];
+            blk += (cells[sg] + sizes[sg] - 1) / sizes[sg];
+            cell += cells[sg];
+        } else { // empty segment: no CTA selects it
+            a.seg_blk[sg] = sg == 0 ? 0 : INT_MAX; a.seg_cell[sg] = cell; a.seg_cpc[sg] = sizes[0];
+        }
+        a.seg_cell[sg + 1] = cell;
+    }
+    return blk;
 }
 
 // One fused push+arrange step.  Nothing is enqueued behind it to catch a declined step: the device records
@@ -875,19 +914,16 @@ static int push_fused(pic_species *s)
     {   // PIC_TRACE: report the launch geometry whenever it changes
         static const bool trace = getenv("PIC_TRACE") != nullptr;
         static int last[6] = {-1, -1, -1, -1, -1, -1};
-        const int now[6] = {geo.rows, geo.cpc, geo.stages, geo.def, geo.ctas_per_sm, (int)geo.smem};
+        const int now[6] = {geo.rows, geo.cpc + 1000 * geo.taper, geo.stages, geo.def, geo.ctas_per_sm, (int)geo.smem};
         if (trace && memcmp(last, now, sizeof now)) {
             memcpy(last, now, sizeof now);
-            fprintf(stderr, "[pic fused] step %lld: rows %d, cells/CTA %d, stages %d, queue %d, CTAs/SM %d, smem %d B (maxcount %d, maxdef %d)\n",
-                    s->steps, geo.rows, geo.cpc, geo.stages, geo.def, geo.ctas_per_sm, (int)geo.smem, s->h_maxcount, s->h_maxdef);
+            fprintf(stderr, "[pic fused] step %lld: rows %d, cells/CTA %d (taper %d), stages %d, queue %d, CTAs/SM %d, smem %d B (maxcount %d, maxdef %d)\n",
+                    s->steps, geo.rows, geo.cpc, geo.taper, geo.stages, geo.def, geo.ctas_per_sm, (int)geo.smem, s->h_maxcount, s->h_maxdef);
         }
     }
     a.step_id = (int)(s->steps & 0x7fffffff);
     const int rows = geo.rows;
-    const int nchunks = (sim->nc + a.CPC - 1) / a.CPC;
-    a.COLS = sim->opt_fused_cols ? std::max(1, std::min(nchunks, sim->sm_count * geo.ctas_per_sm)) : nchunks;
-    a.RUN = (nchunks + a.COLS - 1) / a.COLS;
-    const int grid = a.COLS * a.RUN;
+    const int grid = fused_schedule(a, sim->nc, a.CPC, geo.taper, sim->sm_count * geo.ctas_per_sm);
     const size_t smem = geo.smem;
     if (s->unv_steps == 0) {
         s->unv_steps0 = s->steps;

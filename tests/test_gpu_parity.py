@@ -285,11 +285,13 @@ def test_fused_step_is_the_one_that_runs(config, kw, steps):
 @pytest.mark.parametrize("knobs", [
     {"fused_cells_per_cta": 1}, {"fused_cells_per_cta": 3, "fused_rows": 12}, {"fused_cells_per_cta": 256},
     {"fused_rows": 16}, {"fused_cells_per_cta": 33, "fused_rows": 8}, {"fused_cells_per_cta": 7},
+    {"fused_cells_per_cta": 16, "fused_taper": 3}, {"fused_cells_per_cta": 64, "fused_taper": 1},
+    {"fused_cells_per_cta": 5, "fused_taper": 2}, {"fused_cells_per_cta": 256, "fused_taper": 3},
 ])
 @pytest.mark.parametrize("config,kw", [(4, dict(nc=4099)), (2, dict(nc=1500))])
 def test_fused_knobs_do_not_change_results(knobs, config, kw):
-    """Cells per CTA and rows per tile only move the tile / chunk borders (halo cells, deferred
-    right-movers, carried counts land elsewhere); results stay bit-identical."""
+    """Cells per CTA, the tapered chunk schedule and rows per tile only move the tile / chunk borders (halo cells,
+    deferred right-movers, carried counts land elsewhere); results stay bit-identical."""
     inp = workloads.make(config, **kw)
     sim, _ = run_stepwise(inp, 12, options={"fused": 1, **knobs}, check_every=3)
     info = pic.pic_fused_info(sim.species[0])
