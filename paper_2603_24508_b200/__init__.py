@@ -22,7 +22,7 @@ EXPORTS = [
     "pic_active_buffer", "pic_cell_counts", "pic_step_count", "pic_arrange_info", "pic_workspace_bytes",
     "pic_set_option", "pic_launch_count", "pic_sync", "pic_destroy", "pic_strerror", "pic_last_error",
     "pic_run_host", "pic_kernel_time", "pic_fused_info", "pic_deposit", "pic_n_live", "pic_set_field_device",
-    "pic_solve_field", "pic_get_field",
+    "pic_solve_field", "pic_get_field", "pic_push_all",
 ]
 
 
@@ -76,6 +76,7 @@ def lib():
         L.pic_species_at.argtypes = [vp, C.c_int]
         L.pic_species_at.restype = vp
         L.pic_push.argtypes = [vp, C.c_int]
+        L.pic_push_all.argtypes = [vp, C.c_int]
         L.pic_arrange.argtypes = [vp]
         L.pic_wall_flux.argtypes = [vp, C.POINTER(pic_wall_flux_t)]
         L.pic_set_field.argtypes = [vp, C.POINTER(C.c_double)]
@@ -221,6 +222,11 @@ def pic_species_at(sim, i):
 
 def pic_push(sp, nsteps=1):
     _check(lib().pic_push(sp.handle, int(nsteps)), "pic_push")
+
+
+def pic_push_all(sim, nsteps=1):
+    """Every species of the sim, nsteps steps each; the species' kernels overlap on internal streams."""
+    _check(lib().pic_push_all(sim.handle, int(nsteps)), "pic_push_all")
 
 
 def pic_arrange(sp):

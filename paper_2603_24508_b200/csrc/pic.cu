@@ -41,6 +41,10 @@ static const char *const K_NAMES[K_COUNT] = {"mover", "hist", "scan", "scatter",
 
 struct pic_species {
     pic_sim *sim = nullptr;
+    cudaStream_t stream = nullptr;     // where this species' kernels go: the sim's stream, or -- for the duration of a
+                                       // pic_push_all -- its own (own_stream), so that the species' steps overlap
+    cudaStream_t own_stream = nullptr;
+    cudaEvent_t join_ev = nullptr;
     PushConst k{};
     double qm = 0;
     long long n_ub = 0, capacity = 0; // host-known upper bound of DevState::n
@@ -100,9 +104,10 @@ struct pic_sim {
     double *d_f[2]{}, *d_phi = nullptr, *d_tile = nullptr, *d_scal = nullptr;
     unsigned long long *d_emax = nullptr;
     int device = 0;
+    cudaEvent_t fork_ev = nullptr; // pic_push_all: the species' own streams start behind it
     std::vector<pic_species *> sp;
     unsigned long long launches = 0;
-    int opt_fused = 1, opt_timing = 0, opt_tile_scatter = 1, opt_fused_tma = 1, opt_fused_pdl = 1, opt_fused_taper = -1;
+    int opt_fused = 1, opt_timing = 0, opt_tile_scatter = 1, opt_fused_tma = 1, opt_fused_pdl = 1, opt_fused_taper = -1, opt_species_streams = 1;
     int opt_fused_cpc = 0, opt_fused_rows = 0, opt_fused_slots = 0, opt_fused_stages = 0; // tuning knobs of the fused step (0 = automatic)
     int sm_count = 148;
     // per-kernel device timing (option "kernel_timing"): event pairs recorded around launches
@@ -125,16 +130,17 @@ struct KernelSpan {
         if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); return nullptr; }
         return e;
     }
-    KernelSpan(pic_sim *s, int kid) : sim(s), id(kid)
+    cudaStream_t stream;
+    KernelSpan(pic_sim *s, int kid, cudaStream_t st = nullptr) : sim(s), id(kid), stream(st ? st : s->stream)
     {
         if (!sim->opt_timing) return;
         a = get(sim); b = get(sim);
-        if (a) cudaEventRecord(a, sim->stream);
+        if (a) cudaEventRecord(a, stream);
     }
     ~KernelSpan()
     {
         if (!a || !b) return;
-        cudaEventRecord(b, sim->stream);
+        cudaEventRecord(b, stream);
         sim->spans.push_back({id, a, b});
     }
 };
@@ -171,6 +177,8 @@ static void free_species(pic_species *s)
     cudaFree(s->d_cs);
     if (s->h_tel) cudaFreeHost(s->h_tel);
     if (s->tel_ev) cudaEventDestroy(s->tel_ev);
+    if (s->join_ev) cudaEventDestroy(s->join_ev);
+    if (s->own_stream) cudaStreamDestroy(s->own_stream);
     delete s;
 }
 
@@ -181,6 +189,7 @@ extern "C" void pic_destroy(pic_sim *sim)
     for (pic_species *s : sim->sp) free_species(s);
     for (auto &sp : sim->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
     for (cudaEvent_t e : sim->free_events) cudaEventDestroy(e);
+    if (sim->fork_ev) cudaEventDestroy(sim->fork_ev);
     cudaFree(sim->d_E);
     cudaFree(sim->d_f[0]); cudaFree(sim->d_f[1]); cudaFree(sim->d_phi); cudaFree(sim->d_tile); cudaFree(sim->d_scal);
     cudaFree(sim->d_emax);
@@ -227,10 +236,10 @@ static int run_scan(pic_species *s, const int *in, int *out, int m, ScanFold fol
 {
     pic_sim *sim = s->sim;
     size_t words = scan_scratch_words(m);
-    CU(cudaMemsetAsync(s->d_scan, 0, words * sizeof(unsigned long long), sim->stream));
+    CU(cudaMemsetAsync(s->d_scan, 0, words * sizeof(unsigned long long), s->stream));
     int ntiles = (m + SCAN_TILE - 1) / SCAN_TILE;
-    KernelSpan span(sim, K_SCAN);
-    scan_exclusive_kernel<<<ntiles, SCAN_THREADS, 0, sim->stream>>>(in, out, m, s->d_scan, fold);
+    KernelSpan span(sim, K_SCAN, s->stream);
+    scan_exclusive_kernel<<<ntiles, SCAN_THREADS, 0, s->stream>>>(in, out, m, s->d_scan, fold);
     return launch_check(sim, "scan_exclusive_kernel");
 }
 
@@ -246,7 +255,7 @@ static int run_maxcount(pic_species *s, int which)
 {
     pic_sim *sim = s->sim;
     const int nc = sim->nc;
-    maxcount_kernel<<<(nc + 255) / 256, 256, 0, sim->stream>>>(s->d_off[which], nc, s->d_st);
+    maxcount_kernel<<<(nc + 255) / 256, 256, 0, s->stream>>>(s->d_off[which], nc, s->d_st);
     return launch_check(sim, "maxcount_kernel");
 }
 
@@ -333,6 +342,7 @@ static int alloc_species(pic_sim *sim, const pic_species_desc &d, pic_species **
     if (!s) return PIC_ENOMEM;
     *out = s;
     s->sim = sim;
+    s->stream = sim->stream;
     s->qm = d.qm;
     s->n_ub = d.n;
     s->capacity = d.capacity;
@@ -371,17 +381,17 @@ static int init_species(pic_sim *sim, pic_species *s, const pic_species_desc &d)
     const int nc = sim->nc;
     DevState h{};
     h.n = (int)d.n;
-    CU(cudaMemcpyAsync(s->d_st, &h, sizeof h, cudaMemcpyHostToDevice, sim->stream));
-    CU(cudaStreamSynchronize(sim->stream)); // h is a stack object
+    CU(cudaMemcpyAsync(s->d_st, &h, sizeof h, cudaMemcpyHostToDevice, s->stream));
+    CU(cudaStreamSynchronize(s->stream)); // h is a stack object
 
     // validate the initial state, build count/offset of the initial grouping
     if (d.n > 0) {
         int blocks = (int)((d.n + 255) / 256);
-        validate_kernel<<<blocks, 256, 0, sim->stream>>>(s->x[0], s->vx[0], s->vy[0], s->vz[0], s->cell[0], s->k, s->d_st);
+        validate_kernel<<<blocks, 256, 0, s->stream>>>(s->x[0], s->vx[0], s->vy[0], s->vz[0], s->cell[0], s->k, s->d_st);
         if (int rc = launch_check(sim, "validate_kernel")) return rc;
     }
-    CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, sim->stream));
-    CU(cudaStreamSynchronize(sim->stream));
+    CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
     if (h.status & ERR_BAD_INITIAL) {
         snprintf(g_err, sizeof g_err, "initial state violates 0<=x<L, cell==floor(x/dx), all live");
         return PIC_ESTATE;
@@ -389,7 +399,7 @@ static int init_species(pic_sim *sim, pic_species *s, const pic_species_desc &d)
     bool grouped = !(h.status & ERR_NOT_GROUPED);
     if (d.n > 0) {
         int blocks = (int)((d.n + HIST_THREADS * HIST_ITEMS - 1) / (HIST_THREADS * HIST_ITEMS));
-        hist_kernel<<<blocks, HIST_THREADS, 0, sim->stream>>>(s->cell[0], s->d_count[0], s->d_st);
+        hist_kernel<<<blocks, HIST_THREADS, 0, s->stream>>>(s->cell[0], s->d_count[0], s->d_st);
         if (int rc = launch_check(sim, "hist_kernel")) return rc;
     }
     ScanFold nofold{nullptr, 0, 0, 0, nullptr};
@@ -399,12 +409,12 @@ static int init_species(pic_sim *sim, pic_species *s, const pic_species_desc &d)
     s->h_grouped = grouped;
     h.status = 0;
     h.w_acc = grouped ? 0 : W_UNKNOWN;
-    CU(cudaMemcpyAsync(s->d_st, &h, sizeof h, cudaMemcpyHostToDevice, sim->stream));
-    CU(cudaStreamSynchronize(sim->stream));
+    CU(cudaMemcpyAsync(s->d_st, &h, sizeof h, cudaMemcpyHostToDevice, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
     if (grouped) { // largest per-cell count: sizes the tiles of the fused step
         if (int rc = run_maxcount(s, 0)) return rc;
-        CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, sim->stream));
-        CU(cudaStreamSynchronize(sim->stream));
+        CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, s->stream));
+        CU(cudaStreamSynchronize(s->stream));
         s->h_maxcount = h.maxcount;
     }
     s->cur = 0;
@@ -596,6 +606,7 @@ extern "C" int pic_set_option(pic_sim *sim, const char *key, int value)
     else if (!strcmp(key, "fused") && flag) sim->opt_fused = value;
     else if (!strcmp(key, "fused_tma") && flag) sim->opt_fused_tma = value;
     else if (!strcmp(key, "fused_pdl") && flag) sim->opt_fused_pdl = value;
+    else if (!strcmp(key, "species_streams") && flag) sim->opt_species_streams = value;
     else if (!strcmp(key, "fused_taper") && value >= -1 && value < FUSED_SEGS) sim->opt_fused_taper = value;
     else if (!strcmp(key, "fused_cells_per_cta") && value >= 0 && value <= FUSED_CPC_MAX) sim->opt_fused_cpc = value;
     else if (!strcmp(key, "fused_stage_slots") && value >= 0 && value <= 512 && value % 2 == 0) sim->opt_fused_slots = value;
@@ -650,11 +661,11 @@ static int arrange_split(pic_species *s, bool hist_ready, bool after_mover)
     const int src = s->cur, dst = s->cur ^ 1;
     const int oo = s->cur_off, on = s->cur_off ^ 1;
     if (!hist_ready) {
-        CU(cudaMemsetAsync(s->d_count[on], 0, sizeof(int) * (size_t)nc, sim->stream));
+        CU(cudaMemsetAsync(s->d_count[on], 0, sizeof(int) * (size_t)nc, s->stream));
         if (s->n_ub > 0) {
             int blocks = (int)((s->n_ub + HIST_THREADS * HIST_ITEMS - 1) / (HIST_THREADS * HIST_ITEMS));
-            KernelSpan span(sim, K_HIST);
-            hist_kernel<<<blocks, HIST_THREADS, 0, sim->stream>>>(s->cell[src], s->d_count[on], s->d_st);
+            KernelSpan span(sim, K_HIST, s->stream);
+            hist_kernel<<<blocks, HIST_THREADS, 0, s->stream>>>(s->cell[src], s->d_count[on], s->d_st);
             if (int rc = launch_check(sim, "hist_kernel")) return rc;
         }
     }
@@ -671,7 +682,7 @@ static int arrange_split(pic_species *s, bool hist_ready, bool after_mover)
     const bool general_follows = !(s->h_grouped && s->h_wsum <= FAST_W_LIMIT);
     a.general_follows = general_follows ? 1 : 0;
     {
-        KernelSpan span(sim, K_SCATTER);
+        KernelSpan span(sim, K_SCATTER, s->stream);
         // tile-ranked stable scatter (tilesort.cuh) when the caller gave a workspace; the destination-driven
         // scatter behind it runs only if a tile declined (or instead of it without a workspace)
         const bool tiles = sim->opt_tile_scatter && s->ws && s->ws_bytes >= ts_workspace_bytes(s->n_ub) && s->n_ub > 0;
@@ -685,17 +696,17 @@ static int arrange_split(pic_species *s, bool hist_ready, bool after_mover)
             const int nt = (int)ts_ntiles(s->n_ub);
             t.tinfo = reinterpret_cast<int2 *>(s->ws);
             t.thist = reinterpret_cast<int *>(static_cast<char *>(s->ws) + (((size_t)(nt + 1) * sizeof(int2) + 255) & ~(size_t)255));
-            tile_hist_kernel<<<nt, TS_THREADS, 0, sim->stream>>>(t);
+            tile_hist_kernel<<<nt, TS_THREADS, 0, s->stream>>>(t);
             if (int rc = launch_check(sim, "tile_hist_kernel")) return rc;
-            tile_base_kernel<<<(nc + 255) / 256, 256, 0, sim->stream>>>(t);
+            tile_base_kernel<<<(nc + 255) / 256, 256, 0, s->stream>>>(t);
             if (int rc = launch_check(sim, "tile_base_kernel")) return rc;
-            tile_scatter_kernel<<<nt, TS_THREADS, TS_SMEM_BYTES, sim->stream>>>(t);
+            tile_scatter_kernel<<<nt, TS_THREADS, TS_SMEM_BYTES, s->stream>>>(t);
             if (int rc = launch_check(sim, "tile_scatter_kernel")) return rc;
             a.only_if = &s->d_st->tile_declined;
         }
         long long want = ((long long)nc + SCATTER_THREADS / 32 - 1) / (SCATTER_THREADS / 32);
         int blocks = (int)std::min<long long>(want, (long long)sim->sm_count * 64);
-        scatter_fast_kernel<<<blocks, SCATTER_THREADS, 0, sim->stream>>>(a);
+        scatter_fast_kernel<<<blocks, SCATTER_THREADS, 0, s->stream>>>(a);
         if (int rc = launch_check(sim, "scatter_fast_kernel")) return rc;
     }
     // every kernel of the general path returns at once unless scatter_fast_kernel declined on the device; if it is not
@@ -708,7 +719,7 @@ static int arrange_split(pic_species *s, bool hist_ready, bool after_mover)
         ga.off_old = s->d_off[oo];
         ga.scan_scratch = s->d_scan;
         KernelSpan gspan(sim, K_GENERAL);
-        if (int rc = general_arrange(ga, sim->stream, sim->sm_count, &sim->launches)) return rc == PIC_ECUDA ? cuda_fail(cudaGetLastError(), "general_arrange") : rc;
+        if (int rc = general_arrange(ga, s->stream, sim->sm_count, &sim->launches)) return rc == PIC_ECUDA ? cuda_fail(cudaGetLastError(), "general_arrange") : rc;
     }
     if (s->sim->opt_fused && s->arrange_every == 1)
         if (int rc = run_maxcount(s, on)) return rc;
@@ -736,7 +747,7 @@ extern "C" int pic_arrange(pic_species *s)
 template <bool RC, bool H>
 static void launch_mover(pic_species *s, const MoverArgs &a, int blocks)
 {
-    mover_kernel<RC, H><<<blocks, MOVER_THREADS, 0, s->sim->stream>>>(a);
+    mover_kernel<RC, H><<<blocks, MOVER_THREADS, 0, s->stream>>>(a);
 }
 
 static int push_split(pic_species *s, bool will_arrange)
@@ -744,7 +755,7 @@ static int push_split(pic_species *s, bool will_arrange)
     pic_sim *sim = s->sim;
     const int nc = sim->nc;
     const int on = s->cur_off ^ 1;
-    if (will_arrange) CU(cudaMemsetAsync(s->d_count[on], 0, sizeof(int) * (size_t)nc, sim->stream));
+    if (will_arrange) CU(cudaMemsetAsync(s->d_count[on], 0, sizeof(int) * (size_t)nc, s->stream));
     if (s->n_ub > 0) {
         MoverArgs a{};
         a.x = s->x[s->cur]; a.vx = s->vx[s->cur]; a.vy = s->vy[s->cur]; a.vz = s->vz[s->cur];
@@ -753,7 +764,7 @@ static int push_split(pic_species *s, bool will_arrange)
         long long pairs = (s->n_ub + 1) / 2;
         int blocks = (int)((pairs + MOVER_THREADS - 1) / MOVER_THREADS);
         const bool rc = !s->all_live;
-        KernelSpan span(sim, K_MOVER);
+        KernelSpan span(sim, K_MOVER, s->stream);
         if (rc) { if (will_arrange) launch_mover<true, true>(s, a, blocks); else launch_mover<true, false>(s, a, blocks); }
         else    { if (will_arrange) launch_mover<false, true>(s, a, blocks); else launch_mover<false, false>(s, a, blocks); }
         if (int r = launch_check(sim, "mover_kernel")) return r;
@@ -764,7 +775,7 @@ static int push_split(pic_species *s, bool will_arrange)
     if (!sim->periodic) s->all_live = false;
     s->counts_fresh = false;
     if (!will_arrange) {
-        end_step_kernel<<<1, 1, 0, sim->stream>>>(s->d_st, s->reset_w ? 1 : 0);
+        end_step_kernel<<<1, 1, 0, s->stream>>>(s->d_st, s->reset_w ? 1 : 0);
         s->reset_w = false;
         if (int r = launch_check(sim, "end_step_kernel")) return r;
     }
@@ -931,8 +942,8 @@ static int push_fused(pic_species *s)
         s->unv_off0 = s->cur_off;
     }
     {
-        KernelSpan span(sim, K_FUSED);
-        fused_edge_kernel<<<1, 128, 0, sim->stream>>>(a);
+        KernelSpan span(sim, K_FUSED, s->stream);
+        fused_edge_kernel<<<1, 128, 0, s->stream>>>(a);
         if (int rc = launch_check(sim, "fused_edge_kernel")) return rc;
         const bool bz0 = s->k.tz == 0.0 && s->k.sz == 0.0; // B in the x-y plane: the kernel drops the exact-zero products
         void (*kern)(FusedArgs) = fused_pick(rows, sim->periodic != 0, bz0, sim->opt_fused_tma != 0, geo.def);
@@ -943,7 +954,7 @@ static int push_fused(pic_species *s)
             cfg.gridDim = dim3((unsigned)grid);
             cfg.blockDim = dim3(32);
             cfg.dynamicSmemBytes = smem;
-            cfg.stream = sim->stream;
+            cfg.stream = s->stream;
             cudaLaunchAttribute attr[1];
             attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
             attr[0].val.programmaticStreamSerializationAllowed = 1;
@@ -951,15 +962,15 @@ static int push_fused(pic_species *s)
             cfg.numAttrs = 1;
             CU(cudaLaunchKernelEx(&cfg, kern, a));
         } else {
-            kern<<<grid, 32, smem, sim->stream>>>(a);
+            kern<<<grid, 32, smem, s->stream>>>(a);
         }
         if (int rc = launch_check(sim, "fused_kernel")) return rc;
-        fused_commit_kernel<<<1, 1, 0, sim->stream>>>(s->d_st, a.step_id);
+        fused_commit_kernel<<<1, 1, 0, s->stream>>>(s->d_st, a.step_id);
         if (int rc = launch_check(sim, "fused_commit_kernel")) return rc;
     }
     if (++s->tel_step >= FUSED_TELEMETRY_STEPS && !s->tel_pending) {
-        CU(cudaMemcpyAsync(s->h_tel, s->d_st, sizeof(DevState), cudaMemcpyDeviceToHost, sim->stream));
-        CU(cudaEventRecord(s->tel_ev, sim->stream));
+        CU(cudaMemcpyAsync(s->h_tel, s->d_st, sizeof(DevState), cudaMemcpyDeviceToHost, s->stream));
+        CU(cudaEventRecord(s->tel_ev, s->stream));
         s->tel_pending = true;
         s->tel_step = 0;
     }
@@ -983,8 +994,8 @@ static int verify_fused(pic_species *s)
 {
     if (s->unv_steps == 0) return PIC_OK;
     DevState h;
-    CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, s->sim->stream));
-    CU(cudaStreamSynchronize(s->sim->stream));
+    CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
     const long long run = s->unv_steps;
     s->unv_steps = 0;
     if (!h.fused_disabled) return PIC_OK;
@@ -1042,8 +1053,8 @@ extern "C" int pic_push(pic_species *s, int nsteps)
 static int read_state(pic_species *s, DevState &h)
 {
     if (int rc = verify_fused(s)) return rc;
-    CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, s->sim->stream));
-    CU(cudaStreamSynchronize(s->sim->stream));
+    CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
     if (h.n >= 0 && h.n <= s->n_ub) s->n_ub = h.n;
     s->h_vmax = std::sqrt((double)bits_to_float(h.vmax2));
     s->h_steps_since_sync = 0;
@@ -1051,8 +1062,8 @@ static int read_state(pic_species *s, DevState &h)
     if (!s->sim->emax_known) { // the field was replaced on the device: fetch its max |E| for the displacement bound
         pic_sim *sim = s->sim;
         unsigned long long bits = 0;
-        CU(cudaMemcpyAsync(&bits, sim->d_emax, sizeof bits, cudaMemcpyDeviceToHost, sim->stream));
-        CU(cudaStreamSynchronize(sim->stream));
+        CU(cudaMemcpyAsync(&bits, sim->d_emax, sizeof bits, cudaMemcpyDeviceToHost, s->stream));
+        CU(cudaStreamSynchronize(s->stream));
         double em;
         memcpy(&em, &bits, sizeof em);
         sim->Emax = em;
@@ -1068,11 +1079,48 @@ static int read_state(pic_species *s, DevState &h)
     if (s->fused_off && s->arrange_every == 1 && s->counts_fresh && h.w_acc <= 1 && h.status == 0 &&
         s->steps - s->declined_at >= FUSED_RETRY_STEPS && !(h.abort_reason & FA_EDGE_OVERFLOW) && s->h_maxdef <= FUSED_DEF_BIG) {
         const int zero = 0;
-        CU(cudaMemcpyAsync(&s->d_st->fused_disabled, &zero, sizeof zero, cudaMemcpyHostToDevice, s->sim->stream));
-        CU(cudaStreamSynchronize(s->sim->stream));
+        CU(cudaMemcpyAsync(&s->d_st->fused_disabled, &zero, sizeof zero, cudaMemcpyHostToDevice, s->stream));
+        CU(cudaStreamSynchronize(s->stream));
         s->fused_off = false;
     }
     return PIC_OK;
+}
+
+// All species of the sim, nsteps steps each.  The species are independent within a step (they share only the field,
+// read-only), so each runs on a stream of its own for the duration of the call: their kernels overlap, in particular
+// the ramp and the tail of one species' grid with the bulk of another's ("two streams on one
+// GPU").  Fork and join are events: on return everything is ordered on the sim's stream again.
+extern "C" int pic_push_all(pic_sim *sim, int nsteps)
+{
+    if (!sim || nsteps < 0) return PIC_EINVAL;
+    const size_t ns = sim->sp.size();
+    if (ns <= 1 || !sim->opt_species_streams) {
+        for (int it = 0; it < nsteps; ++it)
+            for (pic_species *s : sim->sp)
+                if (int rc = pic_push(s, 1)) return rc;
+        return PIC_OK;
+    }
+    if (!sim->fork_ev) CU(cudaEventCreateWithFlags(&sim->fork_ev, cudaEventDisableTiming));
+    for (pic_species *s : sim->sp) {
+        if (!s->own_stream) CU(cudaStreamCreateWithFlags(&s->own_stream, cudaStreamNonBlocking));
+        if (!s->join_ev) CU(cudaEventCreateWithFlags(&s->join_ev, cudaEventDisableTiming));
+    }
+    CU(cudaEventRecord(sim->fork_ev, sim->stream));
+    for (pic_species *s : sim->sp) {
+        CU(cudaStreamWaitEvent(s->own_stream, sim->fork_ev, 0));
+        s->stream = s->own_stream;
+    }
+    int rc = PIC_OK;
+    for (int it = 0; it < nsteps && rc == PIC_OK; ++it)
+        for (pic_species *s : sim->sp)
+            if ((rc = pic_push(s, 1)) != PIC_OK) break;
+    for (pic_species *s : sim->sp) { // join, whatever happened
+        s->stream = sim->stream;
+        const cudaError_t e1 = cudaEventRecord(s->join_ev, s->own_stream);
+        const cudaError_t e2 = e1 == cudaSuccess ? cudaStreamWaitEvent(sim->stream, s->join_ev, 0) : e1;
+        if (e2 != cudaSuccess && rc == PIC_OK) rc = cuda_fail(e2, "pic_push_all join");
+    }
+    return rc;
 }
 
 extern "C" int pic_wall_flux(pic_species *s, pic_wall_flux_t *out)
@@ -1133,10 +1181,10 @@ extern "C" int pic_cell_counts(pic_species *s, int32_t *count_host, int32_t *off
     if (!s->counts_fresh) return PIC_ESTATE;
     const int nc = s->sim->nc;
     if (count_host)
-        CU(cudaMemcpyAsync(count_host, s->d_count[s->cur_off], sizeof(int) * (size_t)nc, cudaMemcpyDeviceToHost, s->sim->stream));
+        CU(cudaMemcpyAsync(count_host, s->d_count[s->cur_off], sizeof(int) * (size_t)nc, cudaMemcpyDeviceToHost, s->stream));
     if (offset_host)
-        CU(cudaMemcpyAsync(offset_host, s->d_off[s->cur_off], sizeof(int) * ((size_t)nc + 1), cudaMemcpyDeviceToHost, s->sim->stream));
-    CU(cudaStreamSynchronize(s->sim->stream));
+        CU(cudaMemcpyAsync(offset_host, s->d_off[s->cur_off], sizeof(int) * ((size_t)nc + 1), cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
     return PIC_OK;
 }
 
@@ -1157,14 +1205,14 @@ extern "C" int pic_deposit(pic_species *s, double weight, double *rho_dev, int a
     a.cs = s->d_cs;
     a.nc = nc;
     a.inv_dx = s->k.inv_dx;
-    KernelSpan span(sim, K_DEPOSIT);
+    KernelSpan span(sim, K_DEPOSIT, s->stream);
     const int lpc = s->n_ub <= 448LL * nc ? 16 : 32; // lanes per cell from the mean particles per cell (16 measured best up to 200)
     const long long threads = (long long)nc * lpc;
     const unsigned blocks = (unsigned)((threads + DEP_THREADS - 1) / DEP_THREADS);
-    if (lpc == 16) deposit_cell_kernel<16><<<blocks, DEP_THREADS, 0, sim->stream>>>(a);
-    else deposit_cell_kernel<32><<<blocks, DEP_THREADS, 0, sim->stream>>>(a);
+    if (lpc == 16) deposit_cell_kernel<16><<<blocks, DEP_THREADS, 0, s->stream>>>(a);
+    else deposit_cell_kernel<32><<<blocks, DEP_THREADS, 0, s->stream>>>(a);
     if (int rc = launch_check(sim, "deposit_cell_kernel")) return rc;
-    deposit_node_kernel<<<(nc + 1 + 255) / 256, 256, 0, sim->stream>>>(s->d_cs, nc, sim->periodic, weight, accumulate ? 1 : 0, rho_dev);
+    deposit_node_kernel<<<(nc + 1 + 255) / 256, 256, 0, s->stream>>>(s->d_cs, nc, sim->periodic, weight, accumulate ? 1 : 0, rho_dev);
     return launch_check(sim, "deposit_node_kernel");
 }
 
@@ -1271,7 +1319,7 @@ extern "C" int pic_run_host(const pic_grid_desc *g, pic_host_species *hs, int ns
         rc = pic_create(g, descs.data(), nspecies, &sim);
         if (rc) break;
         mark("pic_create done");
-        for (int i = 0; i < nspecies && rc == PIC_OK; ++i) rc = pic_push(sim->sp[i], nsteps);
+        rc = pic_push_all(sim, nsteps);
         if (rc) break;
         mark("steps done");
         // the copies back: each array on a second stream as soon as its species has been read out, so that they

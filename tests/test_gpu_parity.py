@@ -49,6 +49,46 @@ def test_config3_reduced_two_species(options):
     run_stepwise(inp, 60, options=options, check_every=4)
 
 
+@pytest.mark.parametrize("options", VARIANTS + [pytest.param({"fused": 1, "species_streams": 0}, id="fused-one-stream")])
+@pytest.mark.parametrize("chunk", [1, 7])
+def test_push_all_species_on_their_own_streams(options, chunk):
+    """pic_push_all: electrons, D+ and a neutral species stepped together (each species on an internal stream of its
+    own, kernels overlapping) -- every species must match its oracle bit for bit, the call must leave everything ordered
+    on the sim's stream (the comparison reads the buffers through that stream), and calls may be interleaved with
+    per-species pic_push / pic_arrange."""
+    inp = workloads.make(3, nc=1500)
+    e = inp["species"][0]
+    inp["species"].append(dict(e, qm=0.0, x=e["x"].copy(), vx=e["vx"].copy(), vy=e["vy"].copy(), vz=e["vz"].copy(),
+                               cell=e["cell"].copy()))
+    sim, states = make_pair(inp, options=options)
+    done = 0
+    while done < 42:
+        pic.pic_push_all(sim, chunk)
+        for st in states:
+            st.push(chunk)
+        done += chunk
+        if done == 14:  # one species alone in between, then an explicit arrange of another
+            pic.pic_push(sim.species[1], 2)
+            states[1].push(2)
+            pic.pic_arrange(sim.species[2])
+            states[2].arrange()
+        if done % 14 == 0:
+            for si, (sp, st) in enumerate(zip(sim.species, states)):
+                compare(sp, st, where=f"push_all step {done} species {si}", counts=True, nc=inp["nc"])
+    pic.pic_sync(sim)
+    assert states[0].wall.sum() > 0
+
+
+def test_push_all_single_species_and_errors():
+    inp = workloads.make(1, nc=256, ppc=32)
+    sim, states = make_pair(inp)
+    pic.pic_push_all(sim, 5)
+    states[0].push(5)
+    compare(sim.species[0], states[0], where="push_all, one species", counts=True, nc=inp["nc"])
+    with pytest.raises(pic.PicError):
+        pic.pic_push_all(sim, -1)
+
+
 @pytest.mark.parametrize("options", VARIANTS)
 def test_config4_reduced_periodic(options):
     """configs[3] shape: periodic, 100 ppc, 16 modes; 4,099 cells (odd, prime) -> 409,900 particles."""
