@@ -155,6 +155,9 @@ __global__ void __launch_bounds__(128) fused_edge_kernel(FusedArgs a)
     // programmatic dependent launch: the streaming kernel behind may start now; it waits (griddepcontrol.wait) for
     // this grid to complete before it reads anything written here or writes anything at all
     asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+    // this kernel is itself launched programmatically behind the previous step's commit kernel (its launch overlaps
+    // that kernel): everything it reads -- the state that step wrote, its offsets, DevState -- is complete after this
+    asm volatile("griddepcontrol.wait;\n" ::: "memory");
     if (threadIdx.x == 0) s_bad = 0;
     __syncthreads();
     if (st->fused_disabled) {
@@ -165,37 +168,56 @@ __global__ void __launch_bounds__(128) fused_edge_kernel(FusedArgs a)
     const int s0 = a.off_old[cell], s1 = a.off_old[cell + 1];
     const int ql = warp == 0 ? 0 : 1; // list of this warp (only warps 0 and 3 can see class X)
     int nL = 0, nS = 0, nR = 0, nX = 0, bad = 0;
-    for (int i0 = s0; i0 < s1; i0 += 32) {
-        const int i = i0 + lane;
-        int g = -1;
-        PushOut o;
-        if (i < s1) {
-            const double x = a.sx[i], vx = a.svx[i], vy = a.svy[i], vz = a.svz[i];
-            double xs, jf;
-            int j;
-            if (gather_cell(a.k, x, xs, jf, j) && j == cell) {
-                const double E0 = __ldg(a.E + j), E1 = __ldg(a.E + j + 1);
-                push_core(a.k, x, vx, vy, vz, xs, jf, j, E0, E1, o);
-                g = fused_classify(a.k, j, o, bad);
-            } else {
+    // Batches of EDGE_ROWS rows of 32 slots: all of a batch's particle loads are issued before anything waits for one
+    // of them, then all its E loads -- the kernel is a chain of memory latencies (the streaming kernel behind waits for
+    // it), so a cell costs two round trips instead of two per row.
+    constexpr int EDGE_ROWS = 8;
+    for (int b0 = s0; b0 < s1; b0 += 32 * EDGE_ROWS) {
+        double x[EDGE_ROWS], vx[EDGE_ROWS], vy[EDGE_ROWS], vz[EDGE_ROWS], xs[EDGE_ROWS], jf[EDGE_ROWS], E0[EDGE_ROWS], E1[EDGE_ROWS];
+        int jj[EDGE_ROWS];
+        bool ok[EDGE_ROWS];
+#pragma unroll
+        for (int r = 0; r < EDGE_ROWS; ++r) {
+            const int i = b0 + 32 * r + lane;
+            x[r] = vx[r] = vy[r] = vz[r] = 0.0;
+            if (i < s1) { x[r] = a.sx[i]; vx[r] = a.svx[i]; vy[r] = a.svy[i]; vz[r] = a.svz[i]; }
+        }
+#pragma unroll
+        for (int r = 0; r < EDGE_ROWS; ++r) {
+            const int i = b0 + 32 * r + lane;
+            jj[r] = cell;
+            ok[r] = i < s1 && gather_cell(a.k, x[r], xs[r], jf[r], jj[r]) && jj[r] == cell;
+            E0[r] = E1[r] = 0.0;
+            if (ok[r]) { E0[r] = __ldg(a.E + jj[r]); E1[r] = __ldg(a.E + jj[r] + 1); }
+        }
+#pragma unroll
+        for (int r = 0; r < EDGE_ROWS; ++r) {
+            const int i = b0 + 32 * r + lane;
+            if (b0 + 32 * r >= s1) break; // warp-uniform
+            int g = -1;
+            PushOut o;
+            if (ok[r]) {
+                push_core(a.k, x[r], vx[r], vy[r], vz[r], xs[r], jf[r], jj[r], E0[r], E1[r], o);
+                g = fused_classify(a.k, jj[r], o, bad);
+            } else if (i < s1) {
                 bad = 1;
             }
-        }
-        const unsigned mL = __ballot_sync(FULL, g == 0), mS = __ballot_sync(FULL, g == 1);
-        const unsigned mR = __ballot_sync(FULL, g == 2), mX = __ballot_sync(FULL, g == 3);
-        if (g == 3) {
-            const int r = nX + __popc(mX & lt);
-            if (warp == 0 || warp == 3) {
-                if (r < FUSED_XCAP) {
-                    qx[ql][r] = o.x; qvx[ql][r] = o.vx; qvy[ql][r] = o.vy; qvz[ql][r] = o.vz;
+            const unsigned mL = __ballot_sync(FULL, g == 0), mS = __ballot_sync(FULL, g == 1);
+            const unsigned mR = __ballot_sync(FULL, g == 2), mX = __ballot_sync(FULL, g == 3);
+            if (g == 3) {
+                const int rk = nX + __popc(mX & lt);
+                if (warp == 0 || warp == 3) {
+                    if (rk < FUSED_XCAP) {
+                        qx[ql][rk] = o.x; qvx[ql][rk] = o.vx; qvy[ql][rk] = o.vy; qvz[ql][rk] = o.vz;
+                    } else {
+                        bad |= 2; // more leavers than the list holds
+                    }
                 } else {
-                    bad |= 2; // more leavers than the list holds
+                    bad |= 1; // class X out of cell 1 or nc-2: the particle moved two cells
                 }
-            } else {
-                bad |= 1; // class X out of cell 1 or nc-2: the particle moved two cells
             }
+            nL += __popc(mL); nS += __popc(mS); nR += __popc(mR); nX += __popc(mX);
         }
-        nL += __popc(mL); nS += __popc(mS); nR += __popc(mR); nX += __popc(mX);
     }
     bad = (int)__reduce_or_sync(FULL, (unsigned)bad);
     if (lane == 0) {
@@ -778,6 +800,10 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
 // after every CTA's stores and atomics).
 __global__ void fused_commit_kernel(DevState *st, int step_id)
 {
+    // launched programmatically behind fused_kernel: wait for that grid to complete (no early trigger there, so this
+    // kernel runs after every CTA has exited; and none here, so the next step's edge kernel -- and with it the next
+    // streaming kernel's prologue -- starts only after this step is complete)
+    asm volatile("griddepcontrol.wait;\n" ::: "memory");
     if (!st->abort) {
         st->n = st->n_next;
         st->wall[0] += st->wall_pend[0];

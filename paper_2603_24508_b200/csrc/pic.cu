@@ -45,6 +45,8 @@ struct pic_species {
                                        // pic_push_all -- its own (own_stream), so that the species' steps overlap
     cudaStream_t own_stream = nullptr;
     cudaEvent_t join_ev = nullptr;
+    bool chain_valid = false;          // push_fused: the library's last kernel launch was this species' commit kernel
+    unsigned long long chain_mark = 0; // ... when sim->launches still has this value
     PushConst k{};
     double qm = 0;
     long long n_ub = 0, capacity = 0; // host-known upper bound of DevState::n
@@ -943,16 +945,17 @@ static int push_fused(pic_species *s)
     }
     {
         KernelSpan span(sim, K_FUSED, s->stream);
-        fused_edge_kernel<<<1, 128, 0, s->stream>>>(a);
-        if (int rc = launch_check(sim, "fused_edge_kernel")) return rc;
-        const bool bz0 = s->k.tz == 0.0 && s->k.sz == 0.0; // B in the x-y plane: the kernel drops the exact-zero products
-        void (*kern)(FusedArgs) = fused_pick(rows, sim->periodic != 0, bz0, sim->opt_fused_tma != 0, geo.def);
-        if (sim->opt_fused_pdl) {
-            // programmatic dependent launch: the CTAs start while fused_edge_kernel is still running and do their
-            // prologue (offsets, E window, first bulk copies); griddepcontrol.wait holds them before anything else
+        // programmatic dependent launches (option "fused_pdl"): each kernel of the chain edge -> streaming -> commit ->
+        // next step's edge is set up while its predecessor still runs and waits (griddepcontrol.wait) for it before it
+        // reads or writes anything the predecessor touches; the streaming kernel's prologue overlaps the edge kernel
+        auto launch = [&](bool pdl, auto kern, int grid, int block, size_t smem, auto... args) -> cudaError_t {
+            if (!pdl) {
+                kern<<<grid, block, smem, s->stream>>>(args...);
+                return cudaSuccess;
+            }
             cudaLaunchConfig_t cfg{};
             cfg.gridDim = dim3((unsigned)grid);
-            cfg.blockDim = dim3(32);
+            cfg.blockDim = dim3((unsigned)block);
             cfg.dynamicSmemBytes = smem;
             cfg.stream = s->stream;
             cudaLaunchAttribute attr[1];
@@ -960,13 +963,24 @@ static int push_fused(pic_species *s)
             attr[0].val.programmaticStreamSerializationAllowed = 1;
             cfg.attrs = attr;
             cfg.numAttrs = 1;
-            CU(cudaLaunchKernelEx(&cfg, kern, a));
-        } else {
-            kern<<<grid, 32, smem, s->stream>>>(a);
-        }
+            return cudaLaunchKernelEx(&cfg, kern, args...);
+        };
+        // The edge kernel only when the last kernel this library launched was this species' previous commit kernel
+        // (which waited for its step to complete and triggers nothing early): behind any other kernel the streaming
+        // kernel's prologue -- it starts with the edge kernel and reads E, offsets and particles before it waits --
+        // could run before that kernel's writes are visible.
+        const bool pdl = sim->opt_fused_pdl != 0;
+        const bool chained = pdl && s->chain_valid && s->chain_mark == sim->launches;
+        CU(launch(chained, fused_edge_kernel, 1, 128, (size_t)0, a));
+        if (int rc = launch_check(sim, "fused_edge_kernel")) return rc;
+        const bool bz0 = s->k.tz == 0.0 && s->k.sz == 0.0; // B in the x-y plane: the kernel drops the exact-zero products
+        void (*kern)(FusedArgs) = fused_pick(rows, sim->periodic != 0, bz0, sim->opt_fused_tma != 0, geo.def);
+        CU(launch(pdl, kern, grid, 32, smem, a));
         if (int rc = launch_check(sim, "fused_kernel")) return rc;
-        fused_commit_kernel<<<1, 1, 0, s->stream>>>(s->d_st, a.step_id);
+        CU(launch(pdl, fused_commit_kernel, 1, 1, (size_t)0, s->d_st, a.step_id));
         if (int rc = launch_check(sim, "fused_commit_kernel")) return rc;
+        s->chain_valid = true;
+        s->chain_mark = sim->launches;
     }
     if (++s->tel_step >= FUSED_TELEMETRY_STEPS && !s->tel_pending) {
         CU(cudaMemcpyAsync(s->h_tel, s->d_st, sizeof(DevState), cudaMemcpyDeviceToHost, s->stream));
@@ -1112,8 +1126,14 @@ extern "C" int pic_push_all(pic_sim *sim, int nsteps)
     }
     int rc = PIC_OK;
     for (int it = 0; it < nsteps && rc == PIC_OK; ++it)
-        for (pic_species *s : sim->sp)
+        for (pic_species *s : sim->sp) {
+            const unsigned long long before = sim->launches;
             if ((rc = pic_push(s, 1)) != PIC_OK) break;
+            // these launches went to this species' own stream: they do not stand between another species' commit
+            // kernel and its next edge kernel (push_fused: chain_mark)
+            for (pic_species *o : sim->sp)
+                if (o != s) o->chain_mark += sim->launches - before;
+        }
     for (pic_species *s : sim->sp) { // join, whatever happened
         s->stream = sim->stream;
         const cudaError_t e1 = cudaEventRecord(s->join_ev, s->own_stream);
