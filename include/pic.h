@@ -258,14 +258,23 @@ typedef struct {
 } pic_host_species;
 
 /* End-to-end convenience with HOST buffers: allocates device memory, copies the species up,
- * runs pic_create + pic_push(nsteps) on every species, copies the final state and the wall
- * counters back and releases everything.  grid->stream is used as in pic_create.  Pinned
+ * runs pic_create + pic_push_all(nsteps), copies the final state and the wall
+ * counters back and releases everything (into the library's memory pool, see pic_trim_memory).
+ * grid->stream is used as in pic_create.  Pinned
  * host arrays make the copies faster but are not required.  Syncs.  Errors as pic_create /
  * pic_push, PIC_ENOMEM when the device allocation fails. */
 int pic_run_host(const pic_grid_desc *grid, pic_host_species *species, int nspecies, int nsteps);
 
+/* Device memory the library owns (the handles' small objects, the field-solve scratch, the arena of
+ * pic_run_host) is taken from a stream-ordered memory pool of the current device that KEEPS freed
+ * memory for the next call instead of returning it to the driver ("allocate once, keep
+ * resident, release at the end"): after pic_destroy / pic_run_host the bytes are free for this library
+ * but still held by the process.  pic_trim_memory returns everything not in use to the driver.  Syncs
+ * the device.  Errors: PIC_ECUDA. */
+int pic_trim_memory(void);
+
 int pic_sync(pic_sim *sim);     /* wait for the stream; reports deferred device errors */
-void pic_destroy(pic_sim *sim); /* frees library-owned memory; caller buffers untouched */
+void pic_destroy(pic_sim *sim); /* frees library-owned memory (into the pool, see pic_trim_memory); caller buffers untouched */
 const char *pic_strerror(int status);
 const char *pic_last_error(void); /* text of the last CUDA error seen by this thread */
 

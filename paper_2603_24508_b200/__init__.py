@@ -22,7 +22,7 @@ EXPORTS = [
     "pic_active_buffer", "pic_cell_counts", "pic_step_count", "pic_arrange_info", "pic_workspace_bytes",
     "pic_set_option", "pic_launch_count", "pic_sync", "pic_destroy", "pic_strerror", "pic_last_error",
     "pic_run_host", "pic_kernel_time", "pic_fused_info", "pic_deposit", "pic_n_live", "pic_set_field_device",
-    "pic_solve_field", "pic_get_field", "pic_push_all",
+    "pic_solve_field", "pic_get_field", "pic_push_all", "pic_trim_memory",
 ]
 
 
@@ -103,6 +103,7 @@ def lib():
         L.pic_strerror.restype = C.c_char_p
         L.pic_last_error.argtypes = []
         L.pic_last_error.restype = C.c_char_p
+        L.pic_trim_memory.argtypes = []
         L.pic_run_host.argtypes = [C.POINTER(pic_grid_desc), C.POINTER(pic_host_species), C.c_int, C.c_int]
         _lib = L
     return _lib
@@ -222,6 +223,11 @@ def pic_species_at(sim, i):
 
 def pic_push(sp, nsteps=1):
     _check(lib().pic_push(sp.handle, int(nsteps)), "pic_push")
+
+
+def pic_trim_memory():
+    """Return the device memory cached by the library's pool (freed handles, pic_run_host arenas) to the driver."""
+    _check(lib().pic_trim_memory(), "pic_trim_memory")
 
 
 def pic_push_all(sim, nsteps=1):

@@ -149,6 +149,63 @@ struct KernelSpan {
 
 static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+// Device memory the library owns (handles' small objects, field scratch, the arena of pic_run_host) comes from one
+// stream-ordered memory pool per device that keeps what is freed instead of returning it to the driver: PAPER.md:89
+// "allocate once, keep resident, release at the end", applied across calls -- a second pic_create / pic_run_host of
+// the same size costs no cudaMalloc and no cudaFree (both synchronise the device and take milliseconds for
+// gigabytes).  pic_trim_memory() hands the cached memory back.
+static cudaMemPool_t g_pool[64] = {};
+static std::vector<void *> g_pinned_free; // pinned DevState blocks of destroyed species (telemetry), reused
+// The arena of pic_run_host (gigabytes: two buffer sets and the workspace of every species) is a plain cudaMalloc
+// kept for the next call -- growing a memory pool by 9 GB took 1.15 s against 1-2 ms for cudaMalloc.
+static struct { char *p; size_t bytes; } g_arena[64] = {};
+
+static cudaError_t dev_alloc(void **p, size_t bytes, int device, cudaStream_t st)
+{
+    *p = nullptr;
+    if (device < 0 || device >= 64) return cudaMalloc(p, bytes);
+    if (!g_pool[device]) {
+        cudaMemPoolProps props{};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = device;
+        cudaError_t e = cudaMemPoolCreate(&g_pool[device], &props);
+        if (e != cudaSuccess) { g_pool[device] = nullptr; return e; }
+        unsigned long long keep = ~0ull;
+        e = cudaMemPoolSetAttribute(g_pool[device], cudaMemPoolAttrReleaseThreshold, &keep);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaMallocFromPoolAsync(p, bytes ? bytes : 16, g_pool[device], st);
+}
+
+template <typename T>
+static cudaError_t dev_alloc(T **p, size_t bytes, int device, cudaStream_t st)
+{
+    return dev_alloc(reinterpret_cast<void **>(p), bytes, device, st);
+}
+
+static void dev_free(void *p, cudaStream_t st)
+{
+    if (p) cudaFreeAsync(p, st);
+}
+
+extern "C" int pic_trim_memory(void)
+{
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceSynchronize());
+    if (dev >= 0 && dev < 64 && g_pool[dev]) CU(cudaMemPoolTrimTo(g_pool[dev], 0));
+    if (dev >= 0 && dev < 64 && g_arena[dev].p) {
+        CU(cudaFree(g_arena[dev].p));
+        g_arena[dev].p = nullptr;
+        g_arena[dev].bytes = 0;
+    }
+    for (void *h : g_pinned_free) cudaFreeHost(h);
+    g_pinned_free.clear();
+    return PIC_OK;
+}
+
 extern "C" const char *pic_strerror(int s)
 {
     switch (s) {
@@ -173,11 +230,12 @@ extern "C" size_t pic_workspace_bytes(int32_t nc, int64_t capacity)
 static void free_species(pic_species *s)
 {
     if (!s) return;
-    cudaFree(s->d_st);
-    for (int b = 0; b < 2; ++b) { cudaFree(s->d_count[b]); cudaFree(s->d_off[b]); }
-    cudaFree(s->d_scan);
-    cudaFree(s->d_cs);
-    if (s->h_tel) cudaFreeHost(s->h_tel);
+    cudaStream_t st = s->sim ? s->sim->stream : nullptr;
+    dev_free(s->d_st, st);
+    for (int b = 0; b < 2; ++b) { dev_free(s->d_count[b], st); dev_free(s->d_off[b], st); }
+    dev_free(s->d_scan, st);
+    dev_free(s->d_cs, st);
+    if (s->h_tel) g_pinned_free.push_back(s->h_tel);
     if (s->tel_ev) cudaEventDestroy(s->tel_ev);
     if (s->join_ev) cudaEventDestroy(s->join_ev);
     if (s->own_stream) cudaStreamDestroy(s->own_stream);
@@ -192,9 +250,11 @@ extern "C" void pic_destroy(pic_sim *sim)
     for (auto &sp : sim->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
     for (cudaEvent_t e : sim->free_events) cudaEventDestroy(e);
     if (sim->fork_ev) cudaEventDestroy(sim->fork_ev);
-    cudaFree(sim->d_E);
-    cudaFree(sim->d_f[0]); cudaFree(sim->d_f[1]); cudaFree(sim->d_phi); cudaFree(sim->d_tile); cudaFree(sim->d_scal);
-    cudaFree(sim->d_emax);
+    dev_free(sim->d_E, sim->stream);
+    dev_free(sim->d_f[0], sim->stream); dev_free(sim->d_f[1], sim->stream); dev_free(sim->d_phi, sim->stream);
+    dev_free(sim->d_tile, sim->stream); dev_free(sim->d_scal, sim->stream);
+    dev_free(sim->d_emax, sim->stream);
+    cudaStreamSynchronize(sim->stream); // the frees are stream-ordered: the memory is back in the pool on return
     delete sim;
 }
 
@@ -360,10 +420,10 @@ static int alloc_species(pic_sim *sim, const pic_species_desc &d, pic_species **
     s->k.L = (double)sim->nc * sim->dx;
 
     const int nc = sim->nc;
-    CU(cudaMalloc(&s->d_st, sizeof(DevState)));
+    CU(dev_alloc(&s->d_st, sizeof(DevState), sim->device, sim->stream));
     for (int b = 0; b < 2; ++b) {
-        CU(cudaMalloc(&s->d_count[b], sizeof(int) * ((size_t)nc + 16)));
-        CU(cudaMalloc(&s->d_off[b], sizeof(int) * ((size_t)nc + 16)));
+        CU(dev_alloc(&s->d_count[b], sizeof(int) * ((size_t)nc + 16), sim->device, sim->stream));
+        CU(dev_alloc(&s->d_off[b], sizeof(int) * ((size_t)nc + 16), sim->device, sim->stream));
         CU(cudaMemsetAsync(s->d_count[b], 0, sizeof(int) * ((size_t)nc + 16), sim->stream));
         CU(cudaMemsetAsync(s->d_off[b], 0, sizeof(int) * ((size_t)nc + 16), sim->stream));
     }
@@ -371,8 +431,9 @@ static int alloc_species(pic_sim *sim, const pic_species_desc &d, pic_species **
     // general path's per-tile digit histograms)
     long long max_scan = std::max<long long>((long long)nc + 1, general_scan_elems(d.capacity));
     s->scan_words = scan_scratch_words(max_scan);
-    CU(cudaMalloc(&s->d_scan, s->scan_words * sizeof(unsigned long long)));
-    CU(cudaMallocHost(&s->h_tel, sizeof(DevState)));
+    CU(dev_alloc(&s->d_scan, s->scan_words * sizeof(unsigned long long), sim->device, sim->stream));
+    if (!g_pinned_free.empty()) { s->h_tel = static_cast<DevState *>(g_pinned_free.back()); g_pinned_free.pop_back(); }
+    else CU(cudaMallocHost(&s->h_tel, sizeof(DevState)));
     CU(cudaEventCreateWithFlags(&s->tel_ev, cudaEventDisableTiming));
     return PIC_OK;
 }
@@ -460,7 +521,7 @@ extern "C" int pic_create(const pic_grid_desc *g, const pic_species_desc *specie
         cudaError_t e = cudaDeviceGetAttribute(&sim->sm_count, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess) { rc = cuda_fail(e, "cudaDeviceGetAttribute"); break; }
         // E padded to an even number of nodes (+2) so that 16-byte bulk copies of any window stay inside
-        e = cudaMalloc(&sim->d_E, sizeof(double) * ((size_t)g->nc + 8));
+        e = dev_alloc(&sim->d_E, sizeof(double) * ((size_t)g->nc + 8), sim->device, sim->stream);
         if (e != cudaSuccess) { rc = e == cudaErrorMemoryAllocation ? PIC_ENOMEM : cuda_fail(e, "cudaMalloc E"); break; }
         for (int i = 0; i < nspecies && rc == PIC_OK; ++i) { // all allocations first: nothing here waits on the stream
             pic_species *s = nullptr;
@@ -514,12 +575,12 @@ static int field_alloc(pic_sim *sim)
     if (sim->d_emax) return PIC_OK;
     const size_t nb = sizeof(double) * ((size_t)sim->nc + 8);
     const size_t nt = (size_t)fld_ntiles(sim->nc);
-    cudaError_t e = cudaMalloc(&sim->d_f[0], nb);
-    if (e == cudaSuccess) e = cudaMalloc(&sim->d_f[1], nb);
-    if (e == cudaSuccess) e = cudaMalloc(&sim->d_phi, nb);
-    if (e == cudaSuccess) e = cudaMalloc(&sim->d_tile, sizeof(double) * 4 * nt);
-    if (e == cudaSuccess) e = cudaMalloc(&sim->d_scal, sizeof(double) * 4);
-    if (e == cudaSuccess) e = cudaMalloc(&sim->d_emax, 2 * sizeof(unsigned long long)); // max |E| bits, two tickets
+    cudaError_t e = dev_alloc(&sim->d_f[0], nb, sim->device, sim->stream);
+    if (e == cudaSuccess) e = dev_alloc(&sim->d_f[1], nb, sim->device, sim->stream);
+    if (e == cudaSuccess) e = dev_alloc(&sim->d_phi, nb, sim->device, sim->stream);
+    if (e == cudaSuccess) e = dev_alloc(&sim->d_tile, sizeof(double) * 4 * nt, sim->device, sim->stream);
+    if (e == cudaSuccess) e = dev_alloc(&sim->d_scal, sizeof(double) * 4, sim->device, sim->stream);
+    if (e == cudaSuccess) e = dev_alloc(&sim->d_emax, 2 * sizeof(unsigned long long), sim->device, sim->stream); // max |E| bits, two tickets
     if (e == cudaSuccess) e = cudaMemsetAsync(sim->d_emax, 0, 2 * sizeof(unsigned long long), sim->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(sim->d_scal, 0, sizeof(double) * 4, sim->stream);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? PIC_ENOMEM : cuda_fail(e, "cudaMalloc field scratch");
@@ -1216,7 +1277,7 @@ extern "C" int pic_deposit(pic_species *s, double weight, double *rho_dev, int a
     pic_sim *sim = s->sim;
     const int nc = sim->nc;
     if (!s->d_cs) {
-        cudaError_t e = cudaMalloc(&s->d_cs, sizeof(double2) * (size_t)nc);
+        cudaError_t e = dev_alloc(&s->d_cs, sizeof(double2) * (size_t)nc, sim->device, s->stream);
         if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? PIC_ENOMEM : cuda_fail(e, "cudaMalloc deposition sums");
     }
     DepositArgs a{};
@@ -1294,6 +1355,7 @@ extern "C" int pic_run_host(const pic_grid_desc *g, pic_host_species *hs, int ns
     int rc = PIC_OK;
     pic_sim *sim = nullptr;
     char *arena = nullptr;
+    bool arena_cached = false;
     cudaStream_t copy_stream = nullptr;
     auto align256 = [](size_t b) { return (b + 255) & ~(size_t)255; };
     do {
@@ -1306,8 +1368,20 @@ extern "C" int pic_run_host(const pic_grid_desc *g, pic_host_species *hs, int ns
             total += 2 * (4 * nb + ni) + align256(pic_workspace_bytes(g->nc, h.n) + 16);
         }
         if (rc) break;
-        cudaError_t e = cudaMalloc(&arena, total ? total : 256);
-        if (e != cudaSuccess) { cudaGetLastError(); arena = nullptr; rc = PIC_ENOMEM; break; }
+        int device = 0;
+        cudaGetDevice(&device);
+        const bool cacheable = device >= 0 && device < 64;
+        cudaError_t e = cudaSuccess;
+        if (cacheable && g_arena[device].p && g_arena[device].bytes >= total) {
+            arena = g_arena[device].p; // the previous call's arena (pic_trim_memory releases it)
+        } else {
+            if (cacheable && g_arena[device].p) { cudaFree(g_arena[device].p); g_arena[device].p = nullptr; g_arena[device].bytes = 0; }
+            e = cudaMalloc(&arena, total ? total : 256);
+            if (e != cudaSuccess) { cudaGetLastError(); arena = nullptr; rc = PIC_ENOMEM; break; }
+            if (cacheable) { g_arena[device].p = arena; g_arena[device].bytes = total ? total : 256; }
+            arena_cached = cacheable;
+        }
+        arena_cached = cacheable;
         mark("device arena allocated");
         size_t off = 0;
         auto carve = [&](size_t bytes) { void *p = arena + off; off += bytes; return p; };
@@ -1377,7 +1451,7 @@ extern "C" int pic_run_host(const pic_grid_desc *g, pic_host_species *hs, int ns
     if (sim) pic_destroy(sim);
     else cudaStreamSynchronize(stream);
     mark("sim destroyed");
-    if (arena) cudaFree(arena);
+    if (arena && !arena_cached) cudaFree(arena); // else: kept for the next call
     mark("arena released");
     return rc;
 }

@@ -42,8 +42,8 @@ def test_fullsize_first_steps_elementwise(config, steps, check_every):
     ae = inp["arrange_every"]
     for step in range(1, steps + 1):
         for sp, st in zip(sim.species, states):
-            pic.pic_push(sp, 1)
             st.push(1)
+        pic.pic_push_all(sim, 1)  # the call bench.py times
         if step % check_every == 0 or step == steps:
             for si, (sp, st) in enumerate(zip(sim.species, states)):
                 compare(sp, st, where=f"config {config} full size, step {step} species {si}",
@@ -136,8 +136,8 @@ def test_fullsize_all_steps_sampled_and_properties(config, margin):
 # ---- the whole run, element by element (north_star: "arranged order bit-exact ... on all five configs") ----------
 @pytest.mark.parametrize("config,single_thread_too", [(2, True), (3, False), (4, False), (5, False)])
 def test_fullsize_whole_run_elementwise(config, single_thread_too):
-    """Every step of the config at full size, in bench.py's launch configuration, one pic_push(nsteps) per species
-    (as the e2e leg) -- then the final state against the oracle's: the five arrays bit for bit over [0, n_live),
+    """Every step of the config at full size, in bench.py's launch configuration, one pic_push_all(nsteps) (as the e2e
+    leg; the two species of config 3 overlap on their own streams) -- then the final state against the oracle's: the five arrays bit for bit over [0, n_live),
     counts, offsets, walls.  A wrong rank inside a cell at any step changes the final order, so this covers the
     stable order the sampled test below cannot see."""
     inp = workloads.make(config)
@@ -147,8 +147,7 @@ def test_fullsize_whole_run_elementwise(config, single_thread_too):
     with torch.cuda.stream(stream):
         sim, _ = make_pair(inp, stream=stream)
     del _
-    for sp in sim.species:
-        pic.pic_push(sp, steps)
+    pic.pic_push_all(sim, steps)
     pic.pic_sync(sim)
     for si, (sp, s) in enumerate(zip(sim.species, inp["species"])):
         kw = dict(nc=nc, dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E=inp["E"], qm=s["qm"], B=inp["B"],

@@ -269,6 +269,32 @@ def test_run_host_end_to_end():
         assert np.array_equal(a[:n_out], o)
 
 
+def test_memory_pool_is_reused_and_trimmed():
+    """The library's device memory comes from a pool that keeps freed blocks ("allocate once, keep
+    resident"): repeated pic_run_host calls give the same result from the cached arena, the process holds the memory
+    in between, and pic_trim_memory returns it to the driver."""
+    import torch
+    inp = workloads.make(4, nc=20000)  # 2 M particles: an arena of ~150 MB
+    s = inp["species"][0]
+    st = oracle.State(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], nc=inp["nc"], dx=inp["dx"], dt=inp["dt"],
+                      boundary=inp["boundary"], E=inp["E"], qm=s["qm"], B=inp["B"], arrange_every=1)
+    st.push(5)
+    pic.pic_trim_memory()
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    for _ in range(3):
+        arrs = [np.array(s[k]) for k in ("x", "vx", "vy", "vz", "cell")]
+        n_out, _, _ = pic.pic_run_host(nc=inp["nc"], dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E_nodes=inp["E"],
+                                       B=inp["B"], species=[dict(qm=s["qm"], arrays=arrs, arrange_every=1)], nsteps=5)[0]
+        assert n_out == st.n
+        for a, o in zip(arrs, st.live()):
+            assert np.array_equal(a[:n_out], o)
+    held = free0 - torch.cuda.mem_get_info()[0]
+    assert held >= 100 << 20, f"the pool should still hold the arena, holds {held} bytes"
+    pic.pic_trim_memory()
+    assert free0 - torch.cuda.mem_get_info()[0] < 32 << 20, "pic_trim_memory did not return the cached memory"
+
+
 @pytest.mark.parametrize("config,kw,steps,pinned", [(3, dict(nc=1500), 25, True), (5, dict(nc=2048), 23, False)])
 def test_run_host_two_species_and_pinned_buffers(config, kw, steps, pinned):
     """pic_run_host with several species in one call (one device arena, D2H on a second stream), pinned torch
