@@ -265,6 +265,20 @@ typedef struct {
  * pic_push, PIC_ENOMEM when the device allocation fails. */
 int pic_run_host(const pic_grid_desc *grid, pic_host_species *species, int nspecies, int nsteps);
 
+/* ncycles closed PIC cycles (Fig. 1), the field never leaving the device:
+ *     pic_push_all(sim, 1);  rho = sum over species i of pic_deposit(species i, weights[i]);
+ *     pic_solve_field(sim, rho, smooth_passes, phi_dev)          -- E for the next step
+ * with exactly the results of those calls, but enqueued WITHOUT the host-side check each of them makes of the fused
+ * steps before it (one synchronisation per cycle): should a fused step decline, the device freezes the cycle (no
+ * further fused step starts, E is not replaced) and the next synchronising call redoes every cycle from that one on
+ * with the checked calls.  weights: HOST, one per species (charge per macro-particle over dx, sign included).
+ * rho_dev: DEVICE, nc+1 doubles, caller-owned scratch and output (the last cycle's charge density); phi_dev: DEVICE,
+ * nc+1 doubles or NULL; both must stay valid until the next synchronising call.  Asynchronous whenever every species
+ * runs the fused step (arrange_every == 1, arranged, all live); otherwise each cycle is the three checked calls.
+ * Option "cycle_async" = 0 forces the latter.  Errors: PIC_EINVAL (NULL, ncycles < 0, passes outside 0..1024, nc < 2,
+ * weight not finite), PIC_ESTATE (a species is not arranged), PIC_ENOMEM, PIC_ECUDA. */
+int pic_cycle(pic_sim *sim, int ncycles, const double *weights, int smooth_passes, double *rho_dev, double *phi_dev);
+
 /* Device memory the library owns (the handles' small objects, the field-solve scratch, the arena of
  * pic_run_host) is taken from a stream-ordered memory pool of the current device that KEEPS freed
  * memory for the next call instead of returning it to the driver ("allocate once, keep

@@ -22,7 +22,7 @@ EXPORTS = [
     "pic_active_buffer", "pic_cell_counts", "pic_step_count", "pic_arrange_info", "pic_workspace_bytes",
     "pic_set_option", "pic_launch_count", "pic_sync", "pic_destroy", "pic_strerror", "pic_last_error",
     "pic_run_host", "pic_kernel_time", "pic_fused_info", "pic_deposit", "pic_n_live", "pic_set_field_device",
-    "pic_solve_field", "pic_get_field", "pic_push_all", "pic_trim_memory",
+    "pic_solve_field", "pic_get_field", "pic_push_all", "pic_trim_memory", "pic_cycle",
 ]
 
 
@@ -31,7 +31,7 @@ class PicError(RuntimeError):
         self.status = status
         msg = f"{where}: {pic_strerror(status)} ({status})"
         extra = pic_last_error()
-        if status == PIC_ECUDA and extra:
+        if status in (PIC_ECUDA, PIC_ESTATE) and extra:
             msg += f": {extra}"
         super().__init__(msg)
 
@@ -104,6 +104,7 @@ def lib():
         L.pic_last_error.argtypes = []
         L.pic_last_error.restype = C.c_char_p
         L.pic_trim_memory.argtypes = []
+        L.pic_cycle.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.c_int, vp, vp]
         L.pic_run_host.argtypes = [C.POINTER(pic_grid_desc), C.POINTER(pic_host_species), C.c_int, C.c_int]
         _lib = L
     return _lib
@@ -273,6 +274,29 @@ def pic_solve_field(sim, rho, smooth_passes=0, phi=None, want_phi=False):
                                  C.c_void_p(phi.data_ptr()) if phi is not None else None), "pic_solve_field")
     torch.cuda.current_stream().wait_stream(sim.stream)
     return phi
+
+
+def pic_cycle(sim, ncycles, weights, smooth_passes=0, rho=None, phi=None, want_phi=False):
+    """pic_cycle: ncycles closed PIC cycles (push all species, deposit, smooth + Poisson + E) enqueued without a host
+    round trip.  weights: one per species.  rho / phi: torch float64 device tensors (nc+1), allocated if None (phi only
+    when want_phi); they are kept alive by the Sim until the next call.  Returns (rho, phi)."""
+    import torch
+    dev = sim.species[0].bufs[0][0].device
+    if rho is None:
+        rho = torch.empty(sim.nc + 1, dtype=torch.float64, device=dev)
+    if phi is None and want_phi:
+        phi = torch.empty(sim.nc + 1, dtype=torch.float64, device=dev)
+    for t in (rho, phi):
+        if t is not None:
+            assert t.dtype == torch.float64 and t.numel() == sim.nc + 1 and t.is_contiguous() and t.is_cuda
+    w = (C.c_double * len(sim.species))(*[float(x) for x in weights])
+    assert len(weights) == len(sim.species)
+    sim._cycle_keep = (rho, phi)  # the library reads and writes them until its next synchronising call
+    sim.stream.wait_stream(torch.cuda.current_stream())
+    _check(lib().pic_cycle(sim.handle, int(ncycles), w, int(smooth_passes), C.c_void_p(rho.data_ptr()),
+                           C.c_void_p(phi.data_ptr()) if phi is not None else None), "pic_cycle")
+    torch.cuda.current_stream().wait_stream(sim.stream)
+    return rho, phi
 
 
 def pic_get_field(sim):

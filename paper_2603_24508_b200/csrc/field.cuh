@@ -70,6 +70,8 @@ struct FieldArgs {
     unsigned *ticket;  // two arrival counters (zero between launches): the last block of a reduction finishes it
     int nc, periodic, ntiles;
     double dx2, inv_dx;
+    const int *frozen; // pic_cycle: set on the device when a fused step of the cycle declined -- E must keep the field
+                       // that step was issued under until the host has redone it (NULL outside pic_cycle)
 };
 
 // one pass of the 1-2-1 filter (S27, S28): ((left + 2*centre) + right) * 0.25
@@ -343,6 +345,7 @@ __global__ void __launch_bounds__(FLD_THREADS) field_e_kernel(FieldArgs a)
     __shared__ unsigned long long s_max;
     if (threadIdx.x == 0) s_max = 0ull;
     __syncthreads();
+    if (a.frozen && *(volatile const int *)a.frozen) return; // block-uniform
     const double pm = a.scal[2]; // zero on a bounded grid
     const int nc = a.nc;
     const int j = blockIdx.x * FLD_THREADS + threadIdx.x;

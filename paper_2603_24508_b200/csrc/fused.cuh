@@ -74,6 +74,10 @@ struct FusedArgs {
     // (seg_cell[nseg] = nc, unused seg_blk = INT_MAX).  Large chunks first (little halo work), then ever smaller ones
     // so that the CTAs that run last are short and every SM runs dry at about the same time (pic.cu: fused_schedule).
     int seg_blk[FUSED_SEGS], seg_cell[FUSED_SEGS + 1], seg_cpc[FUSED_SEGS];
+    // pic_cycle (steps of several species, deposition and field solve enqueued without a host check in between): one
+    // flag per sim, set by the commit kernel of whichever species declines a step; from then on no species starts
+    // another fused step and the field is not replaced, until the host has redone the cycle (NULL outside pic_cycle)
+    int *frozen;
 };
 
 // Dynamic shared memory of one fused_kernel CTA (one warp): NST stages of CAP = RMAX*32 slots.
@@ -160,7 +164,7 @@ __global__ void __launch_bounds__(128) fused_edge_kernel(FusedArgs a)
     asm volatile("griddepcontrol.wait;\n" ::: "memory");
     if (threadIdx.x == 0) s_bad = 0;
     __syncthreads();
-    if (st->fused_disabled) {
+    if (st->fused_disabled || (a.frozen && *(volatile int *)a.frozen)) {
         if (threadIdx.x == 0) st->abort = 1;
         return;
     }
@@ -798,7 +802,7 @@ __global__ void __launch_bounds__(32, RMAX == 8 ? 16 : (RMAX == 12 ? 10 : 8)) fu
 
 // Commit or roll back one fused step (one thread, launched behind fused_kernel; the kernel boundary orders it
 // after every CTA's stores and atomics).
-__global__ void fused_commit_kernel(DevState *st, int step_id)
+__global__ void fused_commit_kernel(DevState *st, int step_id, int *frozen)
 {
     // launched programmatically behind fused_kernel: wait for that grid to complete (no early trigger there, so this
     // kernel runs after every CTA has exited; and none here, so the next step's edge kernel -- and with it the next
@@ -821,6 +825,7 @@ __global__ void fused_commit_kernel(DevState *st, int step_id)
         // step it was, every later fused launch exits at once, the host redoes the steps (pic.cu: verify_fused)
         if (!st->fused_disabled) st->fail_step = step_id;
         st->fused_disabled = 1;
+        if (frozen) *frozen = 1;
     }
     st->n_next = 0;
     st->wall_pend[0] = st->wall_pend[1] = 0;

@@ -45,6 +45,7 @@ struct pic_species {
                                        // pic_push_all -- its own (own_stream), so that the species' steps overlap
     cudaStream_t own_stream = nullptr;
     cudaEvent_t join_ev = nullptr;
+    long long cyc_step0 = 0;           // pic_cycle: step count before the first cycle that is still unverified
     bool chain_valid = false;          // push_fused: the library's last kernel launch was this species' commit kernel
     unsigned long long chain_mark = 0; // ... when sim->launches still has this value
     PushConst k{};
@@ -107,9 +108,15 @@ struct pic_sim {
     unsigned long long *d_emax = nullptr;
     int device = 0;
     cudaEvent_t fork_ev = nullptr; // pic_push_all: the species' own streams start behind it
+    // pic_cycle: cycles enqueued without a host check (fused steps + deposition + field solve), to be verified -- and,
+    // should a fused step have declined, redone from that cycle on -- by the next synchronising call
+    struct CycleRec { int ncycles; std::vector<double> w; int passes; double *rho, *phi; };
+    std::vector<CycleRec> cyc_pending;
+    int *d_frozen = nullptr;       // device flag: a fused step of a pending cycle declined (fused.cuh, field.cuh)
+    bool in_cycle = false;         // push_fused hands d_frozen to its kernels
     std::vector<pic_species *> sp;
     unsigned long long launches = 0;
-    int opt_fused = 1, opt_timing = 0, opt_tile_scatter = 1, opt_fused_tma = 1, opt_fused_pdl = 1, opt_fused_taper = -1, opt_species_streams = 1;
+    int opt_fused = 1, opt_timing = 0, opt_tile_scatter = 1, opt_fused_tma = 1, opt_fused_pdl = 1, opt_fused_taper = -1, opt_species_streams = 1, opt_cycle_async = 1;
     int opt_fused_cpc = 0, opt_fused_rows = 0, opt_fused_slots = 0, opt_fused_stages = 0; // tuning knobs of the fused step (0 = automatic)
     int sm_count = 148;
     // per-kernel device timing (option "kernel_timing"): event pairs recorded around launches
@@ -254,6 +261,7 @@ extern "C" void pic_destroy(pic_sim *sim)
     dev_free(sim->d_f[0], sim->stream); dev_free(sim->d_f[1], sim->stream); dev_free(sim->d_phi, sim->stream);
     dev_free(sim->d_tile, sim->stream); dev_free(sim->d_scal, sim->stream);
     dev_free(sim->d_emax, sim->stream);
+    dev_free(sim->d_frozen, sim->stream);
     cudaStreamSynchronize(sim->stream); // the frees are stream-ordered: the memory is back in the pool on return
     delete sim;
 }
@@ -551,6 +559,8 @@ extern "C" pic_species *pic_species_at(pic_sim *sim, int i)
     return sim->sp[i];
 }
 
+static int verify_cycles(pic_sim *sim);
+
 extern "C" int pic_set_field(pic_sim *sim, const double *E)
 {
     if (!sim || !E) return PIC_EINVAL;
@@ -610,11 +620,19 @@ extern "C" int pic_set_field_device(pic_sim *sim, const double *E_dev)
     return PIC_OK;
 }
 
+static int solve_enqueue(pic_sim *sim, const double *rho_dev, int smooth_passes, double *phi_dev, const int *frozen);
+
 extern "C" int pic_solve_field(pic_sim *sim, const double *rho_dev, int smooth_passes, double *phi_dev)
 {
     if (!sim || !rho_dev || smooth_passes < 0 || smooth_passes > 1024) return PIC_EINVAL;
     if (sim->nc < 2) return PIC_EINVAL;
     if (int rc = field_barrier(sim)) return rc;
+    return solve_enqueue(sim, rho_dev, smooth_passes, phi_dev, nullptr);
+}
+
+// The kernels of one field solve, enqueued on the sim's stream without any host-side check.
+static int solve_enqueue(pic_sim *sim, const double *rho_dev, int smooth_passes, double *phi_dev, const int *frozen)
+{
     if (int rc = field_alloc(sim)) return rc;
     const int nc = sim->nc;
     const int nblk = (nc + 1 + FLD_THREADS - 1) / FLD_THREADS;
@@ -634,6 +652,7 @@ extern "C" int pic_solve_field(pic_sim *sim, const double *rho_dev, int smooth_p
     a.scal = sim->d_scal; a.emax_bits = sim->d_emax;
     a.ticket = reinterpret_cast<unsigned *>(sim->d_emax + 1);
     a.nc = nc; a.periodic = sim->periodic;
+    a.frozen = frozen;
     { volatile double d2 = sim->dx * sim->dx; a.dx2 = d2; volatile double inv = 1.0 / sim->dx; a.inv_dx = inv; }
     CU(cudaMemsetAsync(sim->d_emax, 0, sizeof(unsigned long long), sim->stream));
     if (sim->periodic) {
@@ -655,6 +674,8 @@ extern "C" int pic_solve_field(pic_sim *sim, const double *rho_dev, int smooth_p
 extern "C" int pic_get_field(pic_sim *sim, double *E_host)
 {
     if (!sim || !E_host) return PIC_EINVAL;
+    if (!sim->cyc_pending.empty()) // unchecked pic_cycle work decides what the field is
+        if (int rc = verify_cycles(sim)) return rc;
     CU(cudaMemcpyAsync(E_host, sim->d_E, sizeof(double) * ((size_t)sim->nc + 1), cudaMemcpyDeviceToHost, sim->stream));
     CU(cudaStreamSynchronize(sim->stream));
     return PIC_OK;
@@ -670,6 +691,7 @@ extern "C" int pic_set_option(pic_sim *sim, const char *key, int value)
     else if (!strcmp(key, "fused_tma") && flag) sim->opt_fused_tma = value;
     else if (!strcmp(key, "fused_pdl") && flag) sim->opt_fused_pdl = value;
     else if (!strcmp(key, "species_streams") && flag) sim->opt_species_streams = value;
+    else if (!strcmp(key, "cycle_async") && flag) sim->opt_cycle_async = value;
     else if (!strcmp(key, "fused_taper") && value >= -1 && value < FUSED_SEGS) sim->opt_fused_taper = value;
     else if (!strcmp(key, "fused_cells_per_cta") && value >= 0 && value <= FUSED_CPC_MAX) sim->opt_fused_cpc = value;
     else if (!strcmp(key, "fused_stage_slots") && value >= 0 && value <= 512 && value % 2 == 0) sim->opt_fused_slots = value;
@@ -996,6 +1018,7 @@ static int push_fused(pic_species *s)
         }
     }
     a.step_id = (int)(s->steps & 0x7fffffff);
+    a.frozen = sim->in_cycle ? sim->d_frozen : nullptr;
     const int rows = geo.rows;
     const int grid = fused_schedule(a, sim->nc, a.CPC, geo.taper, sim->sm_count * geo.ctas_per_sm);
     const size_t smem = geo.smem;
@@ -1038,7 +1061,7 @@ static int push_fused(pic_species *s)
         void (*kern)(FusedArgs) = fused_pick(rows, sim->periodic != 0, bz0, sim->opt_fused_tma != 0, geo.def);
         CU(launch(pdl, kern, grid, 32, smem, a));
         if (int rc = launch_check(sim, "fused_kernel")) return rc;
-        CU(launch(pdl, fused_commit_kernel, 1, 1, (size_t)0, s->d_st, a.step_id));
+        CU(launch(pdl, fused_commit_kernel, 1, 1, (size_t)0, s->d_st, a.step_id, a.frozen));
         if (int rc = launch_check(sim, "fused_commit_kernel")) return rc;
         s->chain_valid = true;
         s->chain_mark = sim->launches;
@@ -1067,6 +1090,7 @@ static int push_fused(pic_species *s)
 // through the split path.  Syncs when there is anything to check.
 static int verify_fused(pic_species *s)
 {
+    if (!s->sim->cyc_pending.empty()) return verify_cycles(s->sim); // unchecked pic_cycle work: all species together
     if (s->unv_steps == 0) return PIC_OK;
     DevState h;
     CU(cudaMemcpyAsync(&h, s->d_st, sizeof h, cudaMemcpyDeviceToHost, s->stream));
@@ -1105,6 +1129,8 @@ static int verify_fused(pic_species *s)
 extern "C" int pic_push(pic_species *s, int nsteps)
 {
     if (!s || nsteps < 0) return PIC_EINVAL;
+    if (!s->sim->in_cycle && !s->sim->cyc_pending.empty()) // unchecked pic_cycle work: settle it before stepping on
+        if (int rc = verify_cycles(s->sim)) return rc;
     for (int it = 0; it < nsteps; ++it) {
         const bool will_arrange = s->arrange_every > 0 && ((s->steps + 1) % s->arrange_every) == 0;
         const bool fused = will_arrange && fused_possible(s) && s->counts_fresh && s->all_live && s->n_ub > 0;
@@ -1269,11 +1295,19 @@ extern "C" int pic_cell_counts(pic_species *s, int32_t *count_host, int32_t *off
     return PIC_OK;
 }
 
+static int deposit_enqueue(pic_species *s, double weight, double *rho_dev, int accumulate);
+
 extern "C" int pic_deposit(pic_species *s, double weight, double *rho_dev, int accumulate)
 {
     if (!s || !rho_dev || !std::isfinite(weight)) return PIC_EINVAL;
     if (int rc = verify_fused(s)) return rc;
     if (!s->counts_fresh || !s->all_live) return PIC_ESTATE;
+    return deposit_enqueue(s, weight, rho_dev, accumulate);
+}
+
+// The two deposition kernels, enqueued without any host-side check (the state must be arranged and all live).
+static int deposit_enqueue(pic_species *s, double weight, double *rho_dev, int accumulate)
+{
     pic_sim *sim = s->sim;
     const int nc = sim->nc;
     if (!s->d_cs) {
@@ -1295,6 +1329,139 @@ extern "C" int pic_deposit(pic_species *s, double weight, double *rho_dev, int a
     if (int rc = launch_check(sim, "deposit_cell_kernel")) return rc;
     deposit_node_kernel<<<(nc + 1 + 255) / 256, 256, 0, s->stream>>>(s->d_cs, nc, sim->periodic, weight, accumulate ? 1 : 0, rho_dev);
     return launch_check(sim, "deposit_node_kernel");
+}
+
+
+// ------------------------------------------------------------------------------------------
+// pic_cycle: the closed PIC cycle, enqueued without a host round trip
+// ------------------------------------------------------------------------------------------
+// A fused step is checked on the device and may decline (fused.cuh); pic_deposit and pic_solve_field therefore check
+// the unverified steps first, which synchronises once per cycle.  pic_cycle owns the whole loop instead, so it can
+// replay it: steps (every species on its own stream), depositions and field solves are enqueued unchecked; should a
+// step decline, the device freezes -- that species' commit kernel raises the sim's flag, no species starts another
+// fused step, field_e_kernel leaves E alone (the depositions and the rest of the solve only write scratch and rho) --
+// and the next synchronising call finds, per species, the last step that completed, and redoes every cycle from the
+// first incomplete one with the ordinary checked calls.  Results are those of the checked loop either way.
+static bool cycle_fast_ok(pic_sim *sim)
+{
+    if (sim->nc < 2 || !sim->opt_cycle_async) return false;
+    for (pic_species *s : sim->sp)
+        if (!(s->arrange_every == 1 && fused_possible(s) && s->counts_fresh && s->all_live && s->n_ub > 0)) return false;
+    return true;
+}
+
+static int verify_cycles(pic_sim *sim)
+{
+    if (sim->cyc_pending.empty()) return PIC_OK;
+    std::vector<pic_sim::CycleRec> recs;
+    recs.swap(sim->cyc_pending); // from here on the ordinary, checked calls can be used
+    long long total = 0;
+    for (const auto &r : recs) total += r.ncycles;
+    const size_t ns = sim->sp.size();
+    std::vector<DevState> h(ns);
+    for (size_t i = 0; i < ns; ++i)
+        CU(cudaMemcpyAsync(&h[i], sim->sp[i]->d_st, sizeof(DevState), cudaMemcpyDeviceToHost, sim->stream));
+    CU(cudaStreamSynchronize(sim->stream));
+    bool any = false;
+    long long first = total; // the first cycle whose step some species did not complete
+    for (size_t i = 0; i < ns; ++i) {
+        pic_species *s = sim->sp[i];
+        const long long run = s->unv_steps;
+        s->unv_steps = 0;
+        if (run != total) {
+            snprintf(g_err, sizeof g_err, "pic_cycle bookkeeping: %lld unverified steps against %lld pending cycles", run, total);
+            return PIC_ESTATE;
+        }
+        if (!h[i].fused_disabled) continue; // completed every step
+        any = true;
+        const long long k = ((long long)h[i].fail_step - (s->unv_steps0 & 0x7fffffff)) & 0x7fffffff; // steps that completed
+        if (k >= run) {
+            snprintf(g_err, sizeof g_err, "pic_cycle bookkeeping: declined step %d outside the pending cycles", h[i].fail_step);
+            return PIC_ESTATE;
+        }
+        first = std::min(first, k);
+        s->fused_off = true;
+        s->declined_at = s->unv_steps0 + run;
+        s->cur = s->unv_cur0 ^ (int)(k & 1);
+        s->cur_off = s->unv_off0 ^ (int)(k & 1);
+        s->steps = s->unv_steps0 + k;
+        s->counts_fresh = true;
+        s->all_live = true;
+        s->reset_w = true;
+        s->h_wsum = 0;
+        s->h_grouped = true;
+        s->h_vmax = std::sqrt((double)bits_to_float(h[i].vmax2));
+        s->h_steps_since_sync = 0;
+        s->h_kick_acc = 0;
+        s->h_maxcount = h[i].maxcount;
+        s->h_maxdef = std::max(s->h_maxdef, h[i].maxdef);
+        s->chain_valid = false;
+    }
+    if (!any) return PIC_OK;
+    CU(cudaMemsetAsync(sim->d_frozen, 0, sizeof(int), sim->stream));
+    {   // the field in force is the one the frozen device kept; its max |E| was cleared by the solves that were skipped
+        CU(cudaMemsetAsync(sim->d_emax, 0, sizeof(unsigned long long), sim->stream));
+        field_emax_kernel<<<(sim->nc + 1 + FLD_THREADS - 1) / FLD_THREADS, FLD_THREADS, 0, sim->stream>>>(sim->d_E, sim->nc, sim->d_emax);
+        if (int rc = launch_check(sim, "field_emax_kernel")) return rc;
+        sim->emax_known = false;
+    }
+    long long idx = 0;
+    for (const auto &r : recs)
+        for (int c = 0; c < r.ncycles; ++c, ++idx) {
+            if (idx < first) continue;
+            for (pic_species *s : sim->sp) // a species that ran concurrently may have completed this cycle's step
+                if (s->steps < s->cyc_step0 + idx + 1)
+                    if (int rc = pic_push(s, 1)) return rc;
+            for (size_t i = 0; i < ns; ++i)
+                if (int rc = pic_deposit(sim->sp[i], r.w[i], r.rho, i > 0)) return rc;
+            if (int rc = pic_solve_field(sim, r.rho, r.passes, r.phi)) return rc;
+        }
+    return PIC_OK;
+}
+
+extern "C" int pic_cycle(pic_sim *sim, int ncycles, const double *weights, int smooth_passes, double *rho_dev, double *phi_dev)
+{
+    if (!sim || ncycles < 0 || !weights || !rho_dev || smooth_passes < 0 || smooth_passes > 1024) return PIC_EINVAL;
+    if (sim->nc < 2) return PIC_EINVAL;
+    const size_t ns = sim->sp.size();
+    for (size_t i = 0; i < ns; ++i)
+        if (!std::isfinite(weights[i])) return PIC_EINVAL;
+    for (int c = 0; c < ncycles; ++c) {
+        if (sim->cyc_pending.empty())
+            for (pic_species *s : sim->sp) // fused steps of earlier plain pic_push calls: check them first
+                if (int rc = verify_fused(s)) return rc;
+        if (!cycle_fast_ok(sim)) { // the ordinary checked calls
+            if (int rc = verify_cycles(sim)) return rc;
+            if (int rc = pic_push_all(sim, 1)) return rc;
+            for (size_t i = 0; i < ns; ++i)
+                if (int rc = pic_deposit(sim->sp[i], weights[i], rho_dev, i > 0)) return rc;
+            if (int rc = pic_solve_field(sim, rho_dev, smooth_passes, phi_dev)) return rc;
+            continue;
+        }
+        if (sim->cyc_pending.empty()) {
+            if (!sim->d_frozen) {
+                cudaError_t e = dev_alloc(&sim->d_frozen, sizeof(int), sim->device, sim->stream);
+                if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? PIC_ENOMEM : cuda_fail(e, "cudaMalloc cycle flag");
+                CU(cudaMemsetAsync(sim->d_frozen, 0, sizeof(int), sim->stream));
+            }
+            for (pic_species *s : sim->sp) s->cyc_step0 = s->steps;
+        }
+        sim->in_cycle = true;
+        const int rc_push = pic_push_all(sim, 1);
+        sim->in_cycle = false;
+        if (rc_push) return rc_push;
+        // recorded before the rest is enqueued: from here on a synchronising call must find (and can redo) this cycle
+        pic_sim::CycleRec *last = sim->cyc_pending.empty() ? nullptr : &sim->cyc_pending.back();
+        if (last && last->passes == smooth_passes && last->rho == rho_dev && last->phi == phi_dev &&
+            std::equal(last->w.begin(), last->w.end(), weights))
+            last->ncycles++;
+        else
+            sim->cyc_pending.push_back({1, std::vector<double>(weights, weights + ns), smooth_passes, rho_dev, phi_dev});
+        for (size_t i = 0; i < ns; ++i)
+            if (int rc = deposit_enqueue(sim->sp[i], weights[i], rho_dev, i > 0)) return rc;
+        if (int rc = solve_enqueue(sim, rho_dev, smooth_passes, phi_dev, sim->d_frozen)) return rc;
+    }
+    return PIC_OK;
 }
 
 extern "C" int pic_arrange_info(pic_species *s, int32_t *w_bound, int32_t *used_general)

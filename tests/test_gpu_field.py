@@ -222,3 +222,126 @@ def test_closed_pic_loop_against_the_oracle_loop(boundary_cfg):
                     rtol=1e-10, atol=1e-11)
     assert np.max(np.abs(E_o)) > 0
     pic.pic_destroy(sim)
+
+
+def _cycle_inputs(boundary_cfg, fast_vz=None):
+    inp = workloads.make(3, nc=1500) if boundary_cfg == 3 else workloads.make(1, nc=1024, ppc=64)
+    if fast_vz is not None:  # one particle whose gyration turns vz into a vx of more than one cell per step
+        s = inp["species"][0]
+        for k in ("vx", "vy", "vz"):
+            s[k] = s[k].copy()
+        s["vx"][7777], s["vy"][7777], s["vz"][7777] = 0.0, 0.0, fast_vz
+    ppc = len(inp["species"][0]["x"]) / inp["nc"]
+    w = 0.25 / ppc
+    return inp, [-w if s["qm"] < 0 else w for s in inp["species"]]
+
+
+def _make_sim(inp, options=None):
+    descs = [pic.make_species(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], qm=s["qm"], arrange_every=1) for s in inp["species"]]
+    sim = pic.pic_create(nc=inp["nc"], dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E_nodes=inp["E"], B=inp["B"],
+                         species=descs)
+    for k, v in (options or {}).items():
+        pic.pic_set_option(sim, k, v)
+    return sim
+
+
+def _checked_loop(sim, weights, ncycles, passes):
+    rho = None
+    for _ in range(ncycles):
+        rho = None
+        pic.pic_push_all(sim, 1)
+        for si, sp in enumerate(sim.species):
+            rho = pic.pic_deposit(sp, weights[si], rho=rho, accumulate=si > 0)
+        pic.pic_solve_field(sim, rho, smooth_passes=passes)
+    return rho
+
+
+def _assert_same_sims(a, b, rho_a, rho_b, where):
+    Ea, Eb = pic.pic_get_field(a), pic.pic_get_field(b)
+    assert np.array_equal(Ea, Eb), f"{where}: E differs (max {np.max(np.abs(Ea - Eb))} of {np.max(np.abs(Ea))})"
+    assert np.array_equal(rho_a.cpu().numpy(), rho_b.cpu().numpy()), f"{where}: rho differs"
+    for si, (sa, sb) in enumerate(zip(a.species, b.species)):
+        assert pic.pic_n_slots(sa) == pic.pic_n_slots(sb)
+        for ta, tb in zip(sa.state(), sb.state()):
+            assert np.array_equal(ta.cpu().numpy(), tb.cpu().numpy()), f"{where}: species {si} differs"
+        assert pic.pic_wall_flux(sa) == pic.pic_wall_flux(sb)
+        assert pic.pic_step_count(sa) == pic.pic_step_count(sb)
+
+
+@pytest.mark.parametrize("boundary_cfg", [3, 1])
+def test_pic_cycle_is_the_checked_loop_without_the_round_trips(boundary_cfg):
+    """pic_cycle (steps, depositions and field solves enqueued unchecked, one sync at the end) against the loop of
+    checked calls, bit for bit -- state, E, rho, walls -- and against the oracle's loop to rounding."""
+    inp, weights = _cycle_inputs(boundary_cfg)
+    nc, dx, boundary, passes = inp["nc"], inp["dx"], inp["boundary"], 2
+    a, b = _make_sim(inp), _make_sim(inp)
+    rho_a = _checked_loop(a, weights, 20, passes)
+    launches0 = pic.pic_launch_count(b)
+    rho_b, _ = pic.pic_cycle(b, 7, weights, smooth_passes=passes)
+    rho_b, phi_b = pic.pic_cycle(b, 13, weights, smooth_passes=passes, rho=rho_b, want_phi=True)
+    assert pic.pic_launch_count(b) > launches0
+    _assert_same_sims(a, b, rho_a, rho_b, f"pic_cycle, config {boundary_cfg}")
+    for sp in b.species:
+        info = pic.pic_fused_info(sp)
+        assert info["active"] == 1 and info["decline_reasons"] == 0, info
+    # the oracle's loop
+    states = [oracle.State(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], nc=nc, dx=dx, dt=inp["dt"], boundary=boundary,
+                           E=inp["E"].copy(), qm=s["qm"], B=inp["B"], arrange_every=1) for s in inp["species"]]
+    for _ in range(20):
+        rho_o = np.zeros(nc + 1)
+        for si, st in enumerate(states):
+            st.push(1)
+            rho_o = rho_o + st.deposit(weights[si])
+        _, phi_o, E_o = oracle.field_solve(rho_o, nc, dx, boundary, passes)
+        for st in states:
+            st.E[:] = E_o
+    pmax = np.max(np.abs(phi_o))
+    assert np.max(np.abs(pic.pic_get_field(b) - E_o)) <= 1e-11 * max(np.max(np.abs(E_o)), pmax / dx)
+    assert np.max(np.abs(phi_b.cpu().numpy() - phi_o)) <= 1e-10 * pmax
+    for si, (sp, st) in enumerate(zip(b.species, states)):
+        compare(sp, st, where=f"pic_cycle species {si}", bitwise=False, counts=True, nc=nc, rtol=1e-10, atol=1e-11)
+    # cycles interleaved with other calls: each of them settles the pending cycles first
+    pic.pic_cycle(b, 3, weights, smooth_passes=passes, rho=rho_b)
+    pic.pic_push(b.species[0], 1)
+    rho_a = _checked_loop(a, weights, 3, passes)
+    pic.pic_push(a.species[0], 1)
+    pic.pic_cycle(b, 2, weights, smooth_passes=passes, rho=rho_b)
+    rho_a = _checked_loop(a, weights, 2, passes)
+    _assert_same_sims(a, b, rho_a, rho_b, "pic_cycle interleaved with pic_push")
+    pic.pic_destroy(a)
+    pic.pic_destroy(b)
+
+
+@pytest.mark.parametrize("boundary_cfg,fast_vz", [(1, 30.0), (3, 30.0), (3, 45.0)])
+def test_pic_cycle_redoes_the_cycles_after_a_declined_step(boundary_cfg, fast_vz):
+    """A particle that jumps two cells after a few gyration steps: the fused step of that cycle declines on the device,
+    which freezes every species and the field; the next synchronising call redoes the cycles from there.  Result: that
+    of the checked loop (which meets the same decline and redoes the step at once), bit for bit."""
+    inp, weights = _cycle_inputs(boundary_cfg, fast_vz=fast_vz)
+    a, b = _make_sim(inp), _make_sim(inp)
+    rho_a = _checked_loop(a, weights, 16, 1)
+    rho_b, _ = pic.pic_cycle(b, 16, weights, smooth_passes=1)
+    _assert_same_sims(a, b, rho_a, rho_b, f"pic_cycle with a decline, config {boundary_cfg}")
+    info = pic.pic_fused_info(b.species[0])
+    assert info["decline_reasons"] & 1, info
+    assert pic.pic_step_count(b.species[0]) == 16 and pic.pic_step_count(b.species[-1]) == 16
+    # and on from there (the declined species now runs the split kernels: every cycle is the checked calls)
+    rho_a = _checked_loop(a, weights, 4, 1)
+    rho_b, _ = pic.pic_cycle(b, 4, weights, smooth_passes=1, rho=rho_b)
+    _assert_same_sims(a, b, rho_a, rho_b, "pic_cycle after the decline")
+    pic.pic_destroy(a)
+    pic.pic_destroy(b)
+
+
+def test_pic_cycle_arguments():
+    inp, weights = _cycle_inputs(1)
+    sim = _make_sim(inp)
+    with pytest.raises(pic.PicError):
+        pic.pic_cycle(sim, -1, weights)
+    with pytest.raises(pic.PicError):
+        pic.pic_cycle(sim, 1, [float("nan")] * len(weights))
+    with pytest.raises(pic.PicError):
+        pic.pic_cycle(sim, 1, weights, smooth_passes=5000)
+    pic.pic_cycle(sim, 0, weights)
+    pic.pic_sync(sim)
+    pic.pic_destroy(sim)
