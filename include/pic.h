@@ -115,7 +115,7 @@ int pic_push(pic_species *sp, int nsteps);
 
 /* nsteps mover steps of EVERY species of the sim (step by step, species by species: the result is that of
  * pic_push(sp, nsteps) on each).  The species of a step are independent -- they share only the field, which they read
- * (the paper's loop over species inside the mover; SURVEY.md section 8(e) "two streams on one GPU") -- so
+ * (the paper's mover runs over x[species][cell][particle]; SURVEY.md section 8(e) "two streams on one GPU") -- so
  * each species runs on an internal stream of its own for the duration of the call and their kernels overlap; fork and
  * join are events, on return all of it is ordered on the sim's stream.  Option "species_streams" = 0 runs them back to
  * back on the sim's stream instead.  Asynchronous.  Errors: as pic_push. */
