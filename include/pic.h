@@ -223,11 +223,16 @@ size_t pic_workspace_bytes(int32_t nc, int64_t capacity);
  * "fused_cells_per_cta" (cells per chunk, 1..256; 0 = automatic), "fused_rows" (rows
  * of 32 slots per tile: 8, 12 or 16; 0 = automatic from the largest per-cell count),
  * "fused_stage_slots" (largest tile in slots, even, <= 32*rows; 0 = 32*rows), "fused_stages"
- * (stages of the TMA ring: 1 or 2; 0 = automatic: 2 under 8-row tiles, else 1), "fused_pdl" (1 = the streaming
- * kernel is launched with programmatic dependent launch and overlaps its prologue with the edge kernel, default;
+ * (stages of the TMA ring: 1 or 2; 0 = automatic: 2 under 8-row tiles, else 1), "fused_pdl" (1 = the three kernels
+ * of a step are programmatic dependent launches: the streaming kernel overlaps its prologue with the edge kernel, the
+ * commit kernel and the next step's edge kernel are set up while their predecessor runs, default;
  * 0 = plain stream order), "fused_taper" (0..3: how many times the chunk size is halved towards the end of the grid, one
  * machine-load of CTAs per size, so that the CTAs that run last are short; -1 = automatic, default: 64-cell chunks
- * tapered three times on grids of four or more waves, no taper on smaller ones).  Results never depend on any of them.
+ * tapered three times on grids of four or more waves, no taper on smaller ones).  Other flags: "species_streams"
+ * (pic_push_all: 1 = every species on an internal stream of its own, default), "cycle_async" (pic_cycle: 1 = no host
+ * check between the calls of a cycle, default), "field_fused" (pic_solve_field: 1 = one cooperative kernel, default;
+ * 0 = six or seven separate kernels, bit-identical), "field_blocks_per_sm" (0 = automatic, 1..8: resident blocks per SM
+ * of that kernel).  Results never depend on any of them.
  * PIC_EINVAL for an unknown key or a value out of range. */
 int pic_set_option(pic_sim *sim, const char *key, int value);
 

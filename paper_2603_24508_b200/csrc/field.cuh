@@ -23,6 +23,7 @@
 // On a periodic grid rho is neutralised first (uniform background) and phi is returned with zero mean; the gauge
 // phi[0] = 0 used in between satisfies node 0's equation by itself because the neutralised rho sums to zero.
 #pragma once
+#include <cooperative_groups.h>
 #include "pic_device.cuh"
 
 namespace pic {
@@ -75,10 +76,10 @@ struct FieldArgs {
 };
 
 // one pass of the 1-2-1 filter (S27, S28): ((left + 2*centre) + right) * 0.25
-__global__ void __launch_bounds__(FLD_THREADS) field_smooth_kernel(const double *__restrict__ in, double *__restrict__ out, int nc,
-                                                                   int periodic)
+__device__ __forceinline__ void field_smooth_block(const double *__restrict__ in, double *__restrict__ out, int nc, int periodic,
+                                                   int vb)
 {
-    const int j = blockIdx.x * FLD_THREADS + threadIdx.x;
+    const int j = vb * FLD_THREADS + threadIdx.x;
     if (j > nc) return;
     double left, right, centre;
     if (periodic) {
@@ -93,6 +94,12 @@ __global__ void __launch_bounds__(FLD_THREADS) field_smooth_kernel(const double 
     }
     const double t = __dmul_rn(2.0, centre);
     out[j] = __dmul_rn(__dadd_rn(__dadd_rn(left, t), right), 0.25);
+}
+
+__global__ void __launch_bounds__(FLD_THREADS) field_smooth_kernel(const double *__restrict__ in, double *__restrict__ out, int nc,
+                                                                   int periodic)
+{
+    field_smooth_block(in, out, nc, periodic, blockIdx.x);
 }
 
 // block-wide sum with a fixed tree (warp shuffles, then warp 0 over the warp sums)
@@ -131,10 +138,12 @@ __device__ __forceinline__ FieldDD fld_dd_add(FieldDD a, FieldDD b)
 }
 
 // per tile: double-double sum of rho over the distinct nodes 0..nc-1 (only needed on a periodic grid)
-__global__ void __launch_bounds__(FLD_THREADS) field_sum_kernel(FieldArgs a)
+// (vb = the tile, nvb = number of tiles: blockIdx.x / gridDim.x of field_sum_kernel, or the virtual block of the
+// one-kernel solve; the same holds for the other *_block functions below)
+__device__ __forceinline__ void field_sum_block(const FieldArgs &a, int vb, int nvb)
 {
     __shared__ FieldDD s_w[FLD_THREADS / 32];
-    const int base = blockIdx.x * FLD_TILE + threadIdx.x * FLD_ITEMS;
+    const int base = vb * FLD_TILE + threadIdx.x * FLD_ITEMS;
     FieldDD v{0.0, 0.0};
 #pragma unroll
     for (int q = 0; q < FLD_ITEMS; ++q)
@@ -154,10 +163,10 @@ __global__ void __launch_bounds__(FLD_THREADS) field_sum_kernel(FieldArgs a)
     if (threadIdx.x == 0) {
         FieldDD r{0.0, 0.0};
         for (int w = 0; w < FLD_THREADS / 32; ++w) r = fld_dd_add(r, s_w[w]);
-        a.tile_sum[blockIdx.x] = r.hi;
-        a.tile_lo[blockIdx.x] = r.lo;
+        a.tile_sum[vb] = r.hi;
+        a.tile_lo[vb] = r.lo;
         __threadfence();
-        s_last = atomicAdd(a.ticket, 1u) == gridDim.x - 1;
+        s_last = atomicAdd(a.ticket, 1u) == (unsigned)nvb - 1u;
     }
     __syncthreads();
     if (s_last) { // the last tile to arrive adds the tile sums: every thread a fixed subset, then a fixed tree
@@ -187,6 +196,8 @@ __global__ void __launch_bounds__(FLD_THREADS) field_sum_kernel(FieldArgs a)
         }
     }
 }
+
+__global__ void __launch_bounds__(FLD_THREADS) field_sum_kernel(FieldArgs a) { field_sum_block(a, blockIdx.x, gridDim.x); }
 
 // r[j] of the solve: dx^2 (rho[j] - mean) on the unknown nodes 1..nc-1, zero elsewhere; mean = mhi + mlo
 __device__ __forceinline__ double fld_r(const FieldArgs &a, int j, double mhi, double mlo)
@@ -227,24 +238,26 @@ __device__ __forceinline__ FieldSeg fld_tile_scan(const double (&r)[FLD_ITEMS], 
     return fld_combine(wpre, ex);
 }
 
-__global__ void __launch_bounds__(FLD_THREADS) field_tile_kernel(FieldArgs a)
+__device__ __forceinline__ void field_tile_block(const FieldArgs &a, int vb)
 {
     __shared__ FieldSeg s_w[FLD_THREADS / 32];
     const FieldDD mean{a.scal[0], a.scal[3]}; // zero on a bounded grid; written by field_sum_kernel on a periodic one
-    const int base = blockIdx.x * FLD_TILE + threadIdx.x * FLD_ITEMS;
+    const int base = vb * FLD_TILE + threadIdx.x * FLD_ITEMS;
     double r[FLD_ITEMS];
 #pragma unroll
     for (int q = 0; q < FLD_ITEMS; ++q) r[q] = fld_r(a, base + q, mean.hi, mean.lo);
     FieldSeg total;
     fld_tile_scan(r, s_w, total);
     if (threadIdx.x == 0) {
-        a.tile_s[blockIdx.x] = total.s;
-        a.tile_t[blockIdx.x] = total.t;
+        a.tile_s[vb] = total.s;
+        a.tile_t[vb] = total.t;
     }
 }
 
+__global__ void __launch_bounds__(FLD_THREADS) field_tile_kernel(FieldArgs a) { field_tile_block(a, blockIdx.x); }
+
 // One block: exclusive scan of the tile aggregates in tile order (every tile is FLD_TILE nodes long), then F.
-__global__ void __launch_bounds__(FLD_THREADS) field_chain_kernel(FieldArgs a)
+__device__ __forceinline__ void field_chain_block(const FieldArgs &a)
 {
     __shared__ FieldSeg s_w[FLD_THREADS / 32];
     __shared__ FieldSeg s_carry;
@@ -291,19 +304,21 @@ __global__ void __launch_bounds__(FLD_THREADS) field_chain_kernel(FieldArgs a)
     }
 }
 
+__global__ void __launch_bounds__(FLD_THREADS) field_chain_kernel(FieldArgs a) { field_chain_block(a); }
+
 // per tile: phi[j] = j*F - T[j], T[j] = sum of S over the nodes before j (exclusive); per-tile sum of phi
-__global__ void __launch_bounds__(FLD_THREADS) field_phi_kernel(FieldArgs a)
+__device__ __forceinline__ void field_phi_block(const FieldArgs &a, int vb, int nvb)
 {
     __shared__ FieldSeg s_w[FLD_THREADS / 32];
     __shared__ double s_sum[FLD_THREADS / 32];
     const double mhi = a.scal[0], mlo = a.scal[3], F = a.scal[1];
-    const int base = blockIdx.x * FLD_TILE + threadIdx.x * FLD_ITEMS;
+    const int base = vb * FLD_TILE + threadIdx.x * FLD_ITEMS;
     double r[FLD_ITEMS];
 #pragma unroll
     for (int q = 0; q < FLD_ITEMS; ++q) r[q] = fld_r(a, base + q, mhi, mlo);
     FieldSeg total;
     const FieldSeg ex = fld_tile_scan(r, s_w, total);
-    const FieldSeg tpre{a.tile_s[blockIdx.x], a.tile_t[blockIdx.x], (double)blockIdx.x * (double)FLD_TILE};
+    const FieldSeg tpre{a.tile_s[vb], a.tile_t[vb], (double)vb * (double)FLD_TILE};
     const FieldSeg pre = fld_combine(tpre, ex); // all nodes before `base`: pre.s = S[base-1], pre.t = sum_{m<base} S[m]
     double S = pre.s, T = pre.t, psum = 0.0;
 #pragma unroll
@@ -321,9 +336,9 @@ __global__ void __launch_bounds__(FLD_THREADS) field_phi_kernel(FieldArgs a)
     psum = fld_block_sum(psum, s_sum);
     __shared__ int s_last;
     if (threadIdx.x == 0) {
-        a.tile_sum[blockIdx.x] = psum;
+        a.tile_sum[vb] = psum;
         __threadfence();
-        s_last = atomicAdd(a.ticket + 1, 1u) == gridDim.x - 1;
+        s_last = atomicAdd(a.ticket + 1, 1u) == (unsigned)nvb - 1u;
     }
     __syncthreads();
     if (s_last) { // last tile: the mean of phi (the gauge of a periodic grid), by a fixed tree over the tile sums
@@ -339,8 +354,10 @@ __global__ void __launch_bounds__(FLD_THREADS) field_phi_kernel(FieldArgs a)
     }
 }
 
+__global__ void __launch_bounds__(FLD_THREADS) field_phi_kernel(FieldArgs a) { field_phi_block(a, blockIdx.x, gridDim.x); }
+
 // E from phi (S26), gauge shift on a periodic grid (S25), max |E|, optional copy of phi
-__global__ void __launch_bounds__(FLD_THREADS) field_e_kernel(FieldArgs a)
+__device__ __forceinline__ void field_e_block(const FieldArgs &a, int vb)
 {
     __shared__ unsigned long long s_max;
     if (threadIdx.x == 0) s_max = 0ull;
@@ -348,7 +365,7 @@ __global__ void __launch_bounds__(FLD_THREADS) field_e_kernel(FieldArgs a)
     if (a.frozen && *(volatile const int *)a.frozen) return; // block-uniform
     const double pm = a.scal[2]; // zero on a bounded grid
     const int nc = a.nc;
-    const int j = blockIdx.x * FLD_THREADS + threadIdx.x;
+    const int j = vb * FLD_THREADS + threadIdx.x;
     double e = 0.0;
     if (j <= nc) {
         const double mh = -0.5 * a.inv_dx, m1 = -a.inv_dx;
@@ -377,6 +394,54 @@ __global__ void __launch_bounds__(FLD_THREADS) field_e_kernel(FieldArgs a)
     if ((threadIdx.x & 31) == 0 && b) atomicMax(&s_max, b);
     __syncthreads();
     if (threadIdx.x == 0 && s_max > *(volatile unsigned long long *)a.emax_bits) atomicMax(a.emax_bits, s_max);
+}
+
+__global__ void __launch_bounds__(FLD_THREADS) field_e_kernel(FieldArgs a) { field_e_block(a, blockIdx.x); }
+
+// The whole solve as ONE cooperative kernel: the phases above, run by a grid of resident blocks that walk the virtual
+// blocks of each phase and meet at a grid-wide barrier between phases.  The data is 0.5 - 24 MB and every phase a few
+// microseconds: as six or seven launches the solve is launch latency (35 us at 65 K nodes of which 24 us are kernels).
+// Same block-level code, same fixed summation trees, same tickets: bit-identical to the separate kernels.
+// rho_in: the charge density as deposited; f0 / f1: the filter's ping-pong arrays; a.rho is set here to whichever array
+// holds the filtered density.  emax_bits is cleared here (the separate-kernel path uses a memset).
+__global__ void __launch_bounds__(FLD_THREADS) field_solve_kernel(FieldArgs a, const double *rho_in, double *f0, double *f1, int passes)
+{
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    const int nc = a.nc;
+    const int nblk = (nc + 1 + FLD_THREADS - 1) / FLD_THREADS;
+    const int G = (int)gridDim.x;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *a.emax_bits = 0ull;
+    const double *cur = rho_in;
+    for (int p = 0; p < passes; ++p) {
+        double *out = (p & 1) ? f1 : f0;
+        for (int vb = blockIdx.x; vb < nblk; vb += G) field_smooth_block(cur, out, nc, a.periodic, vb);
+        grid.sync();
+        cur = out;
+    }
+    a.rho = cur;
+    if (a.periodic) {
+        for (int vb = blockIdx.x; vb < a.ntiles; vb += G) {
+            field_sum_block(a, vb, a.ntiles);
+            __syncthreads(); // the block's shared arrays are reused by its next virtual block
+        }
+        grid.sync();
+    }
+    for (int vb = blockIdx.x; vb < a.ntiles; vb += G) {
+        field_tile_block(a, vb);
+        __syncthreads();
+    }
+    grid.sync();
+    if (blockIdx.x == 0) field_chain_block(a);
+    grid.sync();
+    for (int vb = blockIdx.x; vb < a.ntiles; vb += G) {
+        field_phi_block(a, vb, a.ntiles);
+        __syncthreads();
+    }
+    grid.sync();
+    for (int vb = blockIdx.x; vb < nblk; vb += G) {
+        field_e_block(a, vb);
+        __syncthreads();
+    }
 }
 
 // max |E| of a field array handed over on the device (pic_set_field_device)

@@ -116,7 +116,8 @@ struct pic_sim {
     bool in_cycle = false;         // push_fused hands d_frozen to its kernels
     std::vector<pic_species *> sp;
     unsigned long long launches = 0;
-    int opt_fused = 1, opt_timing = 0, opt_tile_scatter = 1, opt_fused_tma = 1, opt_fused_pdl = 1, opt_fused_taper = -1, opt_species_streams = 1, opt_cycle_async = 1;
+    int opt_fused = 1, opt_timing = 0, opt_tile_scatter = 1, opt_fused_tma = 1, opt_fused_pdl = 1, opt_fused_taper = -1, opt_species_streams = 1, opt_cycle_async = 1, opt_field_fused = 1, opt_field_bps = 0;
+    int field_grid_max = 0; // resident blocks of field_solve_kernel (cooperative launch)
     int opt_fused_cpc = 0, opt_fused_rows = 0, opt_fused_slots = 0, opt_fused_stages = 0; // tuning knobs of the fused step (0 = automatic)
     int sm_count = 148;
     // per-kernel device timing (option "kernel_timing"): event pairs recorded around launches
@@ -637,15 +638,8 @@ static int solve_enqueue(pic_sim *sim, const double *rho_dev, int smooth_passes,
     const int nc = sim->nc;
     const int nblk = (nc + 1 + FLD_THREADS - 1) / FLD_THREADS;
     KernelSpan span(sim, K_FIELD);
-    const double *rho = rho_dev;
-    for (int p = 0; p < smooth_passes; ++p) {
-        double *out = sim->d_f[p & 1];
-        field_smooth_kernel<<<nblk, FLD_THREADS, 0, sim->stream>>>(rho, out, nc, sim->periodic);
-        if (int rc = launch_check(sim, "field_smooth_kernel")) return rc;
-        rho = out;
-    }
     FieldArgs a{};
-    a.rho = rho; a.phi = sim->d_phi; a.E = sim->d_E; a.phi_out = phi_dev;
+    a.phi = sim->d_phi; a.E = sim->d_E; a.phi_out = phi_dev;
     a.ntiles = fld_ntiles(nc);
     a.tile_s = sim->d_tile; a.tile_t = sim->d_tile + a.ntiles; a.tile_sum = sim->d_tile + 2 * (size_t)a.ntiles;
     a.tile_lo = sim->d_tile + 3 * (size_t)a.ntiles;
@@ -654,6 +648,33 @@ static int solve_enqueue(pic_sim *sim, const double *rho_dev, int smooth_passes,
     a.nc = nc; a.periodic = sim->periodic;
     a.frozen = frozen;
     { volatile double d2 = sim->dx * sim->dx; a.dx2 = d2; volatile double inv = 1.0 / sim->dx; a.inv_dx = inv; }
+    if (sim->opt_field_fused) {
+        // one cooperative kernel: a grid of resident blocks walks the phases and meets at grid-wide barriers
+        if (sim->field_grid_max == 0) {
+            int per_sm = 0;
+            CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, field_solve_kernel, FLD_THREADS, 0));
+            sim->field_grid_max = std::max(1, per_sm * sim->sm_count);
+        }
+        // blocks per SM: the barrier costs more with more blocks, the phases less
+        const int want = sim->opt_field_bps ? sim->opt_field_bps : (nc > 400000 ? 4 : 1);
+        int grid = std::max(1, std::min(std::min(sim->field_grid_max, want * sim->sm_count), nblk));
+        const double *rho_in = rho_dev;
+        double *f0 = sim->d_f[0], *f1 = sim->d_f[1];
+        int passes = smooth_passes;
+        void *args[] = {&a, &rho_in, &f0, &f1, &passes};
+        CU(cudaLaunchCooperativeKernel((const void *)field_solve_kernel, dim3((unsigned)grid), dim3(FLD_THREADS), args, 0, sim->stream));
+        if (int rc = launch_check(sim, "field_solve_kernel")) return rc;
+        sim->emax_known = false;
+        return PIC_OK;
+    }
+    const double *rho = rho_dev;
+    for (int p = 0; p < smooth_passes; ++p) {
+        double *out = sim->d_f[p & 1];
+        field_smooth_kernel<<<nblk, FLD_THREADS, 0, sim->stream>>>(rho, out, nc, sim->periodic);
+        if (int rc = launch_check(sim, "field_smooth_kernel")) return rc;
+        rho = out;
+    }
+    a.rho = rho;
     CU(cudaMemsetAsync(sim->d_emax, 0, sizeof(unsigned long long), sim->stream));
     if (sim->periodic) {
         field_sum_kernel<<<a.ntiles, FLD_THREADS, 0, sim->stream>>>(a);
@@ -692,6 +713,8 @@ extern "C" int pic_set_option(pic_sim *sim, const char *key, int value)
     else if (!strcmp(key, "fused_pdl") && flag) sim->opt_fused_pdl = value;
     else if (!strcmp(key, "species_streams") && flag) sim->opt_species_streams = value;
     else if (!strcmp(key, "cycle_async") && flag) sim->opt_cycle_async = value;
+    else if (!strcmp(key, "field_fused") && flag) sim->opt_field_fused = value;
+    else if (!strcmp(key, "field_blocks_per_sm") && value >= 0 && value <= 8) sim->opt_field_bps = value;
     else if (!strcmp(key, "fused_taper") && value >= -1 && value < FUSED_SEGS) sim->opt_fused_taper = value;
     else if (!strcmp(key, "fused_cells_per_cta") && value >= 0 && value <= FUSED_CPC_MAX) sim->opt_fused_cpc = value;
     else if (!strcmp(key, "fused_stage_slots") && value >= 0 && value <= 512 && value % 2 == 0) sim->opt_fused_slots = value;

@@ -88,6 +88,25 @@ def test_solve_field_at_config4_size_and_repeatable(boundary):
 
 
 @pytest.mark.parametrize("boundary", [workloads.PERIODIC, workloads.ABSORBING])
+@pytest.mark.parametrize("nc", [2, 17, 2049, 70001, 1_000_000])
+def test_one_kernel_solve_equals_the_separate_kernels(nc, boundary):
+    """The solve as one cooperative kernel (default) against the same phases as six or seven launches (option
+    field_fused = 0): the same block-level code and summation trees, so phi, E and max|E| agree bit for bit; the
+    separate kernels are also checked against the oracle here (the other tests run the default)."""
+    rng = np.random.default_rng(5000 + nc)
+    dx = 0.5
+    a, b = _tiny_sim(nc, boundary, dx), _tiny_sim(nc, boundary, dx)
+    pic.pic_set_option(b, "field_fused", 0)
+    for name, rho in list(_rho_cases(nc, boundary, rng).items())[:3]:
+        for passes in (0, 2, 3):
+            phi_a, E_a = _check_fields(a, rho, nc, dx, boundary, passes, f"one kernel nc={nc} {name} passes={passes}")
+            phi_b, E_b = _check_fields(b, rho, nc, dx, boundary, passes, f"separate kernels nc={nc} {name} passes={passes}")
+            assert np.array_equal(phi_a, phi_b) and np.array_equal(E_a, E_b)
+    pic.pic_destroy(a)
+    pic.pic_destroy(b)
+
+
+@pytest.mark.parametrize("boundary", [workloads.PERIODIC, workloads.ABSORBING])
 def test_filter_alone_is_bitwise(boundary):
     """E of a solve with k passes == E of a solve without passes fed the oracle's filtered rho: bit for bit, which
     holds only if the device filter produced exactly the oracle's filtered values."""
