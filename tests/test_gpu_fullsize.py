@@ -166,3 +166,38 @@ def test_fullsize_whole_run_elementwise(config, single_thread_too):
         assert pic.pic_fused_info(sp)["decline_reasons"] == 0, "a fused step declined at full size"
         del st
     pic.pic_destroy(sim)
+
+
+# ---- beyond the configs: particle arrays larger than 2 GiB (maximum sizes) -----------------------------------------------
+def test_arrays_beyond_2_gib_elementwise():
+    """280 M electrons on 2.8 M periodic cells (config 4's shape, 2.8 times its size): every fp64 array is 2.24 GB, so a
+    byte offset no longer fits 31 bits and a slot index approaches 2^28 -- the sizes where 32-bit address arithmetic
+    would first go wrong.  Two fused steps, then (option fused = 0) one step of the split kernels (mover, tile-ranked
+    scatter) and the deposition, each compared element by element with the threaded oracle."""
+    inp = workloads.make(4, nc=2_800_000)
+    s = inp["species"][0]
+    n0 = len(s["x"])
+    assert n0 * 8 > 2**31
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        desc = pic.make_species(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], qm=s["qm"], arrange_every=1)
+    stream.synchronize()
+    sim = pic.pic_create(nc=inp["nc"], dx=inp["dx"], dt=inp["dt"], boundary=inp["boundary"], E_nodes=inp["E"], B=inp["B"],
+                         species=[desc], stream=stream)
+    st = oracle.State(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], nc=inp["nc"], dx=inp["dx"], dt=inp["dt"],
+                      boundary=inp["boundary"], E=inp["E"], qm=s["qm"], B=inp["B"], arrange_every=1, threads=0)
+    sp = sim.species[0]
+    pic.pic_push_all(sim, 2)
+    st.push(2)
+    compare(sp, st, where="280 M particles, two fused steps", counts=True, nc=inp["nc"])
+    info = pic.pic_fused_info(sp)
+    assert info["active"] == 1 and info["decline_reasons"] == 0, info
+    pic.pic_set_option(sim, "fused", 0)
+    pic.pic_push(sp, 1)
+    st.push(1)
+    compare(sp, st, where="280 M particles, one step of the split kernels", counts=True, nc=inp["nc"])
+    assert pic.pic_arrange_info(sp)[1] == 0, "fell to the general arranger"
+    rho = pic.pic_deposit(sp, -1.0).cpu().numpy()
+    ref = st.deposit(-1.0)
+    assert np.all(np.abs(rho - ref) <= 1e-12 * np.maximum(np.abs(ref), 1.0))
+    pic.pic_destroy(sim)
