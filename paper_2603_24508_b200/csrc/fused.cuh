@@ -448,8 +448,8 @@ __device__ __forceinline__ void fused_sweep1a(const PushConst &k, const double *
 // Row groups of the sweeps.  Width 0: rows 4 by 4 while at least four more can follow, then 2, 1, 1 (for RMAX = 8:
 // {0-3} {4,5} {6} {7}; a tile pushes at most one surplus row).  Width W > 0: groups of W rows ({0-3} {4-7}).  A group
 // runs if its first row is inside the tile; rows of it behind the tile are masked out (class X, nothing stored), so
-// that a group is straight-line code whose rows' dependency chains interleave.  The kernel is bound by the latency of
-// these chains, not by issue slots: fewer, wider groups win although they push more surplus rows.
+// that a group is straight-line code whose rows' dependency chains interleave.  (Width 4 everywhere measured equal at
+// config 4 and 8 % slower at config 2, where the surplus rows count: profiles/r02_variants.md.)
 #ifndef FUSED_W1A
 #define FUSED_W1A 0 // sweep 1a (and the loads)
 #endif
