@@ -25,7 +25,8 @@
  *
  * All functions return PIC_OK (0) or a negative pic_status; nothing throws or aborts.
  * Work is enqueued on the stream given at pic_create; calls documented "syncs" wait for
- * it.  One host thread per pic_sim.  There is no CPU fallback: without a CUDA device
+ * it.  One host thread per pic_sim at a time; different sims may be driven from different threads
+ * (what they share -- the memory pool of pic_trim_memory -- is locked).  There is no CPU fallback: without a CUDA device
  * every compute entry point fails with PIC_ECUDA.
  */
 #ifndef PIC_H_

@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -166,25 +167,36 @@ static cudaMemPool_t g_pool[64] = {};
 static std::vector<void *> g_pinned_free; // pinned DevState blocks of destroyed species (telemetry), reused
 // The arena of pic_run_host (gigabytes: two buffer sets and the workspace of every species) is a plain cudaMalloc
 // kept for the next call -- growing a memory pool by 9 GB took 1.15 s against 1-2 ms for cudaMalloc.
-static struct { char *p; size_t bytes; } g_arena[64] = {};
+static struct { char *p; size_t bytes; bool in_use; } g_arena[64] = {};
+
+static std::mutex g_mem_mu; // guards g_pool / g_pinned_free / g_arena (sims of different threads share them)
+static bool g_pool_broken[64] = {}; // the device or driver has no memory pools: plain cudaMalloc from then on
 
 static cudaError_t dev_alloc(void **p, size_t bytes, int device, cudaStream_t st)
 {
     *p = nullptr;
-    if (device < 0 || device >= 64) return cudaMalloc(p, bytes);
-    if (!g_pool[device]) {
-        cudaMemPoolProps props{};
-        props.allocType = cudaMemAllocationTypePinned;
-        props.handleTypes = cudaMemHandleTypeNone;
-        props.location.type = cudaMemLocationTypeDevice;
-        props.location.id = device;
-        cudaError_t e = cudaMemPoolCreate(&g_pool[device], &props);
-        if (e != cudaSuccess) { g_pool[device] = nullptr; return e; }
-        unsigned long long keep = ~0ull;
-        e = cudaMemPoolSetAttribute(g_pool[device], cudaMemPoolAttrReleaseThreshold, &keep);
-        if (e != cudaSuccess) return e;
+    cudaMemPool_t pool = nullptr;
+    if (device >= 0 && device < 64) {
+        std::lock_guard<std::mutex> lock(g_mem_mu);
+        if (!g_pool[device] && !g_pool_broken[device]) {
+            cudaMemPoolProps props{};
+            props.allocType = cudaMemAllocationTypePinned;
+            props.handleTypes = cudaMemHandleTypeNone;
+            props.location.type = cudaMemLocationTypeDevice;
+            props.location.id = device;
+            unsigned long long keep = ~0ull;
+            if (cudaMemPoolCreate(&g_pool[device], &props) != cudaSuccess ||
+                cudaMemPoolSetAttribute(g_pool[device], cudaMemPoolAttrReleaseThreshold, &keep) != cudaSuccess) {
+                cudaGetLastError();
+                if (g_pool[device]) cudaMemPoolDestroy(g_pool[device]);
+                g_pool[device] = nullptr;
+                g_pool_broken[device] = true;
+            }
+        }
+        pool = g_pool[device];
     }
-    return cudaMallocFromPoolAsync(p, bytes ? bytes : 16, g_pool[device], st);
+    if (!pool) return cudaMalloc(p, bytes ? bytes : 16); // dev_free's cudaFreeAsync takes these too
+    return cudaMallocFromPoolAsync(p, bytes ? bytes : 16, pool, st);
 }
 
 template <typename T>
@@ -203,8 +215,9 @@ extern "C" int pic_trim_memory(void)
     int dev = 0;
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceSynchronize());
+    std::lock_guard<std::mutex> lock(g_mem_mu);
     if (dev >= 0 && dev < 64 && g_pool[dev]) CU(cudaMemPoolTrimTo(g_pool[dev], 0));
-    if (dev >= 0 && dev < 64 && g_arena[dev].p) {
+    if (dev >= 0 && dev < 64 && g_arena[dev].p && !g_arena[dev].in_use) {
         CU(cudaFree(g_arena[dev].p));
         g_arena[dev].p = nullptr;
         g_arena[dev].bytes = 0;
@@ -243,7 +256,10 @@ static void free_species(pic_species *s)
     for (int b = 0; b < 2; ++b) { dev_free(s->d_count[b], st); dev_free(s->d_off[b], st); }
     dev_free(s->d_scan, st);
     dev_free(s->d_cs, st);
-    if (s->h_tel) g_pinned_free.push_back(s->h_tel);
+    if (s->h_tel) {
+        std::lock_guard<std::mutex> lock(g_mem_mu);
+        g_pinned_free.push_back(s->h_tel);
+    }
     if (s->tel_ev) cudaEventDestroy(s->tel_ev);
     if (s->join_ev) cudaEventDestroy(s->join_ev);
     if (s->own_stream) cudaStreamDestroy(s->own_stream);
@@ -441,8 +457,11 @@ static int alloc_species(pic_sim *sim, const pic_species_desc &d, pic_species **
     long long max_scan = std::max<long long>((long long)nc + 1, general_scan_elems(d.capacity));
     s->scan_words = scan_scratch_words(max_scan);
     CU(dev_alloc(&s->d_scan, s->scan_words * sizeof(unsigned long long), sim->device, sim->stream));
-    if (!g_pinned_free.empty()) { s->h_tel = static_cast<DevState *>(g_pinned_free.back()); g_pinned_free.pop_back(); }
-    else CU(cudaMallocHost(&s->h_tel, sizeof(DevState)));
+    {
+        std::lock_guard<std::mutex> lock(g_mem_mu);
+        if (!g_pinned_free.empty()) { s->h_tel = static_cast<DevState *>(g_pinned_free.back()); g_pinned_free.pop_back(); }
+    }
+    if (!s->h_tel) CU(cudaMallocHost(&s->h_tel, sizeof(DevState)));
     CU(cudaEventCreateWithFlags(&s->tel_ev, cudaEventDisableTiming));
     return PIC_OK;
 }
@@ -1546,6 +1565,7 @@ extern "C" int pic_run_host(const pic_grid_desc *g, pic_host_species *hs, int ns
     pic_sim *sim = nullptr;
     char *arena = nullptr;
     bool arena_cached = false;
+    int arena_device = -1;
     cudaStream_t copy_stream = nullptr;
     auto align256 = [](size_t b) { return (b + 255) & ~(size_t)255; };
     do {
@@ -1560,18 +1580,30 @@ extern "C" int pic_run_host(const pic_grid_desc *g, pic_host_species *hs, int ns
         if (rc) break;
         int device = 0;
         cudaGetDevice(&device);
-        const bool cacheable = device >= 0 && device < 64;
         cudaError_t e = cudaSuccess;
-        if (cacheable && g_arena[device].p && g_arena[device].bytes >= total) {
-            arena = g_arena[device].p; // the previous call's arena (pic_trim_memory releases it)
-        } else {
-            if (cacheable && g_arena[device].p) { cudaFree(g_arena[device].p); g_arena[device].p = nullptr; g_arena[device].bytes = 0; }
-            e = cudaMalloc(&arena, total ? total : 256);
-            if (e != cudaSuccess) { cudaGetLastError(); arena = nullptr; rc = PIC_ENOMEM; break; }
-            if (cacheable) { g_arena[device].p = arena; g_arena[device].bytes = total ? total : 256; }
-            arena_cached = cacheable;
+        {   // the previous call's arena if it is large enough and free (a concurrent call of another thread gets its own)
+            std::lock_guard<std::mutex> lock(g_mem_mu);
+            if (device >= 0 && device < 64 && !g_arena[device].in_use) {
+                if (g_arena[device].p && g_arena[device].bytes < total) {
+                    cudaFree(g_arena[device].p);
+                    g_arena[device].p = nullptr;
+                    g_arena[device].bytes = 0;
+                }
+                if (!g_arena[device].p) {
+                    e = cudaMalloc(&g_arena[device].p, total ? total : 256);
+                    if (e != cudaSuccess) g_arena[device].p = nullptr;
+                    else g_arena[device].bytes = total ? total : 256;
+                }
+                if (g_arena[device].p) {
+                    arena = g_arena[device].p;
+                    g_arena[device].in_use = true;
+                    arena_cached = true;
+                    arena_device = device;
+                }
+            }
         }
-        arena_cached = cacheable;
+        if (!arena && e == cudaSuccess) e = cudaMalloc(&arena, total ? total : 256);
+        if (e != cudaSuccess || !arena) { cudaGetLastError(); arena = nullptr; rc = PIC_ENOMEM; break; }
         mark("device arena allocated");
         size_t off = 0;
         auto carve = [&](size_t bytes) { void *p = arena + off; off += bytes; return p; };
@@ -1641,7 +1673,11 @@ extern "C" int pic_run_host(const pic_grid_desc *g, pic_host_species *hs, int ns
     if (sim) pic_destroy(sim);
     else cudaStreamSynchronize(stream);
     mark("sim destroyed");
-    if (arena && !arena_cached) cudaFree(arena); // else: kept for the next call
+    if (arena && !arena_cached) cudaFree(arena);
+    if (arena_cached) { // kept for the next call
+        std::lock_guard<std::mutex> lock(g_mem_mu);
+        g_arena[arena_device].in_use = false;
+    }
     mark("arena released");
     return rc;
 }
