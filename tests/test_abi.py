@@ -61,4 +61,8 @@ def test_argument_validation_without_gpu():
     assert L.pic_wall_flux(None, None) == pic.PIC_EINVAL
     assert L.pic_sync(None) == pic.PIC_EINVAL
     assert L.pic_run_host(None, None, 0, 0) == pic.PIC_EINVAL
+    assert L.pic_push_all(None, 1) == pic.PIC_EINVAL
+    assert L.pic_cycle(None, 1, None, 0, None, None) == pic.PIC_EINVAL
+    assert L.pic_solve_field(None, None, 0, None) == pic.PIC_EINVAL
+    assert L.pic_deposit(None, 1.0, None, 0) == pic.PIC_EINVAL
     L.pic_destroy(None)
