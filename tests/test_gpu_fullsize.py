@@ -201,3 +201,47 @@ def test_arrays_beyond_2_gib_elementwise():
     ref = st.deposit(-1.0)
     assert np.all(np.abs(rho - ref) <= 1e-12 * np.maximum(np.abs(ref), 1.0))
     pic.pic_destroy(sim)
+
+
+# ---- the closed cycle at full size ----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("config,cycles", [(3, 20), (4, 10)])
+def test_fullsize_closed_cycle_against_the_oracle_loop(config, cycles):
+    """pic_cycle at BASELINE.json's full sizes (config 3: e- + D+ between absorbing walls, 2 x 20 M particles, 10^5 nodes;
+    config 4: 100 M electrons on a ring of 10^6 nodes with a neutralising background): push + arrange, deposit, two
+    filter passes, Poisson, E, the field never leaving the device -- against the same loop of the oracle (threaded
+    mover / arranger twin, sequential deposition, binary128 Thomas solve).  The fields agree to rounding (DESIGN.md
+    section 12), so the particles agree to the tolerance of the reduced closed-loop test and cells, counts, arranged order
+    and wall counters bit for bit."""
+    inp = workloads.make(config)
+    nc, dx, boundary, passes = inp["nc"], inp["dx"], inp["boundary"], 2
+    ppc = len(inp["species"][0]["x"]) / nc
+    w = 0.25 / ppc
+    weights = [-w if s["qm"] < 0 else w for s in inp["species"]]
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        descs = [pic.make_species(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], qm=s["qm"], arrange_every=1)
+                 for s in inp["species"]]
+    stream.synchronize()
+    sim = pic.pic_create(nc=nc, dx=dx, dt=inp["dt"], boundary=boundary, E_nodes=inp["E"], B=inp["B"], species=descs,
+                         stream=stream)
+    rho_t, phi_t = pic.pic_cycle(sim, cycles, weights, smooth_passes=passes, want_phi=True)
+    states = [oracle.State(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], nc=nc, dx=dx, dt=inp["dt"], boundary=boundary,
+                           E=inp["E"].copy(), qm=s["qm"], B=inp["B"], arrange_every=1, threads=0) for s in inp["species"]]
+    for _ in range(cycles):
+        rho_o = np.zeros(nc + 1)
+        for si, st in enumerate(states):
+            st.push(1)
+            rho_o = rho_o + st.deposit(weights[si])
+        _, phi_o, E_o = oracle.field_solve(rho_o, nc, dx, boundary, passes)
+        for st in states:
+            st.E[:] = E_o
+    E = pic.pic_get_field(sim)  # settles the pending cycles
+    pmax = max(np.max(np.abs(phi_o)), dx * dx * np.max(np.abs(rho_o)))
+    assert np.max(np.abs(rho_t.cpu().numpy() - rho_o)) <= 1e-11 * max(np.max(np.abs(rho_o)), w)
+    assert np.max(np.abs(phi_t.cpu().numpy() - phi_o)) <= 1e-10 * pmax
+    assert np.max(np.abs(E - E_o)) <= 1e-10 * max(np.max(np.abs(E_o)), pmax / dx)
+    for si, (sp, st) in enumerate(zip(sim.species, states)):
+        compare(sp, st, where=f"config {config} full size, {cycles} closed cycles, species {si}", bitwise=False, counts=True,
+                nc=nc, rtol=1e-10, atol=1e-11)
+        assert pic.pic_fused_info(sp)["decline_reasons"] == 0
+    pic.pic_destroy(sim)
