@@ -28,6 +28,12 @@
  * it.  One host thread per pic_sim at a time; different sims may be driven from different threads
  * (what they share -- the memory pool of pic_trim_memory -- is locked).  There is no CPU fallback: without a CUDA device
  * every compute entry point fails with PIC_ECUDA.
+ *
+ * Tracing: every kernel class is launched inside an NVTX range of its name ("mover", "hist", "scan",
+ * "scatter", "general", "fused", "deposit", "field"; the names pic_kernel_time takes), pic_push_all,
+ * pic_cycle and pic_run_host inside a range of theirs -- for nsys, or `ncu --nvtx --nvtx-include "fused/"`.
+ * No cost without a profiler attached.  PIC_TRACE=1 in the environment prints the launch geometry of the
+ * fused step and the phases of pic_run_host to stderr.
  */
 #ifndef PIC_H_
 #define PIC_H_

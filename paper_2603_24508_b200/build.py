@@ -16,7 +16,7 @@ LIB = os.path.join(HERE, "libpic.so")
 SOURCES = [os.path.join(CSRC, "pic.cu")]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-fmad=false", "-shared", "-Xcompiler", "-fPIC,-ffp-contract=off,-Wall",
-         "-cudart", "static"]
+         "-cudart", "static", "-ldl"]
 
 
 def _deps():

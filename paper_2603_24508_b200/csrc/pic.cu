@@ -12,6 +12,8 @@
 #include <new>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h> // header-only; a no-op unless a profiler (nsys, ncu --nvtx) is attached
+
 #include "pic_device.cuh"
 #include "mover.cuh"
 #include "scan.cuh"
@@ -129,7 +131,17 @@ struct pic_sim {
     unsigned long long k_launches[K_COUNT] = {};
 };
 
-// Records an event pair around the launches made during its lifetime (only when timing is on).
+// NVTX range for the lifetime of the object (ranges "mover", "hist", "scan", "scatter", ... per
+// kernel class, plus one per multi-phase API call).
+struct NvtxRange {
+    explicit NvtxRange(const char *name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+    NvtxRange(const NvtxRange &) = delete;
+    NvtxRange &operator=(const NvtxRange &) = delete;
+};
+
+// Records an event pair around the launches made during its lifetime (only when timing is on), inside an NVTX range
+// named after the kernel class.
 struct KernelSpan {
     pic_sim *sim;
     cudaEvent_t a = nullptr, b = nullptr;
@@ -144,12 +156,14 @@ struct KernelSpan {
     cudaStream_t stream;
     KernelSpan(pic_sim *s, int kid, cudaStream_t st = nullptr) : sim(s), id(kid), stream(st ? st : s->stream)
     {
+        nvtxRangePushA(K_NAMES[kid]);
         if (!sim->opt_timing) return;
         a = get(sim); b = get(sim);
         if (a) cudaEventRecord(a, stream);
     }
     ~KernelSpan()
     {
+        nvtxRangePop();
         if (!a || !b) return;
         cudaEventRecord(b, stream);
         sim->spans.push_back({id, a, b});
@@ -1236,6 +1250,7 @@ static int read_state(pic_species *s, DevState &h)
 extern "C" int pic_push_all(pic_sim *sim, int nsteps)
 {
     if (!sim || nsteps < 0) return PIC_EINVAL;
+    NvtxRange range("pic_push_all");
     const size_t ns = sim->sp.size();
     if (ns <= 1 || !sim->opt_species_streams) {
         for (int it = 0; it < nsteps; ++it)
@@ -1465,6 +1480,7 @@ extern "C" int pic_cycle(pic_sim *sim, int ncycles, const double *weights, int s
 {
     if (!sim || ncycles < 0 || !weights || !rho_dev || smooth_passes < 0 || smooth_passes > 1024) return PIC_EINVAL;
     if (sim->nc < 2) return PIC_EINVAL;
+    NvtxRange range("pic_cycle");
     const size_t ns = sim->sp.size();
     for (size_t i = 0; i < ns; ++i)
         if (!std::isfinite(weights[i])) return PIC_EINVAL;
@@ -1550,6 +1566,7 @@ extern "C" int pic_sync(pic_sim *sim)
 extern "C" int pic_run_host(const pic_grid_desc *g, pic_host_species *hs, int nspecies, int nsteps)
 {
     if (!g || !hs || nspecies < 1 || nsteps < 0) return PIC_EINVAL;
+    NvtxRange range("pic_run_host");
     cudaStream_t stream = static_cast<cudaStream_t>(g->stream);
     // optional wall-clock trace of the phases (stderr), switched on by the environment variable PIC_TRACE
     const bool trace = getenv("PIC_TRACE") != nullptr;
