@@ -364,3 +364,30 @@ def test_pic_cycle_arguments():
     pic.pic_cycle(sim, 0, weights)
     pic.pic_sync(sim)
     pic.pic_destroy(sim)
+
+
+def test_pic_cycle_long_run_keeps_its_invariants():
+    """600 closed cycles of the two-species slab (reduced config 3) in calls of 100, nothing checked in between but at the
+    call boundaries: particles are conserved exactly (live + absorbed = initial), the state stays grouped with
+    cell = floor(x/dx), the fused path stays on (tile sizing follows the drifting per-cell maximum through the
+    asynchronous telemetry), the self-consistent field stays finite."""
+    inp, weights = _cycle_inputs(3)
+    sim = _make_sim(inp)
+    n0 = [len(s["x"]) for s in inp["species"]]
+    rho = None
+    for _ in range(6):
+        rho, _ = pic.pic_cycle(sim, 100, weights, smooth_passes=2, rho=rho)
+        pic.pic_sync(sim)
+        for si, sp in enumerate(sim.species):
+            wf = pic.pic_wall_flux(sp)
+            assert pic.pic_n_live(sp) + wf["left_total"] + wf["right_total"] == n0[si]
+            info = pic.pic_fused_info(sp)
+            assert info["active"] == 1 and info["decline_reasons"] == 0, info
+    E = pic.pic_get_field(sim)
+    assert np.all(np.isfinite(E)) and 0 < np.max(np.abs(E)) < 10
+    for sp in sim.species:
+        x, _, _, _, cell = sp.state()
+        assert bool((cell[1:] >= cell[:-1]).all())
+        assert bool((torch.floor(x / inp["dx"]).to(torch.int32).clamp(max=inp["nc"] - 1) == cell).all())
+        assert pic.pic_step_count(sp) == 600
+    pic.pic_destroy(sim)
