@@ -32,13 +32,17 @@ def residual_ld(phi, rho, dx, nodes):
 
 
 # ------------------------------------------------------------------------------------------------ Poisson, bounded
-@pytest.mark.parametrize("nc,dx,rho0", [(8, 1.0, 1.0), (100, 0.5, -2.5), (1000, 0.125, 0.75)])
+@pytest.mark.parametrize("nc,dx,rho0", [(8, 1.0, 1.0), (100, 0.5, -2.5), (1000, 0.125, 0.75),
+                                        (100000, 0.3, -1.25), (1000000, 1.0, 0.1)])
 def test_uniform_rho_gives_the_exact_parabola(nc, dx, rho0):
     phi = oracle.poisson(np.full(nc + 1, rho0), nc, dx, ABSORBING)
     j = np.arange(nc + 1, dtype=np.float64)
     want = rho0 * dx * dx * j * (nc - j) / 2.0  # the second difference of a quadratic is exact on the grid
     assert phi[0] == 0.0 and phi[nc] == 0.0
-    # the elimination runs in long double (S28): the binary64 result is the exact parabola to a few ulp
+    # the elimination runs in binary128 (S28): the binary64 result is the exact parabola to a few ulp AT EVERY SIZE THE
+    # ORACLE IS USED.  The two large grids are the pin for that precision: an x87 long double elimination passes the
+    # small cases but is 2e-13 (1e5 nodes) and 7e-12 (1e6 nodes) of max |phi| away from the parabola, 300x and
+    # 8000x this bound, while the binary128 one stays below 1e-16 (measured, "What's weak" 1).
     assert np.max(np.abs(phi - want)) <= 4 * np.finfo(np.float64).eps * np.max(np.abs(want))
 
 
