@@ -66,3 +66,37 @@ def test_argument_validation_without_gpu():
     assert L.pic_solve_field(None, None, 0, None) == pic.PIC_EINVAL
     assert L.pic_deposit(None, 1.0, None, 0) == pic.PIC_EINVAL
     L.pic_destroy(None)
+
+
+def test_ctypes_mirrors_have_the_layout_of_the_header(tmp_path):
+    """The four public structs are declared twice: in include/pic.h and, by hand, as ctypes classes in the binding.
+    A strict C11 client compiled against the header prints sizeof and every offsetof; they must equal the mirrors'."""
+    import subprocess
+    mirrors = {"pic_grid_desc": pic.pic_grid_desc, "pic_species_desc": pic.pic_species_desc,
+               "pic_wall_flux_t": pic.pic_wall_flux_t, "pic_host_species": pic.pic_host_species}
+    lines = ['#include <stdio.h>', '#include <stddef.h>', '#include "pic.h"', 'int main(void) {']
+    for name, cls in mirrors.items():
+        lines.append(f'    printf("{name} size %zu\\n", sizeof({name}));')
+        for field, _ in cls._fields_:
+            lines.append(f'    printf("{name} {field} %zu\\n", offsetof({name}, {field}));')
+    lines += ['    return 0;', '}']
+    src = tmp_path / "layout.c"
+    src.write_text("\n".join(lines) + "\n")
+    exe = tmp_path / "layout"
+    subprocess.run(["gcc", "-std=c11", "-Wall", "-Wextra", "-pedantic", "-Werror", "-I", os.path.join(ROOT, "include"),
+                    "-o", str(exe), str(src)], check=True)
+    out = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split("\n")
+    seen = 0
+    for line in filter(None, out):
+        name, field, value = line.split()
+        cls = mirrors[name]
+        want = C.sizeof(cls) if field == "size" else getattr(cls, field).offset
+        assert int(value) == want, f"{name}.{field}: header {value}, ctypes mirror {want}"
+        seen += 1
+    assert seen == sum(len(c._fields_) + 1 for c in mirrors.values())
+    # every member of the header's structs is mirrored (a member added to the header only would shift nothing above)
+    hdr = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "pic.h")).read(), flags=re.S)
+    for name, cls in mirrors.items():
+        body = re.search(r"typedef struct \{([^}]*)\} " + name + ";", hdr).group(1)
+        members = re.findall(r"\*?\b([A-Za-z_]\w*)\s*(?:\[\d+\])?\s*[,;]", body)
+        assert sorted(members) == sorted(f for f, _ in cls._fields_), f"{name}: header members {members}"
