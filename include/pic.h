@@ -152,6 +152,48 @@ int pic_wall_flux(pic_species *sp, pic_wall_flux_t *out);
  * arranged slots.  Deterministic (fixed summation tree); agrees with a sequential sum to rounding. */
 int pic_deposit(pic_species *sp, double weight, double *rho_dev, int accumulate);
 
+/* The same deposition (PIC phase (ii)) for a caller that must not cause a device allocation.
+ *
+ * Who that is.  pic_deposit takes its per-cell scratch (one pair of doubles per cell) from the library's memory
+ * pool the first time a species deposits, and a handle only exists after pic_create, which allocates too.  A host
+ * code built the way the paper builds BIT1 -- every device array mapped once at start-up and kept for the whole run
+ * (PAPER.md:89), the rest of the GPU's memory budgeted to other owners -- may have nothing left to give, or may run
+ * its time loop under a rule that nothing in it allocates: cudaMalloc and cudaFree serialise the whole device, so
+ * an allocation hidden in a per-step call stalls every other stream (the other species, the copies running beside
+ * them) exactly where the paper wants them to overlap.  Such a caller already owns x and an offset
+ * table; this call needs nothing else.
+ *
+ * What it does.  No handle: the caller passes the arranged positions, the offset table and the grid, and gets rho.
+ *   x_dev       DEVICE, n doubles: positions of the live particles grouped by cell (the active x buffer after an
+ *               arrange), every x in [0, nc*dx) with min(floor(x*(1/dx)), nc-1) equal to its cell
+ *   offset_dev  DEVICE, nc+1 int32: the particles of cell c are x_dev[offset[c] .. offset[c+1]), offset[0] = 0,
+ *               offset[nc] = n (what pic_cell_counts returns, uploaded by the caller)
+ *   n, nc, dx   particle count (0 <= n < 2^31), cells (1 <= nc <= PIC_DEPOSIT_STATIC_MAX_NC), cell width
+ *   boundary    pic_boundary: on a periodic grid nodes 0 and nc are one point and carry the same summed value
+ *   weight, accumulate, rho_dev   as pic_deposit (rho_dev: DEVICE, nc+1 doubles, caller-owned, the output)
+ *   stream      a cudaStream_t of the current device, or NULL for the legacy default stream
+ * Same kernels, same summation tree and therefore the same bits as pic_deposit on the same state (pic_deposit picks
+ * its lanes per cell from an upper bound of n; where that bound is loose the two agree to rounding instead).
+ * Asynchronous on `stream`.  Nothing is read or written on the host side except the arguments.
+ *
+ * The scratch is a fixed array inside the library image, 16 bytes per cell for PIC_DEPOSIT_STATIC_MAX_NC cells =
+ * 16 MiB, which every GPU that loads libpic.so carries until the process exits, used or not.  The call never calls
+ * cudaMalloc, cudaFree, a memory pool or any library routine that allocates; it launches two kernels.
+ *   - The FIRST call on each device looks up the device address of that array (cudaGetSymbolAddress, once per
+ *     device, with that device current) before it launches.  Make that first call during set-up, outside any
+ *     stream capture; later calls on the device only launch.
+ *   - There is ONE array per device and every call uses it.  Calls that may overlap on the GPU -- different
+ *     streams without an event between them, or two host threads -- race on it and produce garbage in rho: keep all
+ *     calls of a device on one stream or order them with events.  The array keeps what the last call left in it;
+ *     nothing in it has to start at zero, because the first kernel writes the entry of every cell c < nc before
+ *     the second reads it, so the call clears nothing.
+ * Errors: PIC_EINVAL (NULL pointer, n or nc out of range, dx not finite or <= 0, weight not finite, boundary not a
+ * pic_boundary), PIC_ECAPACITY (nc > PIC_DEPOSIT_STATIC_MAX_NC: nothing is launched; pic_last_error names both
+ * numbers -- use pic_deposit, or split the grid), PIC_ECUDA.  Validation happens before any CUDA call. */
+#define PIC_DEPOSIT_STATIC_MAX_NC (1 << 20)
+int pic_deposit_static(const double *x_dev, const int32_t *offset_dev, int64_t n, int32_t nc, double dx,
+                       int32_t boundary, double weight, int accumulate, double *rho_dev, void *stream);
+
 /* Replace E from a HOST array (nc+1 doubles, copied).  Steps already enqueued run with the old field.  Syncs (the
  * caller's array may be pageable, and unchecked fused steps are checked first).  PIC_EINVAL for a non-finite value. */
 int pic_set_field(pic_sim *sim, const double *E_nodes_host);

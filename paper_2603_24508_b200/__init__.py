@@ -22,8 +22,9 @@ EXPORTS = [
     "pic_active_buffer", "pic_cell_counts", "pic_step_count", "pic_arrange_info", "pic_workspace_bytes",
     "pic_set_option", "pic_launch_count", "pic_sync", "pic_destroy", "pic_strerror", "pic_last_error",
     "pic_run_host", "pic_kernel_time", "pic_fused_info", "pic_deposit", "pic_n_live", "pic_set_field_device",
-    "pic_solve_field", "pic_get_field", "pic_push_all", "pic_trim_memory", "pic_cycle",
+    "pic_solve_field", "pic_get_field", "pic_push_all", "pic_trim_memory", "pic_cycle", "pic_deposit_static",
 ]
+PIC_DEPOSIT_STATIC_MAX_NC = 1 << 20  # include/pic.h: cells the built-in scratch array of pic_deposit_static holds
 
 
 class PicError(RuntimeError):
@@ -96,6 +97,7 @@ def lib():
         L.pic_kernel_time.argtypes = [vp, C.c_char_p, C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
         L.pic_fused_info.argtypes = [vp, i32p, i32p, i32p, i32p]
         L.pic_deposit.argtypes = [vp, C.c_double, vp, C.c_int]
+        L.pic_deposit_static.argtypes = [vp, vp, C.c_int64, C.c_int32, C.c_double, C.c_int32, C.c_double, C.c_int, vp, vp]
         L.pic_sync.argtypes = [vp]
         L.pic_destroy.argtypes = [vp]
         L.pic_destroy.restype = None
@@ -354,6 +356,31 @@ def pic_deposit(sp, weight, rho=None, accumulate=False):
     assert rho.dtype == torch.float64 and rho.numel() == nc + 1 and rho.is_contiguous()
     _check(lib().pic_deposit(sp.handle, float(weight), C.c_void_p(rho.data_ptr()), 1 if accumulate else 0), "pic_deposit")
     torch.cuda.current_stream().wait_stream(sp.sim.stream)  # rho is produced on the sim's stream
+    return rho
+
+
+def pic_deposit_static(x, offset, *, nc, dx, boundary, weight, rho, accumulate=False, stream=None):
+    """pic_deposit_static: pic_deposit without a handle and without any device allocation, for a caller whose time
+    loop must not allocate (all device memory handed out at start-up, or an allocation would stall its other streams;
+    include/pic.h has the full reasoning).  Every array is the caller's: x (float64, the n arranged positions), offset
+    (int32, nc+1, offset[nc] = n), rho (float64, nc+1, the output) are CUDA tensors; the binding creates none and the
+    library uses a 16 MiB array built into libpic.so as scratch, so nc <= PIC_DEPOSIT_STATIC_MAX_NC (PicError with
+    PIC_ECAPACITY beyond it).  Runs on `stream` (default: torch's current stream).  All calls on a device share that
+    one scratch array: keep them on one stream, overlapping calls race.  The first call on a device also looks up the
+    array's device address; make it during set-up."""
+    import torch
+    assert x.is_cuda and x.dtype == torch.float64 and x.is_contiguous() and x.dim() == 1
+    assert offset.is_cuda and offset.dtype == torch.int32 and offset.is_contiguous() and offset.numel() == nc + 1
+    assert rho.is_cuda and rho.dtype == torch.float64 and rho.is_contiguous() and rho.numel() == nc + 1
+    st = stream if stream is not None else torch.cuda.current_stream()
+    rc = lib().pic_deposit_static(C.c_void_p(x.data_ptr()), C.c_void_p(offset.data_ptr()), int(x.numel()), int(nc),
+                                  float(dx), int(boundary), float(weight), 1 if accumulate else 0,
+                                  C.c_void_p(rho.data_ptr()), C.c_void_p(st.cuda_stream))
+    if rc != PIC_OK:
+        err = PicError(rc, "pic_deposit_static")
+        if rc in (PIC_EINVAL, PIC_ECAPACITY):  # this call always leaves the reason in pic_last_error
+            err.args = (f"{err.args[0]}: {pic_last_error()}",)
+        raise err
     return rho
 
 

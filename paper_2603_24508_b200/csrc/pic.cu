@@ -1698,3 +1698,76 @@ extern "C" int pic_run_host(const pic_grid_desc *g, pic_host_species *hs, int ns
     mark("arena released");
     return rc;
 }
+
+// ------------------------------------------------------------------------------------------
+// pic_deposit_static: the deposition for callers that may not allocate device memory (include/pic.h)
+// ------------------------------------------------------------------------------------------
+// The per-cell sums {sum (1-w), sum w} live in an array that is part of the library image instead of coming from the
+// pool: 16 B * PIC_DEPOSIT_STATIC_MAX_NC = 16 MiB on every device that loads the library, for the life of the process.
+// One array per device, shared by every call; it keeps the previous call's sums, which no call reads: entry c < nc is
+// written by deposit_cell_kernel before deposit_node_kernel reads it, and entries >= nc are never read.
+static __device__ __align__(256) double2 g_dep_static_cs[PIC_DEPOSIT_STATIC_MAX_NC];
+
+// On the host, g_dep_static_cs is only the handle the runtime knows the array by, not an address a kernel can use.  Its
+// device address differs per device and is looked up once per device (with that device current) by the first call.
+static double2 *g_dep_static_addr[64] = {};
+static std::mutex g_dep_static_mu;
+
+static int dep_static_fail(int rc, const char *fmt, long long a = 0, long long b = 0)
+{
+    snprintf(g_err, sizeof g_err, fmt, a, b);
+    return rc;
+}
+
+extern "C" int pic_deposit_static(const double *x_dev, const int32_t *offset_dev, int64_t n, int32_t nc, double dx,
+                                  int32_t boundary, double weight, int accumulate, double *rho_dev, void *stream)
+{
+    // argument checks first: none of them touches CUDA
+    if (!x_dev || !offset_dev || !rho_dev) return dep_static_fail(PIC_EINVAL, "pic_deposit_static: NULL device pointer");
+    if (nc < 1) return dep_static_fail(PIC_EINVAL, "pic_deposit_static: nc = %lld, need nc >= 1", nc);
+    if (nc > PIC_DEPOSIT_STATIC_MAX_NC)
+        return dep_static_fail(PIC_ECAPACITY,
+                               "pic_deposit_static: nc = %lld cells exceeds PIC_DEPOSIT_STATIC_MAX_NC = %lld, the size of the "
+                               "built-in scratch array (use pic_deposit, or deposit the grid in pieces)",
+                               nc, PIC_DEPOSIT_STATIC_MAX_NC);
+    if (n < 0 || n >= (int64_t)INT_MAX - 64)
+        return dep_static_fail(PIC_EINVAL, "pic_deposit_static: n = %lld outside [0, 2^31 - 64)", n);
+    if (!std::isfinite(dx) || dx <= 0.0 || !std::isfinite(weight))
+        return dep_static_fail(PIC_EINVAL, "pic_deposit_static: dx must be finite and positive, weight finite");
+    if (boundary != PIC_PERIODIC && boundary != PIC_ABSORBING)
+        return dep_static_fail(PIC_EINVAL, "pic_deposit_static: boundary = %lld is not a pic_boundary", boundary);
+
+    int device = -1;
+    CU(cudaGetDevice(&device));
+    if (device < 0 || device >= 64) return dep_static_fail(PIC_EINVAL, "pic_deposit_static: device ordinal %lld not supported", device);
+    double2 *cs = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_dep_static_mu);
+        if (!g_dep_static_addr[device]) { // set-up, once per device: the first call on it (before any stream capture)
+            void *p = nullptr;
+            CU(cudaGetSymbolAddress(&p, g_dep_static_cs));
+            g_dep_static_addr[device] = static_cast<double2 *>(p);
+        }
+        cs = g_dep_static_addr[device];
+    }
+
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    DepositArgs a{};
+    a.x = x_dev;
+    a.off = offset_dev;
+    a.cs = cs;
+    a.nc = nc;
+    { volatile double inv = 1.0 / dx; a.inv_dx = inv; } // as boris_constants: one rounded division
+    NvtxRange range("pic_deposit_static");
+    const int lpc = n <= 448LL * nc ? 16 : 32; // the rule of deposit_enqueue, from n itself
+    const long long threads = (long long)nc * lpc;
+    const unsigned blocks = (unsigned)((threads + DEP_THREADS - 1) / DEP_THREADS);
+    if (lpc == 16) deposit_cell_kernel<16><<<blocks, DEP_THREADS, 0, st>>>(a);
+    else deposit_cell_kernel<32><<<blocks, DEP_THREADS, 0, st>>>(a);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "deposit_cell_kernel (static scratch)");
+    deposit_node_kernel<<<(nc + 1 + 255) / 256, 256, 0, st>>>(cs, nc, boundary == PIC_PERIODIC ? 1 : 0, weight, accumulate ? 1 : 0, rho_dev);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "deposit_node_kernel (static scratch)");
+    return PIC_OK;
+}
