@@ -293,7 +293,14 @@ def pic_cycle(sim, ncycles, weights, smooth_passes=0, rho=None, phi=None, want_p
             assert t.dtype == torch.float64 and t.numel() == sim.nc + 1 and t.is_contiguous() and t.is_cuda
     w = (C.c_double * len(sim.species))(*[float(x) for x in weights])
     assert len(weights) == len(sim.species)
-    sim._cycle_keep = (rho, phi)  # the library reads and writes them until its next synchronising call
+    # The library keeps the rho / phi pointers of EVERY call whose cycles are still unchecked and, should a fused step
+    # have declined, writes into all of them at its next synchronising call: hold every pair until then (a caller who
+    # drops the returned rho must not hand its memory back to torch's allocator under the library's feet).
+    keep = sim.__dict__.setdefault("_cycle_keep", [])
+    if len(keep) >= 64:  # bound the list: settle what is pending (pic_sync clears it)
+        pic_sync(sim)
+    if not any(r is rho and p is phi for r, p in keep):
+        keep.append((rho, phi))
     sim.stream.wait_stream(torch.cuda.current_stream())
     _check(lib().pic_cycle(sim.handle, int(ncycles), w, int(smooth_passes), C.c_void_p(rho.data_ptr()),
                            C.c_void_p(phi.data_ptr()) if phi is not None else None), "pic_cycle")
@@ -410,6 +417,9 @@ def pic_kernel_time(sim, kernel):
 
 def pic_sync(sim):
     _check(lib().pic_sync(sim.handle), "pic_sync")
+    keep = sim.__dict__.get("_cycle_keep")
+    if keep:  # pending cycles are settled: only the latest pair may still be in the caller's hands
+        del keep[:-1]
 
 
 def pic_destroy(sim):

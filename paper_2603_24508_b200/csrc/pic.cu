@@ -96,6 +96,7 @@ struct pic_species {
     bool counts_fresh = false; // count/offset describe the current state
     bool all_live = true;      // no flagged-dead particle in [0, n)
     bool reset_w = false;      // an arrange ran since the displacement bound was last folded
+    int trace_last[6] = {-1, -1, -1, -1, -1, -1}; // PIC_TRACE: the launch geometry last reported
 };
 
 struct pic_sim {
@@ -403,9 +404,11 @@ static void (*fused_pick(int rows, bool periodic, bool bz0, bool tma, int def))(
 
 // The fused kernels need more dynamic shared memory than the default limit: raise it once per DEVICE (the attribute
 // is per device and per function; a process may create sims on several devices).
+static std::mutex g_attr_mu;
 static int fused_set_attributes(int device)
 {
     static bool done[64] = {};
+    std::lock_guard<std::mutex> lock(g_attr_mu); // sims of different threads may be created at the same time
     if (device >= 0 && device < 64 && done[device]) return PIC_OK;
     std::vector<void (*)(FusedArgs)> kerns;
     for (int rows : {8, 12, 16})
@@ -859,7 +862,7 @@ static int arrange_split(pic_species *s, bool hist_ready, bool after_mover)
         ga.st = s->d_st; ga.nc = nc; ga.n_ub = s->n_ub; ga.ws = s->ws; ga.ws_bytes = s->ws_bytes;
         ga.off_old = s->d_off[oo];
         ga.scan_scratch = s->d_scan;
-        KernelSpan gspan(sim, K_GENERAL);
+        KernelSpan gspan(sim, K_GENERAL, s->stream); // general_arrange launches on the species' stream
         if (int rc = general_arrange(ga, s->stream, sim->sm_count, &sim->launches)) return rc == PIC_ECUDA ? cuda_fail(cudaGetLastError(), "general_arrange") : rc;
     }
     if (s->sim->opt_fused && s->arrange_every == 1)
@@ -912,7 +915,9 @@ static int push_split(pic_species *s, bool will_arrange)
     }
     s->h_wsum = std::min<long long>(s->h_wsum + host_step_bound(s), 1LL << 40);
     s->h_steps_since_sync++;
-    s->h_kick_acc += s->vkick;
+    // a step enqueued while max |E| of a device-side field is still unknown has no known kick: the bound stays
+    // "unknown" (infinite) until the next read_state refreshes the speed bound, even if pic_set_field intervenes
+    s->h_kick_acc += s->sim->emax_known ? s->vkick : (double)INFINITY;
     if (!sim->periodic) s->all_live = false;
     s->counts_fresh = false;
     if (!will_arrange) {
@@ -1065,7 +1070,7 @@ static int push_fused(pic_species *s)
     a.NST = geo.stages;
     {   // PIC_TRACE: report the launch geometry whenever it changes
         static const bool trace = getenv("PIC_TRACE") != nullptr;
-        static int last[6] = {-1, -1, -1, -1, -1, -1};
+        int *last = s->trace_last; // per species: sims of different threads share no mutable static
         const int now[6] = {geo.rows, geo.cpc + 1000 * geo.taper, geo.stages, geo.def, geo.ctas_per_sm, (int)geo.smem};
         if (trace && memcmp(last, now, sizeof now)) {
             memcpy(last, now, sizeof now);
@@ -1130,7 +1135,9 @@ static int push_fused(pic_species *s)
     }
     s->unv_steps++;
     s->h_steps_since_sync++;
-    s->h_kick_acc += s->vkick;
+    // a step enqueued while max |E| of a device-side field is still unknown has no known kick: the bound stays
+    // "unknown" (infinite) until the next read_state refreshes the speed bound, even if pic_set_field intervenes
+    s->h_kick_acc += s->sim->emax_known ? s->vkick : (double)INFINITY;
     s->cur = dst;
     s->cur_off = on;
     s->counts_fresh = true;
@@ -1251,6 +1258,12 @@ extern "C" int pic_push_all(pic_sim *sim, int nsteps)
 {
     if (!sim || nsteps < 0) return PIC_EINVAL;
     NvtxRange range("pic_push_all");
+    // Unchecked pic_cycle work is settled HERE, while every species still runs on the sim's stream: should a fused step
+    // of those cycles have declined, verify_cycles redoes pushes, depositions (species after species into one rho)
+    // and field solves, which are ordered only on a common stream.  Left to the first pic_push below, that redo
+    // would run with each species on its own, mutually unordered stream.
+    if (!sim->in_cycle && !sim->cyc_pending.empty())
+        if (int rc = verify_cycles(sim)) return rc;
     const size_t ns = sim->sp.size();
     if (ns <= 1 || !sim->opt_species_streams) {
         for (int it = 0; it < nsteps; ++it)
@@ -1264,11 +1277,12 @@ extern "C" int pic_push_all(pic_sim *sim, int nsteps)
         if (!s->join_ev) CU(cudaEventCreateWithFlags(&s->join_ev, cudaEventDisableTiming));
     }
     CU(cudaEventRecord(sim->fork_ev, sim->stream));
-    for (pic_species *s : sim->sp) {
-        CU(cudaStreamWaitEvent(s->own_stream, sim->fork_ev, 0));
+    int rc = PIC_OK;
+    for (pic_species *s : sim->sp) { // fork; a failure still goes through the join below, which restores every stream
+        const cudaError_t e = cudaStreamWaitEvent(s->own_stream, sim->fork_ev, 0);
+        if (e != cudaSuccess) { rc = cuda_fail(e, "pic_push_all fork"); break; }
         s->stream = s->own_stream;
     }
-    int rc = PIC_OK;
     for (int it = 0; it < nsteps && rc == PIC_OK; ++it)
         for (pic_species *s : sim->sp) {
             const unsigned long long before = sim->launches;
@@ -1279,6 +1293,7 @@ extern "C" int pic_push_all(pic_sim *sim, int nsteps)
                 if (o != s) o->chain_mark += sim->launches - before;
         }
     for (pic_species *s : sim->sp) { // join, whatever happened
+        if (s->stream != s->own_stream) continue; // the fork failed before this species
         s->stream = sim->stream;
         const cudaError_t e1 = cudaEventRecord(s->join_ev, s->own_stream);
         const cudaError_t e2 = e1 == cudaSuccess ? cudaStreamWaitEvent(sim->stream, s->join_ev, 0) : e1;

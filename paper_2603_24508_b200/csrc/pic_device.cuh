@@ -15,7 +15,6 @@ constexpr int ERR_OUT_OF_DOMAIN = 1;  // a live particle's gather cell fell outs
 constexpr int ERR_NEED_WORKSPACE = 2; // general arranger needed but no / too small workspace
 constexpr int ERR_BAD_INITIAL = 4;    // initial state violates cell == floor(x/dx), live, in range
 constexpr int ERR_NOT_GROUPED = 8;    // (info) initial state is not grouped by cell
-constexpr int ERR_FUSED_OVERFLOW = 16; // (info) fused step fell back to the split path
 constexpr int ERR_ARRANGE_SKIPPED = 32; // the fast arranger declined on the device but the general path was not enqueued
 
 constexpr int W_UNKNOWN = 1 << 29; // displacement bound of a state that is not grouped by cell
@@ -37,7 +36,6 @@ struct DevState {
     int abort;                       // fused step in flight: some CTA declined
     int abort_reason;                // FA_* bits of every decline so far (diagnostics)
     int f_OL, f_AR;                  // fused step in flight: leavers of cell 0 downwards / wrapped arrivals in cell 0
-    int ntiles, ntiles_next;         // tiles of the current partition (fused.cuh) / of the one being written
     int maxcount, maxcount_next;     // upper bound of the largest per-cell count: current state / step in flight
     int maxdef;                      // fused step: most right-movers of one cell that overflowed the deferred queue (0: never)
     int fail_step;                   // step id (FusedArgs::step_id) of the first fused step that declined

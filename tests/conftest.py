@@ -14,11 +14,6 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
 
 
-def pytest_collection_modifyitems(config, items):
-    """GPU tests fail loudly (never skip silently) if selected on a box without CUDA."""
-    return
-
-
 @pytest.fixture(scope="session")
 def golden_dir():
     return GOLDEN
