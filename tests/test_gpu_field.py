@@ -199,6 +199,56 @@ def test_n_live_between_arranges():
     pic.pic_destroy(sim)
 
 
+# Closed loops: the GPU's and the oracle's fields agree to rounding, not bitwise (different summation orders in the
+# deposition and the solve), and every step adds h * dE to v, so x and v drift apart by rounding-sized amounts while cells,
+# counts, order and walls stay exact.  Bounds = about ten times the largest deviation observed over the committed cases
+# (DESIGN.md section 12 lists the observed values); deviation = |a-b| / max(|b|, 0.1), i.e. rtol with atol = rtol / 10.
+CLOSED_RTOL = 1e-12    # observed 8.3e-14 (config 3), 1.4e-14 (config 1); phi in pic_cycle 2.1e-13
+CLOSED_E_RTOL = 5e-13  # observed 6.3e-14
+
+
+def particle_deviation(sp, st):
+    g = [t.cpu().numpy() for t in sp.state()]
+    o = st.live()
+    return max((float(np.max(np.abs(g[k] - o[k]) / np.maximum(np.abs(o[k]), 0.1))) for k in range(4) if len(o[k])), default=0.0)
+
+
+@pytest.mark.parametrize("boundary_cfg", [3, 1])
+def test_closed_loop_is_bitwise_when_both_movers_see_the_same_field(boundary_cfg):
+    """The same 20-step closed loop, but after every solve the oracle's states take the GPU's E (copied out with
+    pic_get_field) instead of the oracle's own.  Both movers then push with identical fields, so the particles must agree
+    BITWISE at every step -- all five arrays, counts, offsets, walls -- and what separates the two loops is only the
+    error of ONE deposition + ONE field solve on identical particles, which is held to the one-call bar of 1e-12."""
+    inp, weights = _cycle_inputs(boundary_cfg)
+    nc, dx, boundary, passes = inp["nc"], inp["dx"], inp["boundary"], 2
+    sim = _make_sim(inp)
+    states = [oracle.State(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], nc=nc, dx=dx, dt=inp["dt"], boundary=boundary,
+                           E=inp["E"].copy(), qm=s["qm"], B=inp["B"], arrange_every=1) for s in inp["species"]]
+    worst = 0.0
+    for step in range(1, 21):
+        rho_t = None
+        pic.pic_push_all(sim, 1)
+        for si, sp in enumerate(sim.species):
+            rho_t = pic.pic_deposit(sp, weights[si], rho=rho_t, accumulate=si > 0)
+        pic.pic_solve_field(sim, rho_t, smooth_passes=passes)
+        rho_o = np.zeros(nc + 1)
+        for si, st in enumerate(states):
+            st.push(1)
+            rho_o = rho_o + st.deposit(weights[si])
+        for si, (sp, st) in enumerate(zip(sim.species, states)):
+            compare(sp, st, where=f"same-field loop step {step} species {si}", bitwise=True, counts=True, nc=nc)
+        _, phi_o, E_o = oracle.field_solve(rho_o, nc, dx, boundary, passes)
+        E = pic.pic_get_field(sim)
+        scale = max(np.max(np.abs(E_o)), np.max(np.abs(phi_o)) / dx)
+        worst = max(worst, np.max(np.abs(E - E_o)) / scale)
+        assert worst <= 1e-12, f"step {step}: one deposition + one solve on identical particles differ by {worst:.2e}"
+        for st in states:
+            st.E[:] = E  # the GPU's field, bit for bit
+    print(f"same-field loop, config {boundary_cfg}: particles bitwise for 20 steps; largest one-call field deviation {worst:.3e}")
+    assert np.max(np.abs(E)) > 0
+    pic.pic_destroy(sim)
+
+
 @pytest.mark.parametrize("boundary_cfg", [3, 1])
 def test_closed_pic_loop_against_the_oracle_loop(boundary_cfg):
     """push -> arrange -> deposit (all species) -> smooth -> solve -> push ..., 20 steps, field kept on the device
@@ -218,6 +268,7 @@ def test_closed_pic_loop_against_the_oracle_loop(boundary_cfg):
         states.append(oracle.State(s["x"], s["vx"], s["vy"], s["vz"], s["cell"], nc=nc, dx=dx, dt=inp["dt"],
                                    boundary=boundary, E=inp["E"].copy(), qm=s["qm"], B=inp["B"], arrange_every=1))
     sim = pic.pic_create(nc=nc, dx=dx, dt=inp["dt"], boundary=boundary, E_nodes=inp["E"], B=inp["B"], species=descs)
+    seen_E, seen_p = 0.0, 0.0
     for step in range(1, 21):
         rho_t = None
         for si, sp in enumerate(sim.species):
@@ -233,12 +284,16 @@ def test_closed_pic_loop_against_the_oracle_loop(boundary_cfg):
             st.E[:] = E_o
         E = pic.pic_get_field(sim)
         pmax = np.max(np.abs(phi_o))
-        assert np.max(np.abs(E - E_o)) <= 1e-11 * max(np.max(np.abs(E_o)), pmax / dx), f"step {step}: E drifted"
+        seen_E = max(seen_E, np.max(np.abs(E - E_o)) / max(np.max(np.abs(E_o)), pmax / dx))
+        assert seen_E <= CLOSED_E_RTOL, f"step {step}: E drifted to {seen_E:.2e}"
         for si, (sp, st) in enumerate(zip(sim.species, states)):
             # the fields agree to rounding (1e-12 of max|phi|/dx), not bitwise, so from the second step on neither do
             # the particles: each step adds a kick difference h*dE to v; cells, counts, order and walls stay exact
             compare(sp, st, where=f"closed loop step {step} species {si}", bitwise=False, counts=True, nc=nc,
-                    rtol=1e-10, atol=1e-11)
+                    rtol=CLOSED_RTOL, atol=0.1 * CLOSED_RTOL)
+            seen_p = max(seen_p, particle_deviation(sp, st))
+    print(f"closed loop, config {boundary_cfg}, 20 steps: observed max E deviation {seen_E:.3e} (bound {CLOSED_E_RTOL}), "
+          f"particle deviation {seen_p:.3e} (bound {CLOSED_RTOL})")
     assert np.max(np.abs(E_o)) > 0
     pic.pic_destroy(sim)
 
@@ -315,10 +370,15 @@ def test_pic_cycle_is_the_checked_loop_without_the_round_trips(boundary_cfg):
         for st in states:
             st.E[:] = E_o
     pmax = np.max(np.abs(phi_o))
-    assert np.max(np.abs(pic.pic_get_field(b) - E_o)) <= 1e-11 * max(np.max(np.abs(E_o)), pmax / dx)
-    assert np.max(np.abs(phi_b.cpu().numpy() - phi_o)) <= 1e-10 * pmax
+    dev_E = np.max(np.abs(pic.pic_get_field(b) - E_o)) / max(np.max(np.abs(E_o)), pmax / dx)
+    dev_phi = np.max(np.abs(phi_b.cpu().numpy() - phi_o)) / pmax
+    assert dev_E <= CLOSED_E_RTOL and dev_phi <= CLOSED_RTOL, (dev_E, dev_phi)
+    dev_p = 0.0
     for si, (sp, st) in enumerate(zip(b.species, states)):
-        compare(sp, st, where=f"pic_cycle species {si}", bitwise=False, counts=True, nc=nc, rtol=1e-10, atol=1e-11)
+        compare(sp, st, where=f"pic_cycle species {si}", bitwise=False, counts=True, nc=nc, rtol=CLOSED_RTOL,
+                atol=0.1 * CLOSED_RTOL)
+        dev_p = max(dev_p, particle_deviation(sp, st))
+    print(f"pic_cycle, config {boundary_cfg}, 20 cycles: observed E {dev_E:.3e}, phi {dev_phi:.3e}, particles {dev_p:.3e}")
     # cycles interleaved with other calls: each of them settles the pending cycles first
     pic.pic_cycle(b, 3, weights, smooth_passes=passes, rho=rho_b)
     pic.pic_push(b.species[0], 1)
@@ -348,6 +408,46 @@ def test_pic_cycle_redoes_the_cycles_after_a_declined_step(boundary_cfg, fast_vz
     rho_a = _checked_loop(a, weights, 4, 1)
     rho_b, _ = pic.pic_cycle(b, 4, weights, smooth_passes=1, rho=rho_b)
     _assert_same_sims(a, b, rho_a, rho_b, "pic_cycle after the decline")
+    pic.pic_destroy(a)
+    pic.pic_destroy(b)
+
+
+@pytest.mark.parametrize("fast_vz", [30.0, 45.0])
+def test_pic_push_all_directly_after_cycles_with_a_declined_step(fast_vz):
+    """pic_cycle -> (a fused step declines on the device) -> pic_push_all, two species.  pic_push_all settles the
+    pending cycles before it moves the species to their own streams: the redo of pushes, depositions into one rho
+    and field solves is ordered on the sim's stream.  Result: the checked loop followed by pic_push_all, bit for bit."""
+    inp, weights = _cycle_inputs(3, fast_vz=fast_vz)
+    assert len(inp["species"]) == 2
+    a, b = _make_sim(inp), _make_sim(inp)
+    rho_a = _checked_loop(a, weights, 16, 1)
+    pic.pic_push_all(a, 3)
+    rho_b, _ = pic.pic_cycle(b, 16, weights, smooth_passes=1)
+    pic.pic_push_all(b, 3)  # no synchronising call in between
+    _assert_same_sims(a, b, rho_a, rho_b, "pic_cycle, decline, pic_push_all")
+    assert pic.pic_fused_info(b.species[0])["decline_reasons"] & 1
+    assert pic.pic_step_count(b.species[0]) == 19 and pic.pic_step_count(b.species[1]) == 19
+    pic.pic_destroy(a)
+    pic.pic_destroy(b)
+
+
+def test_pic_cycle_one_at_a_time_dropping_rho_survives_a_decline():
+    """pic_cycle(sim, 1, w) in a loop, the returned rho dropped every time, and a step that declines on the way: the
+    redo writes into the rho of every unsettled call, so the binding keeps them all alive until the library has
+    settled them.  Result: the checked loop's, and fresh tensors allocated meanwhile are left alone."""
+    import torch
+    inp, weights = _cycle_inputs(3, fast_vz=30.0)
+    a, b = _make_sim(inp), _make_sim(inp)
+    rho_a = _checked_loop(a, weights, 16, 1)
+    canaries = []
+    for _ in range(15):
+        pic.pic_cycle(b, 1, weights, smooth_passes=1)  # rho allocated by the binding and dropped here
+        canaries.append(torch.full((inp["nc"] + 1,), 123.0, dtype=torch.float64, device="cuda"))
+    rho_b, _ = pic.pic_cycle(b, 1, weights, smooth_passes=1)
+    _assert_same_sims(a, b, rho_a, rho_b, "16 single cycles with a decline")
+    for c in canaries:
+        assert bool((c == 123.0).all()), "a redone cycle wrote into memory the caller no longer lent to the library"
+    assert pic.pic_fused_info(b.species[0])["decline_reasons"] & 1
     pic.pic_destroy(a)
     pic.pic_destroy(b)
 

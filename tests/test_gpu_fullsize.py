@@ -203,6 +203,12 @@ def test_arrays_beyond_2_gib_elementwise():
     pic.pic_destroy(sim)
 
 
+# Bounds of the full-size closed cycle: about ten times the largest deviation observed; the
+# deviation of a particle array is |a-b| / max(|b|, 0.1).
+# observed (config 3 / config 4): rho 2.0e-12 / 2.7e-12, phi 2.2e-11 / 4.6e-11, E 3.7e-13 / 5.6e-14, particles 5.1e-12 / 1.4e-11
+FULL_RHO_RTOL, FULL_PHI_RTOL, FULL_E_RTOL, FULL_P_RTOL = 1e-11, 1e-10, 4e-12, 1e-10
+
+
 # ---- the closed cycle at full size ----------------------------------------------------------------------------------------
 @pytest.mark.parametrize("config,cycles", [(3, 20), (4, 10)])
 def test_fullsize_closed_cycle_against_the_oracle_loop(config, cycles):
@@ -237,11 +243,17 @@ def test_fullsize_closed_cycle_against_the_oracle_loop(config, cycles):
             st.E[:] = E_o
     E = pic.pic_get_field(sim)  # settles the pending cycles
     pmax = max(np.max(np.abs(phi_o)), dx * dx * np.max(np.abs(rho_o)))
-    assert np.max(np.abs(rho_t.cpu().numpy() - rho_o)) <= 1e-11 * max(np.max(np.abs(rho_o)), w)
-    assert np.max(np.abs(phi_t.cpu().numpy() - phi_o)) <= 1e-10 * pmax
-    assert np.max(np.abs(E - E_o)) <= 1e-10 * max(np.max(np.abs(E_o)), pmax / dx)
+    dev_rho = np.max(np.abs(rho_t.cpu().numpy() - rho_o)) / max(np.max(np.abs(rho_o)), w)
+    dev_phi = np.max(np.abs(phi_t.cpu().numpy() - phi_o)) / pmax
+    dev_E = np.max(np.abs(E - E_o)) / max(np.max(np.abs(E_o)), pmax / dx)
+    assert dev_rho <= FULL_RHO_RTOL and dev_phi <= FULL_PHI_RTOL and dev_E <= FULL_E_RTOL, (dev_rho, dev_phi, dev_E)
+    dev_p = 0.0
     for si, (sp, st) in enumerate(zip(sim.species, states)):
         compare(sp, st, where=f"config {config} full size, {cycles} closed cycles, species {si}", bitwise=False, counts=True,
-                nc=nc, rtol=1e-10, atol=1e-11)
+                nc=nc, rtol=FULL_P_RTOL, atol=0.1 * FULL_P_RTOL)
+        g, o = [t.cpu().numpy() for t in sp.state()], st.live()
+        dev_p = max(dev_p, max(float(np.max(np.abs(g[k] - o[k]) / np.maximum(np.abs(o[k]), 0.1))) for k in range(4)))
         assert pic.pic_fused_info(sp)["decline_reasons"] == 0
+    print(f"full-size closed cycle, config {config}, {cycles} cycles: observed rho {dev_rho:.3e}, phi {dev_phi:.3e}, "
+          f"E {dev_E:.3e}, particles {dev_p:.3e}")
     pic.pic_destroy(sim)
