@@ -23,6 +23,8 @@ library's stream.  `e2e`: the same metric through the C-ABI call pic_run_host wi
 CUDA events inside the timed region (pic_kernel_time), against MEASURED_PEAKS.json.
 `cpu_baseline`: the CPU oracle (oracle/, as it stands) on the full-size workload for a reduced step
 count: single thread (the authority), and `threaded`: its bit-identical OpenMP twin on all host cores.
+`per_config` (default at --config 4 on one GPU; --no-per-config skips it): value, ms per step, dominant kernel and its
+roofline fraction for the other four configs, each measured by this script in a subprocess (10 timed steps).
 `fused_path`: how many timed steps took the fused kernel / were redone by the split kernels; a
 decline inside the timed region marks the line "invalid" and the exit code is 3.
 
@@ -252,14 +254,14 @@ def compact(line):
 
 def per_config_block(args, own_line):
     """The five configs in one place: this run's own, and the other four measured by this script in subprocesses
-    (device-resident leg only: no e2e, no CPU baseline), 30 timed steps after 3 warm-up steps each."""
+    (device-resident leg only: no e2e, no CPU baseline, no field legs), 10 timed steps after 3 warm-up steps each."""
     import subprocess
     out = {str(args.config): compact(own_line)}
     for c in (1, 2, 3, 4, 5):
         if c == args.config:
             continue
-        cmd = [sys.executable, os.path.abspath(__file__), "--config", str(c), "--steps", "30", "--warmup", "3", "--no-e2e",
-               "--no-cpu", "--no-field"] + [a for o in args.option for a in ("--option", o)]
+        cmd = [sys.executable, os.path.abspath(__file__), "--config", str(c), "--steps", "10", "--warmup", "3", "--no-e2e",
+               "--no-cpu", "--no-field", "--no-per-config"] + [a for o in args.option for a in ("--option", o)]
         r = subprocess.run(cmd, capture_output=True, text=True, cwd=ROOT)
         try:
             out[str(c)] = compact(json.loads(r.stdout.strip().splitlines()[-1]))
@@ -284,7 +286,9 @@ def main():
     ap.add_argument("--no-deposit", action="store_true", help="skip the separate timing of pic_deposit")
     ap.add_argument("--no-field", action="store_true", help="skip the separate timing of pic_solve_field and of the closed cycle")
     ap.add_argument("--all-configs", action="store_true",
-                    help="append a compact per_config block: the other four configs, each run by this script in a subprocess")
+                    help="append a compact per_config block: the other four configs, each run by this script in a "
+                         "subprocess (the default at --config 4 on one GPU; this flag forces it for any --config)")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block")
     ap.add_argument("--option", action="append", default=[], help="pic_set_option key=value (e.g. fused=0)")
     ap.add_argument("--scale", type=float, default=1.0, help="scale nc (debug only; the line is then not a bench value)")
     ap.add_argument("--debug-fast-particle", type=float, default=None, metavar="VZ",
@@ -448,8 +452,14 @@ def main():
             pic.pic_solve_field(sim, rho, smooth_passes=2)
         fms, fn = pic.pic_kernel_time(sim, "field")
         if fn:
+            # algorithmic bytes of a solve: rho read once, E written once (phi is not asked for here) = 16 B per node;
+            # the filter passes, the two prefix sums and the mean work on node arrays that stay in the 126 MB L2
+            f_gbs = 16.0 * (inp["nc"] + 1) / (fms / fn * 1e-3) / 1e9
             field = {"ms_per_call": fms / fn, "calls": int(fn), "nodes": inp["nc"] + 1, "smooth_passes": 2,
-                     "note": "launch-latency bound: 8-24 MB of node data, 7 small kernels"}
+                     "algorithmic_bytes_per_node": 16, "achieved": f_gbs, "unit": "GB/s", "frac": f_gbs / peak,
+                     "note": "one cooperative kernel per solve (option field_fused=1, the default; 0 = six or seven "
+                             "separate kernels); bound by its grid-wide barriers and launch latency, not by HBM: "
+                             "8-24 MB of node data that stay in L2"}
         pic.pic_set_field(sim, inp["E"])  # the workload's own field again
         # macro-particle weights small enough that the self-consistent field stays of the order of the workload's own
         # (|E| <~ 0.05) even where nothing neutralises the charge (one species between absorbing walls)
@@ -480,7 +490,13 @@ def main():
         pic.pic_cycle(sim, 2, wts, smooth_passes=2, rho=rho_c)  # warm-up
         cms = timed(lambda: pic.pic_cycle(sim, ncyc, wts, smooth_passes=2, rho=rho_c))
         cms_checked = timed(checked_calls)
+        # algorithmic bytes of a cycle per particle: the fused step's 68 (read 32, write 36) + 8 for the deposition, which
+        # reads x again (the node arrays add 16-40 B per NODE, i.e. < 1 % at 100 particles per cell)
+        cyc_bytes = ALG_BYTES["fused"][0] if expect_fused else None
+        cyc_gbs = ((cyc_bytes + DEPOSIT_BYTES) * n_per_launch * len(sim.species) / (cms * 1e-3) / 1e9) if cyc_bytes else None
         cycle = {"ms_per_cycle": cms, "cycles": ncyc, "pushes_per_s": n_per_launch * len(sim.species) / (cms * 1e-3),
+                 "algorithmic_bytes_per_particle": (cyc_bytes + DEPOSIT_BYTES) if cyc_bytes else None,
+                 "achieved": cyc_gbs, "unit": "GB/s", "frac": (cyc_gbs / peak) if cyc_gbs else None,
                  "what": "pic_cycle: push + arrange (all species), deposit, 2-pass filter, Poisson, E -- enqueued without a host "
                          "round trip; E never leaves the device",
                  "ms_per_cycle_checked_calls": cms_checked,
@@ -552,7 +568,9 @@ def main():
             line["config"]["workload"] += f" SCALED x{args.scale} (debug, not a bench value)"
         if args.debug_fast_particle is not None:
             line["config"]["workload"] += " with an injected fast particle (debug, not a bench value)"
-        if args.all_configs and world == 1:
+        # north_star asks for throughput on all five workloads: the headline run carries the other four too
+        want_all = args.all_configs or (args.config == 4 and args.scale == 1.0 and args.debug_fast_particle is None)
+        if want_all and not args.no_per_config and world == 1:
             line["per_config"] = per_config_block(args, line)
         if invalid:
             line["invalid"] = True
