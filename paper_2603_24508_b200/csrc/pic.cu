@@ -953,11 +953,24 @@ static int fused_cells_per_cta(const pic_species *s, int rows, int stages, int d
             return best;
         }
     }
+    // Species that step concurrently (inside pic_push_all each runs on a stream of its own) share the machine's CTA
+    // slots: the waves are then counted over the chunks of ALL of them, a few waves beat two full ones (the species'
+    // ramps and tails overlap), and a last wave with a little slack beats a packed one.  Measured at config 3
+    // (profiles/r03_variants.md: 57 cells, the single-species optimum, 0.5435 ms; 39 / 23 cells 0.5162 / 0.5166 ms).
+    const int conc = (s->own_stream && s->stream == s->own_stream) ? (int)sim->sp.size() : 1;
     double best_score = -1.0;
     for (int cpc = 2; cpc <= FUSED_CPC_SEARCH; ++cpc) {
         const double resident = (double)sim->sm_count * fused_ctas_per_sm(rows, cpc, stages, def);
         const double chunks = (double)((sim->nc + cpc - 1) / cpc);
-        const double score = chunks / (std::ceil(chunks / resident) * resident) * cpc / (cpc + 2.0);
+        double score;
+        if (conc == 1) {
+            score = chunks / (std::ceil(chunks / resident) * resident) * cpc / (cpc + 2.0);
+        } else {
+            const double total = chunks * conc, waves = std::ceil(total / resident);
+            double fill = total / (waves * resident);
+            if (fill > 0.97) fill = 0.97 - 0.5 * (fill - 0.97);
+            score = fill * cpc / (cpc + 2.0) * waves / (waves + 0.35);
+        }
         if (score > best_score * 1.0001) { best_score = score; best = cpc; }
     }
     return best;
