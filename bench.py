@@ -254,13 +254,15 @@ def compact(line):
 
 def per_config_block(args, own_line):
     """The five configs in one place: this run's own, and the other four measured by this script in subprocesses
-    (device-resident leg only: no e2e, no CPU baseline, no field legs), 10 timed steps after 3 warm-up steps each."""
+    (device-resident leg only: no e2e, no CPU baseline, no field legs), 10 timed steps after 3 warm-up steps each (config 1:
+    200, its full run)."""
     import subprocess
     out = {str(args.config): compact(own_line)}
     for c in (1, 2, 3, 4, 5):
         if c == args.config:
             continue
-        cmd = [sys.executable, os.path.abspath(__file__), "--config", str(c), "--steps", "10", "--warmup", "3", "--no-e2e",
+        # config 1 is its full 200 steps: at 25 us per step ten steps are a timer-resolution measurement
+        cmd = [sys.executable, os.path.abspath(__file__), "--config", str(c), "--steps", "200" if c == 1 else "10", "--warmup", "3", "--no-e2e",
                "--no-cpu", "--no-field", "--no-per-config"] + [a for o in args.option for a in ("--option", o)]
         r = subprocess.run(cmd, capture_output=True, text=True, cwd=ROOT)
         try:
